@@ -1,0 +1,172 @@
+"""CPU oracle for QLD (arXiv 1511.03390) -- TEST INFRASTRUCTURE, not part of the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs may
+import this package.  The arithmetic lives in qld_oracle.c (plain C, long double / int64, frame
+order as in PAPER.md:169); this file is the ctypes marshalling around it plus the few lines that
+express a sliding window and K references as repeated calls of the single-window definition
+("sliding sequence"; "a series of QLDs ... at different frequencies").
+It shares nothing with paper_1511_03390_b200/csrc and does not import the binding.
+
+Conventions: frame index s starts at 1; I = sum x sin
+(in-phase, the reference sinusoid), Q = sum x cos (the 90-degree shifted one);
+amplitude R = sqrt(I^2 + Q^2) with no normalisation; phase = atan2(Q, I).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qld_oracle.c")
+_SO = os.path.join(_HERE, "libqld_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile qld_oracle.c with gcc (no fast-math: long double and rounding semantics matter)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fPIC", "-shared", "-fopenmp", "-std=c11", "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        l = C.CDLL(build())
+        dp, i64, i32p, i64p, vp = C.POINTER(C.c_double), C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int64), C.c_void_p
+        l.qldo_ref_real.argtypes = [C.c_double, C.c_double, i64, i64, dp, dp]
+        l.qldo_ref_real.restype = None
+        l.qldo_ref_rational.argtypes = [i64, i64, i64, C.c_double, i64, i64, dp, dp]
+        l.qldo_ref_rational.restype = None
+        l.qldo_bin_index.argtypes = [i64, i64, i64, i64, i32p]
+        l.qldo_bin_index.restype = None
+        l.qldo_demod_f64.argtypes = [vp, C.c_int, i64, i64, i64, dp, dp, dp, dp, C.c_int]
+        l.qldo_demod_i64.argtypes = [vp, C.c_int, i64, i64, i64, i64p, i64p, i64p, i64p, C.c_int]
+        l.qldo_bins_i64.argtypes = [vp, C.c_int, i64, i64, i64, i32p, i64, i64p]
+        l.qldo_finalise.argtypes = [dp, dp, i64, C.c_double, dp, dp]
+        l.qldo_finalise.restype = None
+        l.qldo_max_threads.restype = C.c_int
+        _lib = l
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+_DT = {np.dtype(np.uint8): 0, np.dtype(np.uint16): 1, np.dtype(np.float64): 2}
+
+
+def max_threads() -> int:
+    return int(lib().qldo_max_threads())
+
+
+def ref_tables(ref: dict, s_first: int, n: int) -> Tuple[np.ndarray, np.ndarray]:
+    """sin(theta_s), cos(theta_s) for s = s_first .. s_first+n-1 as float64 arrays.
+
+    ref = {"nu": float, "num": int, "den": int, "phase": float, "phase_quarter": int}; den > 0
+    means nu == num/den exactly (angles reduced in integers)."""
+    sn = np.empty(n, dtype=np.float64)
+    cs = np.empty(n, dtype=np.float64)
+    den = int(ref.get("den", 0) or 0)
+    if den > 0:
+        lib().qldo_ref_rational(int(ref["num"]), den, int(ref.get("phase_quarter", 0)), float(ref.get("phase", 0.0)),
+                                int(s_first), int(n), _dp(sn), _dp(cs))
+    else:
+        ph = float(ref.get("phase", 0.0)) + int(ref.get("phase_quarter", 0)) * (np.pi / 2)
+        lib().qldo_ref_real(float(ref["nu"]), ph, int(s_first), int(n), _dp(sn), _dp(cs))
+    return sn, cs
+
+
+def _as_stack(frames: np.ndarray) -> Tuple[np.ndarray, int, int]:
+    f = np.ascontiguousarray(frames)
+    if f.dtype not in _DT:
+        raise TypeError(f"unsupported dtype {f.dtype}")
+    n = f.shape[0]
+    hw = int(np.prod(f.shape[1:])) if f.ndim > 1 else 1
+    return f.reshape(n, hw), n, hw
+
+
+def demod(frames: np.ndarray, sin_tab: np.ndarray, cos_tab: np.ndarray, nthreads: int = 1):
+    """I = sum_s x_s sin_s, Q = sum_s x_s cos_s per pixel (float64), for one window.
+
+    frames: [N, ...pixels]; tables: length N (entry i belongs to frames[i])."""
+    f, n, hw = _as_stack(frames)
+    assert len(sin_tab) == n and len(cos_tab) == n
+    sn = np.ascontiguousarray(sin_tab, dtype=np.float64)
+    cs = np.ascontiguousarray(cos_tab, dtype=np.float64)
+    I = np.empty(hw, dtype=np.float64)
+    Q = np.empty(hw, dtype=np.float64)
+    rc = lib().qldo_demod_f64(f.ctypes.data, _DT[f.dtype], n, hw, hw, _dp(sn), _dp(cs), _dp(I), _dp(Q), int(nthreads))
+    assert rc == 0
+    return I.reshape(frames.shape[1:]), Q.reshape(frames.shape[1:])
+
+
+def demod_int(frames: np.ndarray, isin: Sequence[int], icos: Sequence[int], nthreads: int = 1):
+    """The same sums with integer-valued reference tables, exact in int64."""
+    f, n, hw = _as_stack(frames)
+    a = np.ascontiguousarray(isin, dtype=np.int64)
+    b = np.ascontiguousarray(icos, dtype=np.int64)
+    assert len(a) == n and len(b) == n
+    I = np.empty(hw, dtype=np.int64)
+    Q = np.empty(hw, dtype=np.int64)
+    p = C.POINTER(C.c_int64)
+    rc = lib().qldo_demod_i64(f.ctypes.data, _DT[f.dtype], n, hw, hw, a.ctypes.data_as(p), b.ctypes.data_as(p),
+                              I.ctypes.data_as(p), Q.ctypes.data_as(p), int(nthreads))
+    assert rc == 0
+    return I.reshape(frames.shape[1:]), Q.reshape(frames.shape[1:])
+
+
+def bin_index(num: int, den: int, s_first: int, n: int) -> np.ndarray:
+    out = np.empty(n, dtype=np.int32)
+    lib().qldo_bin_index(int(num), int(den), int(s_first), int(n), out.ctypes.data_as(C.POINTER(C.c_int32)))
+    return out
+
+
+def bins(frames: np.ndarray, num: int, den: int, s_first: int = 1) -> np.ndarray:
+    """Phase-bin sums B[r] = sum_{s: (num*s mod den) == r} x_s, int64 [den, ...pixels]."""
+    f, n, hw = _as_stack(frames)
+    idx = bin_index(num, den, s_first, n)
+    B = np.empty((den, hw), dtype=np.int64)
+    rc = lib().qldo_bins_i64(f.ctypes.data, _DT[f.dtype], n, hw, hw, idx.ctypes.data_as(C.POINTER(C.c_int32)),
+                             int(den), B.ctypes.data_as(C.POINTER(C.c_int64)))
+    assert rc == 0
+    return B.reshape((den,) + tuple(frames.shape[1:]))
+
+
+def finalise(I: np.ndarray, Q: np.ndarray, scale: float = 1.0):
+    """amplitude = scale * sqrt(I^2 + Q^2), phase = atan2(Q, I) (0 where I = Q = 0)."""
+    i = np.ascontiguousarray(I, dtype=np.float64).reshape(-1)
+    q = np.ascontiguousarray(Q, dtype=np.float64).reshape(-1)
+    R = np.empty_like(i)
+    ph = np.empty_like(i)
+    lib().qldo_finalise(_dp(i), _dp(q), i.size, float(scale), _dp(R), _dp(ph))
+    return R.reshape(np.shape(I)), ph.reshape(np.shape(I))
+
+
+def qld(frames: np.ndarray, ref: dict, s_first: int = 1, nthreads: int = 1, scale: float = 1.0):
+    """One window, one reference: returns (I, Q, amplitude, phase); frames[i] is frame s_first+i."""
+    sn, cs = ref_tables(ref, s_first, frames.shape[0])
+    I, Q = demod(frames, sn, cs, nthreads)
+    R, ph = finalise(I, Q, scale)
+    return I * scale, Q * scale, R, ph
+
+
+def qld_multi(frames: np.ndarray, refs: Sequence[dict], s_first: int = 1, nthreads: int = 1):
+    """K references = K independent single-reference QLDs (reading G13)."""
+    return [qld(frames, r, s_first, nthreads) for r in refs]
+
+
+def qld_sliding(stream: np.ndarray, ref: dict, N: int, hop: int, nthreads: int = 1, windows: Optional[Sequence[int]] = None):
+    """Sliding sequence: window w covers absolute frames w*hop+1 .. w*hop+N and is
+    recomputed from the definition every time, references indexed by absolute frame number
+    (reading G10).  stream[i] is frame i+1.  Yields (w, I, Q, amplitude, phase)."""
+    n_win = (stream.shape[0] - N) // hop + 1
+    for w in (range(n_win) if windows is None else windows):
+        a = w * hop
+        yield (w,) + qld(stream[a:a + N], ref, s_first=a + 1, nthreads=nthreads)
