@@ -1,0 +1,195 @@
+/*
+ * qld.h -- C ABI of the B200-native quadrature lock-in discrimination (QLD) hot path.
+ *
+ * Method: arXiv 1511.03390, "Real-time quadrature lock-in discrimination imaging through
+ * scattering media".  Citations "P:<n>" are line numbers of the paper text;
+ * "G<n>" are the readings listed in DESIGN.md section 2.
+ *
+ * For every pixel p of a stack of camera frames x_s(p), s = 1..N, and every reference k:
+ *
+ *     I_k(p) = sum_s x_s(p) * sin(theta_{k,s})     in-phase sum      (G1, G5)
+ *     Q_k(p) = sum_s x_s(p) * cos(theta_{k,s})     quadrature sum
+ *     theta_{k,s} = 2*pi*nu_k*s + phase_k          nu = f_mod / f_s   (G4, G7, G8)
+ *     amplitude R_k(p) = sqrt(I_k^2 + Q_k^2)       (G2)         phase_k(p) = atan2(Q_k, I_k) (G6)
+ *
+ * No normalisation and no background removal unless asked for (G3, G9).
+ *
+ * General rules
+ *  - Every function returns a qld_status (QLD_OK = 0, errors negative) unless stated otherwise; nothing
+ *    aborts, throws or prints.  qld_last_error() gives a text for the last failure of a context.
+ *  - All work is enqueued on CUDA streams; nothing blocks the host except qld_sync(), qld_push_done(block=1),
+ *    qld_create(), qld_destroy() and the qld_read_* calls that say so.
+ *  - "host" pointers are CPU memory (pinned for truly asynchronous copies; pageable works but serialises);
+ *    "device" pointers are CUDA global memory of the current device.  The library never frees caller memory.
+ *  - Frames are frame-major: frame f of a batch starts at byte f*H*W*bytes_per_sample, rows of W samples,
+ *    no padding.  Maps are row-major [K][H][W] float32.
+ *  - One context is not thread-safe; distinct contexts are independent.
+ *  - There is no CPU fallback: without a CUDA device qld_create() fails with QLD_E_CUDA.
+ */
+#ifndef QLD_H
+#define QLD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qld_ctx qld_ctx; /* opaque; one per stream of frames */
+
+typedef enum { QLD_U8 = 0, QLD_U16 = 1 } qld_dtype;
+
+typedef enum {
+    QLD_OK = 0,
+    QLD_E_INVAL = -1,       /* bad argument (sizes < 1, nu outside (0, 0.5), hop outside 1..N, null pointer ...) */
+    QLD_E_NOMEM = -2,       /* device/host allocation failed, or caller workspace too small / misaligned */
+    QLD_E_CUDA = -3,        /* a CUDA call failed; sticky; text in qld_last_error() */
+    QLD_E_STATE = -4,       /* call not valid now: demod before N frames are stored, SLIDE before hop new frames */
+    QLD_E_OVERRUN = -5,     /* push would overwrite frames a pending window still needs / store is full */
+    QLD_E_UNSUPPORTED = -6  /* requested accumulation cannot be exact or safe for this (dtype, N, nu) */
+} qld_status;
+
+/* Accumulation (G11).
+ *  FP32     : fp32 references (fp64 sincospi of the exactly reduced angle, rounded once), fp32 FMA on
+ *             pedestal-subtracted samples (x - x_first(p), exact), pedestal term and finalise in fp64.
+ *             Parity: <= 1e-5 relative (floored at the map median).
+ *  INT_BINS : every reference must be rational (den > 0).  Phase-bin sums B_r = sum_{s: num*s mod den = r} x_s
+ *             in int32, exact; I, Q = sum_r B_r * sin/cos(2*pi*r/den + phase) in fp64.  For den = 4 and a
+ *             phase that is a multiple of pi/2 the references are integers {0, +-1} and I, Q are exact
+ *             integers ("integer-valued reference" path).  QLD_E_UNSUPPORTED if a bin could overflow int32.
+ *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds, else FP32. */
+typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2 } qld_accum;
+
+typedef enum { QLD_NORM_PAPER = 0 /* no scaling (G3) */, QLD_NORM_AMPLITUDE = 1 /* I, Q, R times 2/N */ } qld_norm;
+
+typedef enum { QLD_WHOLE = 0, QLD_SLIDE = 1 } qld_mode;
+
+/* Which maps qld_demod produces (bit mask; unrequested maps are not computed or written). */
+enum { QLD_MAP_I = 1, QLD_MAP_Q = 2, QLD_MAP_AMP = 4, QLD_MAP_PHASE = 8, QLD_MAP_ALL = 15 };
+
+typedef struct {
+    double nu;             /* f_mod/f_s in cycles per sample, 0 < nu < 0.5 (G18); ignored when den > 0 */
+    double phase;          /* reference phase in radians (G7) */
+    int64_t num, den;      /* den > 0: nu == num/den exactly, 0 < num/den < 1/2, angles reduced in integers */
+    int32_t phase_quarter; /* adds phase_quarter * pi/2 exactly */
+    int32_t reserved;
+} qld_ref;
+
+typedef struct {
+    int32_t H, W;            /* frame size in pixels, >= 1 */
+    int32_t dtype;           /* qld_dtype */
+    int32_t N;               /* window length in frames, >= 1 */
+    int32_t K;               /* number of references, 1..8 */
+    const qld_ref *refs;     /* K entries, copied by qld_create */
+    int32_t ring_frames;     /* 0: whole-window store of exactly N frames.  > 0: ring buffer for streaming,
+                                must be >= N + largest hop or push batch */
+    int32_t accum;           /* qld_accum */
+    int32_t norm;            /* qld_norm */
+    int32_t maps;            /* mask of QLD_MAP_*; 0 means QLD_MAP_ALL */
+    uint32_t max_value;      /* largest sample value the caller guarantees (0 = type maximum); used only for
+                                the INT_BINS overflow bound */
+    int32_t resync_hops;     /* SLIDE, FP32: recompute the window from the ring every this many hops (0 = never) */
+    void *workspace;         /* device memory of qld_workspace_bytes() bytes, 256-byte aligned, owned by the
+                                caller (e.g. a torch tensor) and kept alive until qld_destroy; NULL: the
+                                library allocates and frees it */
+    size_t workspace_bytes;
+    void *compute_stream;    /* cudaStream_t for kernels (e.g. torch's current stream); NULL: library creates one */
+    void *copy_stream;       /* cudaStream_t for host->device copies; NULL: library creates one */
+} qld_config;
+
+/* Size of the device workspace a context with this configuration needs (frame store or ring, reference
+ * tables, accumulators, maps).  QLD_E_INVAL / QLD_E_UNSUPPORTED as for qld_create. */
+int qld_workspace_bytes(const qld_config *cfg, size_t *bytes_out);
+
+/* Build a context: validate, carve the workspace, fill the reference tables on the device (A1; P:99,
+ * P:156 "creates tables of sine and cosine functions").  *ctx_out is NULL on failure. */
+int qld_create(const qld_config *cfg, qld_ctx **ctx_out);
+
+/* A2 ("thread T3 fetches data (raw frames)"): enqueue the copy of n_frames frames, host -> device
+ * frame store, on the copy stream, and return.  The frames get absolute indices pushed+1 .. pushed+n.
+ * The host buffer must stay unchanged until qld_push_done() reports completion.
+ * Whole-window store: QLD_E_OVERRUN once N frames are stored (qld_reset starts the next stack).
+ * Ring: QLD_E_OVERRUN if the push would overwrite a frame that a not-yet-requested window update needs;
+ * QLD_E_INVAL if n_frames < 1 or n_frames > capacity. */
+int qld_push_frames(qld_ctx *ctx, const void *host_frames, int n_frames);
+
+/* Same, for frames that are already in device memory (device -> device copy on the copy stream). */
+int qld_push_frames_device(qld_ctx *ctx, const void *device_frames, int n_frames);
+
+/* Whole-window store only: use the caller's device buffer of N frames in place (no copy).  The buffer
+ * must stay valid and unchanged while demods that use it are in flight.  Counts as N frames pushed. */
+int qld_attach_frames_device(qld_ctx *ctx, const void *device_frames);
+
+/* Have all pushes issued so far completed (host buffers reusable)?  block = 0: returns QLD_OK when done,
+ * QLD_E_STATE when still in flight.  block = 1: waits, then QLD_OK. */
+int qld_push_done(qld_ctx *ctx, int block);
+
+/* A3/A3'/A4/A5/A6: enqueue one demodulation on the compute stream; it waits (on the device) for every push
+ * issued before it.
+ *  QLD_WHOLE: the window is the most recent N frames stored (whole store: frames 1..N).  hop is ignored.
+ *  QLD_SLIDE: ring contexts only.  The first call produces window 0 (frames 1..N); each later call advances
+ *             the window by hop frames (1 <= hop <= N; window w = frames w*hop+1 .. w*hop+N for constant
+ *             hop, G10), adding the hop new frames and subtracting the hop expired ones.
+ * References are indexed by absolute frame number in both modes.
+ * QLD_E_STATE if the frames the window needs are not all pushed yet. */
+int qld_demod(qld_ctx *ctx, int mode, int hop);
+
+/* Device pointers to the maps of reference k written by the last qld_demod: row-major [H][W] float32, valid
+ * until the next qld_demod / qld_reset / qld_destroy; read them on the compute stream or after qld_sync().
+ * Any out-pointer may be NULL.  A map that was not requested in cfg.maps comes back as NULL. */
+int qld_get_maps(qld_ctx *ctx, int k, const float **I, const float **Q, const float **amp, const float **phase);
+
+/* INT_BINS only: device pointer to the exact int32 accumulators of reference k, [n_rows][H][W].  For even
+ * den the rows are the differences D_r = B_r - B_{r+den/2}, r = 0..den/2-1 (n_rows = den/2); for odd den the
+ * bins B_r (n_rows = den).  For den = 4, phase 0: D_0 = Q, D_1 = I exactly. */
+int qld_get_bins(qld_ctx *ctx, int k, const int32_t **rows, int *n_rows);
+
+/* Enqueue an asynchronous copy of one map of reference k (which = one QLD_MAP_* bit) to host memory on the
+ * compute stream, after the last demod.  Complete after qld_sync(). */
+int qld_read_map(qld_ctx *ctx, int k, int which, float *host_dst);
+
+/* The reference table the kernels use: sin and cos of theta_{k,s} for s = s_first .. s_first+n-1, as float32
+ * (FP32 accumulation) -- for inspection and tests.  Blocks until done.  Host pointers. */
+int qld_read_ref_table(qld_ctx *ctx, int k, int64_t s_first, int n, float *sin_out, float *cos_out);
+
+/* Bookkeeping (host side, never blocks): frames pushed so far, windows produced so far. */
+int qld_counters(const qld_ctx *ctx, int64_t *frames_pushed, int64_t *windows_done);
+
+int qld_sync(qld_ctx *ctx);    /* wait for both streams */
+int qld_reset(qld_ctx *ctx);   /* forget all frames and accumulators; the next push is frame 1 again */
+void qld_destroy(qld_ctx *ctx);/* waits for pending work, frees what the library allocated; NULL is a no-op */
+
+/* Text of the last error of this context ("" if none).  ctx may be NULL: text of the last failed qld_create
+ * on this thread. */
+const char *qld_last_error(const qld_ctx *ctx);
+
+/* Launch statistics for benchmarks: kernels launched by this context so far. */
+int64_t qld_kernel_launches(const qld_ctx *ctx);
+
+/* ---- synthetic input filler (not part of the method; device twin of paper_1511_03390_b200/synth.py) ---- */
+typedef struct {
+    int32_t H, W;
+    int32_t dtype;            /* qld_dtype */
+    uint32_t maxval;
+    uint64_t key;             /* noise-stream key (synth.seed_key(seed, 1)) */
+    int32_t n_terms;          /* J: number of weight maps / modulation rows, 0..8 */
+    int32_t has_disk;
+    const float *base;        /* device, [H*W] */
+    const float *weights;     /* device, [J][H*W] */
+    const double *mods;       /* device, [J][mod_stride], indexed by absolute frame s */
+    int64_t mod_stride;
+    double noise_a, noise_b;
+    int32_t disk_x0, disk_cy, disk_radius, reserved;
+    double disk_amp;
+    const double *disk_mod;   /* device, indexed by absolute frame s */
+} qld_synth_scene;
+
+/* Fill n_frames frames s_first .. s_first+n-1 into device memory `out` (frame-major) on `stream`
+ * (cudaStream_t or NULL).  Bit-identical to synth.frames(). */
+int qld_synth_fill(const qld_synth_scene *scene, int64_t s_first, int n_frames, void *out_device, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QLD_H */

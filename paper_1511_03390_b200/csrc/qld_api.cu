@@ -1,0 +1,619 @@
+// C-ABI entry points of libqld.so (include/qld.h): context, frame ingest (A2), stream/event ordering, and the
+// host-side bookkeeping of whole-window and sliding-window demodulation.  No arithmetic of the method runs on
+// the host: tables, sums and maps are all produced by the kernels in qld_tables.cu / qld_kernels.cu.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+
+#include "qld_internal.h"
+
+namespace {
+
+constexpr int N_PUSH_EVENTS = 64;
+constexpr int N_DEMOD_EVENTS = 32;
+constexpr double PI = 3.14159265358979323846;
+
+thread_local std::string g_create_error;
+
+struct DemodEvent {
+    cudaEvent_t ev;
+    int64_t oldest_read;   // oldest absolute frame index the demod reads
+    bool used;
+};
+
+}  // namespace
+
+struct qld_ctx {
+    // configuration
+    int H, W, dtype, bytes, N, K, accum, norm, maps, resync_hops;
+    int64_t HW;
+    uint32_t max_value;
+    int cap, cap_w;          // frame store capacity, weight table capacity
+    bool ring, external;     // ring buffer / frames attached by the caller
+    bool is_int;
+    int rows, rows_pad;
+    RefPlan ref[QLD_MAX_K];
+    FinParams fin;
+    // device memory
+    void *ws;
+    bool own_ws;
+    size_t ws_bytes;
+    unsigned char *frames;   // store (or attached buffer)
+    void *wtab;
+    double *cum;
+    void *acc;
+    float *ped;
+    float *mapI, *mapQ, *mapA, *mapP;
+    // streams and events
+    cudaStream_t s_comp, s_copy;
+    bool own_comp, own_copy;
+    cudaEvent_t push_ev[N_PUSH_EVENTS];
+    int push_ev_next;
+    bool push_pending;
+    DemodEvent demod_ev[N_DEMOD_EVENTS];
+    int demod_ev_next;
+    cudaEvent_t tables_ev;
+    // state
+    int64_t pushed;          // frames pushed since reset (absolute index of the newest frame)
+    int64_t windows_done;
+    bool seeded;             // sliding accumulators valid
+    int64_t win_start;       // 0-based offset a of the current window: frames a+1 .. a+N
+    int64_t hops_since_seed;
+    int64_t launches;
+    bool sticky;
+    std::string err;
+};
+
+namespace {
+
+int fail(qld_ctx *c, int code, const char *msg)
+{
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+
+int cuda_fail(qld_ctx *c, cudaError_t e, const char *what)
+{
+    char buf[256];
+    snprintf(buf, sizeof buf, "%s: %s", what, cudaGetErrorString(e));
+    if (c) { c->err = buf; c->sticky = true; } else g_create_error = buf;
+    return QLD_E_CUDA;
+}
+
+#define CU(c, call)                                              \
+    do {                                                         \
+        cudaError_t e_ = (call);                                 \
+        if (e_ != cudaSuccess) return cuda_fail((c), e_, #call); \
+    } while (0)
+
+size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int64_t gcd64(int64_t a, int64_t b) { while (b) { int64_t t = a % b; a = b; b = t; } return a; }
+
+// exact sin/cos of 2*pi*a/D for multiples of a quarter and a twelfth of a turn, libm otherwise
+void exact_sincos(int64_t a, int64_t D, double extra, double *sn, double *cs)
+{
+    a %= D;
+    if (extra == 0.0 && (4 * a) % D == 0) {
+        static const double qs[4] = {0, 1, 0, -1}, qc[4] = {1, 0, -1, 0};
+        const int j = (int)((4 * a) / D) & 3;
+        *sn = qs[j]; *cs = qc[j];
+        return;
+    }
+    const long double th = 2.0L * 3.141592653589793238462643383279502884L * ((long double)a / (long double)D) + (long double)extra;
+    long double s = sinl(th), c = cosl(th);
+    if (extra == 0.0 && (12 * a) % D == 0) {
+        const int j = (int)((12 * a) / D) % 12;
+        if (j == 1 || j == 5) s = 0.5L;
+        if (j == 7 || j == 11) s = -0.5L;
+        if (j == 2 || j == 10) c = 0.5L;
+        if (j == 4 || j == 8) c = -0.5L;
+    }
+    *sn = (double)s; *cs = (double)c;
+}
+
+struct Plan {
+    int H, W, dtype, bytes, N, K, accum, norm, maps, cap, cap_w, rows, rows_pad;
+    bool ring, external, is_int;
+    int64_t HW;
+    RefPlan ref[QLD_MAX_K];
+    FinParams fin;
+    // workspace offsets
+    size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, total;
+};
+
+int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
+{
+    auto bad = [&](int code, const char *m) { *err = m; return code; };
+    if (!cfg) return bad(QLD_E_INVAL, "config is NULL");
+    if (cfg->H < 1 || cfg->W < 1) return bad(QLD_E_INVAL, "H and W must be >= 1");
+    if (cfg->dtype != QLD_U8 && cfg->dtype != QLD_U16) return bad(QLD_E_INVAL, "dtype must be QLD_U8 or QLD_U16");
+    if (cfg->N < 1) return bad(QLD_E_INVAL, "N must be >= 1");
+    if (cfg->K < 1 || cfg->K > QLD_MAX_K || !cfg->refs) return bad(QLD_E_INVAL, "K must be 1..8 with refs given");
+    if (cfg->ring_frames < -1 || (cfg->ring_frames > 0 && cfg->ring_frames <= cfg->N))
+        return bad(QLD_E_INVAL, "ring_frames must be -1, 0, or > N");
+    if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_INT_BINS) return bad(QLD_E_INVAL, "unknown accum");
+    if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
+    if (cfg->maps & ~QLD_MAP_ALL) return bad(QLD_E_INVAL, "unknown bits in maps");
+    memset(pl, 0, sizeof *pl);
+    pl->H = cfg->H; pl->W = cfg->W; pl->dtype = cfg->dtype; pl->bytes = cfg->dtype == QLD_U8 ? 1 : 2;
+    pl->N = cfg->N; pl->K = cfg->K; pl->norm = cfg->norm; pl->maps = cfg->maps ? cfg->maps : QLD_MAP_ALL;
+    pl->HW = (int64_t)cfg->H * cfg->W;
+    pl->ring = cfg->ring_frames > 0; pl->external = cfg->ring_frames == -1;
+    pl->cap = pl->ring ? cfg->ring_frames : cfg->N;
+    pl->cap_w = pl->cap + 1;
+
+    bool all_rational = true;
+    int64_t max_den = 0;
+    for (int k = 0; k < cfg->K; ++k) {
+        const qld_ref &r = cfg->refs[k];
+        RefPlan &rp = pl->ref[k];
+        rp.phase = r.phase; rp.phase_quarter = r.phase_quarter;
+        if (!isfinite(r.phase)) return bad(QLD_E_INVAL, "phase must be finite");
+        if (r.den > 0) {
+            if (r.den >= (1ll << 31) || r.num <= 0 || 2 * r.num >= r.den) return bad(QLD_E_INVAL, "need 0 < num/den < 1/2 and den < 2^31");
+            const int64_t g = gcd64(r.num, r.den);
+            rp.num = r.num / g; rp.den = r.den / g; rp.nu = (double)rp.num / (double)rp.den;
+            if (rp.den > max_den) max_den = rp.den;
+        } else {
+            if (!(r.nu > 0.0 && r.nu < 0.5)) return bad(QLD_E_INVAL, "nu must lie in (0, 0.5)");
+            rp.nu = r.nu; rp.num = 0; rp.den = 0;
+            all_rational = false;
+        }
+    }
+    // accumulation mode
+    const uint64_t vmax = cfg->max_value ? cfg->max_value : (cfg->dtype == QLD_U8 ? 255u : 65535u);
+    auto bins_rows = [&](int *rows_out) {
+        int rows = 0;
+        for (int k = 0; k < cfg->K; ++k) {
+            const int64_t den = pl->ref[k].den;
+            rows += (int)((den % 2 == 0) ? den / 2 : den);
+        }
+        *rows_out = rows;
+        return rows <= QLD_MAX_ROWS;
+    };
+    auto bins_fit = [&]() {   // |row sum| <= vmax * (number of frames that can land in one row)
+        for (int k = 0; k < cfg->K; ++k) {
+            const int64_t den = pl->ref[k].den;
+            const int64_t per_row = ((int64_t)cfg->N + den - 1) / den * ((den % 2 == 0) ? 1 : 1);
+            // a difference row takes +x from bin r and -x from bin r+den/2: magnitude bounded by one bin's sum
+            if ((unsigned __int128)vmax * (uint64_t)(per_row + 1) >= (1ull << 31)) return false;
+        }
+        return true;
+    };
+    int acc = cfg->accum;
+    int rows = 0;
+    if (acc == QLD_ACC_AUTO) {
+        acc = (all_rational && max_den <= 16 && bins_rows(&rows) && bins_fit()) ? QLD_ACC_INT_BINS : QLD_ACC_FP32;
+    }
+    if (acc == QLD_ACC_INT_BINS) {
+        if (!all_rational) return bad(QLD_E_UNSUPPORTED, "INT_BINS needs every reference rational (den > 0)");
+        if (!bins_rows(&rows)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
+        if (!bins_fit()) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
+    }
+    pl->accum = acc;
+    pl->is_int = acc == QLD_ACC_INT_BINS;
+    FinParams &f = pl->fin;
+    f.K = cfg->K; f.is_int = pl->is_int;
+    f.scale = cfg->norm == QLD_NORM_AMPLITUDE ? 2.0 / (double)cfg->N : 1.0;
+    if (pl->is_int) {
+        int off = 0;
+        for (int k = 0; k < cfg->K; ++k) {
+            RefPlan &rp = pl->ref[k];
+            rp.use_diff = rp.den % 2 == 0;
+            rp.n_rows = (int)(rp.use_diff ? rp.den / 2 : rp.den);
+            rp.row_off = off;
+            f.row_off[k] = off; f.n_rows[k] = rp.n_rows;
+            const int64_t D = 4 * rp.den;
+            for (int r = 0; r < rp.n_rows; ++r) {
+                const int64_t a = (4 * (int64_t)r + (int64_t)((rp.phase_quarter % 4 + 4) % 4) * rp.den) % D;
+                exact_sincos(a, D, rp.phase, &f.sw[off + r], &f.cw[off + r]);
+            }
+            off += rp.n_rows;
+        }
+        pl->rows = off;
+    } else {
+        for (int k = 0; k < cfg->K; ++k) {
+            pl->ref[k].row_off = 2 * k; pl->ref[k].n_rows = 2;
+            f.row_off[k] = 2 * k; f.n_rows[k] = 2;
+        }
+        pl->rows = 2 * cfg->K;
+    }
+    pl->rows_pad = pl->rows <= 2 ? 2 : pl->rows <= 4 ? 4 : pl->rows <= 8 ? 8 : 16;
+
+    // workspace layout
+    size_t o = 0;
+    pl->off_frames = o; if (!pl->external) o += align_up((size_t)pl->cap * pl->HW * pl->bytes);
+    pl->off_wtab = o; o += align_up((size_t)pl->cap_w * pl->rows_pad * 4);
+    pl->off_cum = o; o += align_up((size_t)pl->cap_w * pl->rows_pad * 8);
+    pl->off_acc = o; o += align_up((size_t)pl->rows_pad * pl->HW * (pl->is_int ? 4 : 8));
+    pl->off_ped = o; o += align_up((size_t)pl->HW * 4);
+    const size_t map = align_up((size_t)pl->K * pl->HW * 4);
+    pl->off_I = o; if (pl->maps & QLD_MAP_I) o += map;
+    pl->off_Q = o; if (pl->maps & QLD_MAP_Q) o += map;
+    pl->off_A = o; if (pl->maps & QLD_MAP_AMP) o += map;
+    pl->off_P = o; if (pl->maps & QLD_MAP_PHASE) o += map;
+    pl->total = o;
+    return QLD_OK;
+}
+
+int fill_tables(qld_ctx *c, int64_t s_first, int n, cudaStream_t st)
+{
+    TableFillParams tp;
+    memset(&tp, 0, sizeof tp);
+    tp.K = c->K; tp.is_int = c->is_int; tp.rows = c->rows_pad;
+    for (int k = 0; k < c->K; ++k) tp.ref[k] = c->ref[k];
+    tp.s_first = s_first; tp.n = n; tp.cap_w = c->cap_w; tp.wtab = c->wtab; tp.cum = c->cum;
+    CU(c, qld_launch_table_fill(tp, st));
+    c->launches++;
+    return QLD_OK;
+}
+
+int init_device_state(qld_ctx *c)
+{
+    // tables zeroed (padding rows stay zero; cum entry of frame 0 is zero), then filled for the whole store
+    CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
+    CU(c, cudaMemsetAsync(c->cum, 0, (size_t)c->cap_w * c->rows_pad * 8, c->s_copy));
+    if (!c->ring) {
+        int rc = fill_tables(c, 1, c->N, c->s_copy);
+        if (rc) return rc;
+    }
+    CU(c, cudaEventRecord(c->tables_ev, c->s_copy));
+    CU(c, cudaStreamWaitEvent(c->s_comp, c->tables_ev, 0));
+    return QLD_OK;
+}
+
+// make the copy stream wait for demods that still read frames <= last_overwritten
+int wait_for_readers(qld_ctx *c, int64_t last_overwritten)
+{
+    int best = -1;
+    int64_t best_age = -1;
+    for (int i = 0; i < N_DEMOD_EVENTS; ++i) {
+        const int idx = (c->demod_ev_next + i) % N_DEMOD_EVENTS;   // oldest .. newest
+        if (c->demod_ev[idx].used && c->demod_ev[idx].oldest_read <= last_overwritten) { best = idx; best_age = i; }
+    }
+    (void)best_age;
+    if (best >= 0) CU(c, cudaStreamWaitEvent(c->s_copy, c->demod_ev[best].ev, 0));
+    return QLD_OK;
+}
+
+int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (!src || n < 1) return fail(c, QLD_E_INVAL, "push: null buffer or n_frames < 1");
+    if (c->external) return fail(c, QLD_E_STATE, "push: this context takes attached frames only (ring_frames = -1)");
+    if (n > c->cap) return fail(c, QLD_E_INVAL, "push: more frames than the store holds");
+    const size_t fb = (size_t)c->HW * c->bytes;
+    if (!c->ring) {
+        if (c->pushed + n > c->N) return fail(c, QLD_E_OVERRUN, "push: whole-window store already holds N frames (qld_reset first)");
+        // frames still being read by an earlier demod of the previous stack
+        int rc = wait_for_readers(c, INT64_MAX);
+        if (rc) return rc;
+        CU(c, cudaMemcpyAsync(c->frames + (size_t)c->pushed * fb, src, (size_t)n * fb, kind, c->s_copy));
+    } else {
+        const int64_t first = c->pushed + 1, last = c->pushed + n;
+        const int64_t oldest_needed = c->seeded ? c->win_start + 1 : 1;
+        if (last - c->cap >= oldest_needed) return fail(c, QLD_E_OVERRUN, "push: would overwrite frames a pending window still needs");
+        if (last - c->cap >= 1) {
+            int rc = wait_for_readers(c, last - c->cap);
+            if (rc) return rc;
+        }
+        const int slot = (int)((first - 1) % c->cap);
+        const int n1 = n < c->cap - slot ? n : c->cap - slot;
+        CU(c, cudaMemcpyAsync(c->frames + (size_t)slot * fb, src, (size_t)n1 * fb, kind, c->s_copy));
+        if (n1 < n) CU(c, cudaMemcpyAsync(c->frames, static_cast<const unsigned char *>(src) + (size_t)n1 * fb, (size_t)(n - n1) * fb, kind, c->s_copy));
+        int rc = fill_tables(c, first, n, c->s_copy);
+        if (rc) return rc;
+    }
+    c->pushed += n;
+    cudaEvent_t ev = c->push_ev[c->push_ev_next];
+    c->push_ev_next = (c->push_ev_next + 1) % N_PUSH_EVENTS;
+    CU(c, cudaEventRecord(ev, c->s_copy));
+    c->push_pending = true;
+    return QLD_OK;
+}
+
+cudaEvent_t last_push_event(qld_ctx *c) { return c->push_ev[(c->push_ev_next + N_PUSH_EVENTS - 1) % N_PUSH_EVENTS]; }
+
+FinParams fin_with_maps(const qld_ctx *c)
+{
+    FinParams f = c->fin;
+    f.I = c->mapI; f.Q = c->mapQ; f.amp = c->mapA; f.phase = c->mapP;
+    return f;
+}
+
+int record_demod(qld_ctx *c, int64_t oldest_read)
+{
+    DemodEvent &d = c->demod_ev[c->demod_ev_next];
+    c->demod_ev_next = (c->demod_ev_next + 1) % N_DEMOD_EVENTS;
+    d.oldest_read = oldest_read; d.used = true;
+    CU(c, cudaEventRecord(d.ev, c->s_comp));
+    return QLD_OK;
+}
+
+// whole-window kernel over absolute frames a+1 .. a+N; seeds the sliding accumulators when asked
+int run_whole(qld_ctx *c, int64_t a, bool seed)
+{
+    DemodParams p;
+    memset(&p, 0, sizeof p);
+    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+    p.cap = c->cap; p.slot0 = (int)(a % c->cap); p.n = c->N;
+    p.cap_w = c->cap_w; p.w0 = (int)((a + 1) % c->cap_w);
+    p.cum_lo = (int)(a % c->cap_w); p.cum_hi = (int)((a + c->N) % c->cap_w);
+    p.wtab = c->wtab; p.cum = c->cum;
+    p.acc_out = (seed || c->is_int) ? c->acc : nullptr;
+    p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
+    p.fin = fin_with_maps(c);
+    CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+    c->launches++;
+    return record_demod(c, a + 1);
+}
+
+int run_slide(qld_ctx *c, int64_t a_old, int hop)
+{
+    const int64_t a_new = a_old + hop;
+    SlideParams p;
+    memset(&p, 0, sizeof p);
+    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+    p.cap = c->cap; p.cap_w = c->cap_w; p.hop = hop;
+    p.new_slot0 = (int)((a_old + c->N) % c->cap);          // first new frame is a_old+N+1 -> slot (a_old+N) mod cap
+    p.old_slot0 = (int)(a_old % c->cap);                   // first expired frame is a_old+1
+    p.new_w0 = (int)((a_old + c->N + 1) % c->cap_w);
+    p.old_w0 = (int)((a_old + 1) % c->cap_w);
+    p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
+    p.wtab = c->wtab; p.cum = c->cum; p.acc = c->acc; p.ped = c->ped;
+    p.fin = fin_with_maps(c);
+    CU(c, qld_launch_demod_slide(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+    c->launches++;
+    return record_demod(c, a_old + 1);
+}
+
+}  // namespace
+
+extern "C" {
+
+int qld_workspace_bytes(const qld_config *cfg, size_t *bytes_out)
+{
+    Plan pl;
+    std::string err;
+    int rc = make_plan(cfg, &pl, &err);
+    if (rc) { g_create_error = err; return rc; }
+    if (!bytes_out) return fail(nullptr, QLD_E_INVAL, "bytes_out is NULL");
+    *bytes_out = pl.total;
+    return QLD_OK;
+}
+
+int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
+{
+    if (!ctx_out) return fail(nullptr, QLD_E_INVAL, "ctx_out is NULL");
+    *ctx_out = nullptr;
+    Plan pl;
+    std::string err;
+    int rc = make_plan(cfg, &pl, &err);
+    if (rc) { g_create_error = err; return rc; }
+    int ndev = 0;
+    cudaError_t ce = cudaGetDeviceCount(&ndev);
+    if (ce != cudaSuccess || ndev < 1) {
+        (void)cudaGetLastError();
+        return fail(nullptr, QLD_E_CUDA, "no CUDA device: this library has no CPU fallback");
+    }
+    qld_ctx *c = new (std::nothrow) qld_ctx();
+    if (!c) return fail(nullptr, QLD_E_NOMEM, "host allocation failed");
+    c->H = pl.H; c->W = pl.W; c->dtype = pl.dtype; c->bytes = pl.bytes; c->N = pl.N; c->K = pl.K;
+    c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops > 0 ? cfg->resync_hops : 0;
+    c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
+    c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
+    for (int k = 0; k < pl.K; ++k) c->ref[k] = pl.ref[k];
+    c->fin = pl.fin;
+    c->ws_bytes = pl.total;
+    auto cleanup = [&](int code) { qld_destroy(c); return code; };
+    if (cfg->workspace) {
+        if (cfg->workspace_bytes < pl.total || (reinterpret_cast<uintptr_t>(cfg->workspace) & 255)) {
+            delete c;
+            return fail(nullptr, QLD_E_NOMEM, "caller workspace too small or not 256-byte aligned");
+        }
+        c->ws = cfg->workspace; c->own_ws = false;
+    } else {
+        ce = cudaMalloc(&c->ws, pl.total);
+        if (ce != cudaSuccess) { (void)cudaGetLastError(); delete c; return fail(nullptr, QLD_E_NOMEM, "cudaMalloc of the workspace failed"); }
+        c->own_ws = true;
+    }
+    unsigned char *b = static_cast<unsigned char *>(c->ws);
+    c->frames = pl.external ? nullptr : b + pl.off_frames;
+    c->wtab = b + pl.off_wtab; c->cum = reinterpret_cast<double *>(b + pl.off_cum);
+    c->acc = b + pl.off_acc; c->ped = reinterpret_cast<float *>(b + pl.off_ped);
+    c->mapI = (pl.maps & QLD_MAP_I) ? reinterpret_cast<float *>(b + pl.off_I) : nullptr;
+    c->mapQ = (pl.maps & QLD_MAP_Q) ? reinterpret_cast<float *>(b + pl.off_Q) : nullptr;
+    c->mapA = (pl.maps & QLD_MAP_AMP) ? reinterpret_cast<float *>(b + pl.off_A) : nullptr;
+    c->mapP = (pl.maps & QLD_MAP_PHASE) ? reinterpret_cast<float *>(b + pl.off_P) : nullptr;
+
+    c->s_comp = static_cast<cudaStream_t>(cfg->compute_stream);
+    c->s_copy = static_cast<cudaStream_t>(cfg->copy_stream);
+    if (!c->s_comp) { if (cudaStreamCreateWithFlags(&c->s_comp, cudaStreamNonBlocking) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "stream creation failed")); c->own_comp = true; }
+    if (!c->s_copy) { if (cudaStreamCreateWithFlags(&c->s_copy, cudaStreamNonBlocking) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "stream creation failed")); c->own_copy = true; }
+    for (int i = 0; i < N_PUSH_EVENTS; ++i)
+        if (cudaEventCreateWithFlags(&c->push_ev[i], cudaEventDisableTiming) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "event creation failed"));
+    for (int i = 0; i < N_DEMOD_EVENTS; ++i) {
+        if (cudaEventCreateWithFlags(&c->demod_ev[i].ev, cudaEventDisableTiming) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "event creation failed"));
+        c->demod_ev[i].used = false;
+    }
+    if (cudaEventCreateWithFlags(&c->tables_ev, cudaEventDisableTiming) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "event creation failed"));
+    rc = init_device_state(c);
+    if (rc) { g_create_error = c->err; return cleanup(rc); }
+    ce = cudaStreamSynchronize(c->s_copy);
+    if (ce != cudaSuccess) { g_create_error = cudaGetErrorString(ce); return cleanup(QLD_E_CUDA); }
+    *ctx_out = c;
+    return QLD_OK;
+}
+
+int qld_push_frames(qld_ctx *c, const void *host_frames, int n_frames) { return push_common(c, host_frames, n_frames, cudaMemcpyHostToDevice); }
+
+int qld_push_frames_device(qld_ctx *c, const void *device_frames, int n_frames) { return push_common(c, device_frames, n_frames, cudaMemcpyDeviceToDevice); }
+
+int qld_attach_frames_device(qld_ctx *c, const void *device_frames)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (!device_frames) return fail(c, QLD_E_INVAL, "attach: null buffer");
+    if (c->ring) return fail(c, QLD_E_STATE, "attach: ring contexts copy their frames (use qld_push_frames_device)");
+    c->frames = const_cast<unsigned char *>(static_cast<const unsigned char *>(device_frames));
+    c->pushed = c->N;
+    return QLD_OK;
+}
+
+int qld_push_done(qld_ctx *c, int block)
+{
+    if (!c) return QLD_E_INVAL;
+    if (!c->push_pending) return QLD_OK;
+    cudaEvent_t ev = last_push_event(c);
+    if (block) { CU(c, cudaEventSynchronize(ev)); c->push_pending = false; return QLD_OK; }
+    cudaError_t e = cudaEventQuery(ev);
+    if (e == cudaSuccess) { c->push_pending = false; return QLD_OK; }
+    if (e == cudaErrorNotReady) return QLD_E_STATE;
+    return cuda_fail(c, e, "cudaEventQuery");
+}
+
+int qld_demod(qld_ctx *c, int mode, int hop)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (mode != QLD_WHOLE && mode != QLD_SLIDE) return fail(c, QLD_E_INVAL, "demod: unknown mode");
+    if (!c->frames) return fail(c, QLD_E_STATE, "demod: no frames attached");
+    if (c->push_pending || c->pushed > 0) CU(c, cudaStreamWaitEvent(c->s_comp, last_push_event(c), 0));
+    if (mode == QLD_WHOLE) {
+        if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames stored");
+        const int64_t a = c->ring ? c->pushed - c->N : 0;
+        int rc = run_whole(c, a, c->ring);
+        if (rc) return rc;
+        if (c->ring) { c->seeded = true; c->win_start = a; c->hops_since_seed = 0; }
+        c->windows_done++;
+        return QLD_OK;
+    }
+    if (!c->ring) return fail(c, QLD_E_STATE, "demod: QLD_SLIDE needs a ring context (ring_frames > N)");
+    if (!c->seeded) {
+        if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames pushed");
+        int rc = run_whole(c, 0, true);
+        if (rc) return rc;
+        c->seeded = true; c->win_start = 0; c->hops_since_seed = 0; c->windows_done++;
+        return QLD_OK;
+    }
+    if (hop < 1 || hop > c->N) return fail(c, QLD_E_INVAL, "demod: hop must be 1..N");
+    if (c->pushed < c->win_start + hop + c->N) return fail(c, QLD_E_STATE, "demod: fewer than hop new frames pushed");
+    int rc;
+    if (!c->is_int && c->resync_hops > 0 && c->hops_since_seed + 1 >= c->resync_hops) {
+        rc = run_whole(c, c->win_start + hop, true);
+        c->hops_since_seed = 0;
+    } else {
+        rc = run_slide(c, c->win_start, hop);
+        c->hops_since_seed++;
+    }
+    if (rc) return rc;
+    c->win_start += hop;
+    c->windows_done++;
+    return QLD_OK;
+}
+
+int qld_get_maps(qld_ctx *c, int k, const float **I, const float **Q, const float **amp, const float **phase)
+{
+    if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "get_maps: k out of range") : QLD_E_INVAL;
+    const size_t o = (size_t)k * c->HW;
+    if (I) *I = c->mapI ? c->mapI + o : nullptr;
+    if (Q) *Q = c->mapQ ? c->mapQ + o : nullptr;
+    if (amp) *amp = c->mapA ? c->mapA + o : nullptr;
+    if (phase) *phase = c->mapP ? c->mapP + o : nullptr;
+    return QLD_OK;
+}
+
+int qld_get_bins(qld_ctx *c, int k, const int32_t **rows, int *n_rows)
+{
+    if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "get_bins: k out of range") : QLD_E_INVAL;
+    if (!c->is_int) return fail(c, QLD_E_STATE, "get_bins: context does not accumulate integer bins");
+    if (rows) *rows = static_cast<const int32_t *>(c->acc) + (size_t)c->ref[k].row_off * c->HW;
+    if (n_rows) *n_rows = c->ref[k].n_rows;
+    return QLD_OK;
+}
+
+int qld_read_map(qld_ctx *c, int k, int which, float *host_dst)
+{
+    if (!c || !host_dst || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "read_map: bad argument") : QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    const float *src = which == QLD_MAP_I ? c->mapI : which == QLD_MAP_Q ? c->mapQ : which == QLD_MAP_AMP ? c->mapA : which == QLD_MAP_PHASE ? c->mapP : nullptr;
+    if (!src) return fail(c, QLD_E_INVAL, "read_map: map not produced by this context");
+    CU(c, cudaMemcpyAsync(host_dst, src + (size_t)k * c->HW, (size_t)c->HW * 4, cudaMemcpyDeviceToHost, c->s_comp));
+    return QLD_OK;
+}
+
+int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out, float *cos_out)
+{
+    if (!c || k < 0 || k >= c->K || n < 1 || s_first < 1) return c ? fail(c, QLD_E_INVAL, "read_ref_table: bad argument") : QLD_E_INVAL;
+    if (c->is_int) return fail(c, QLD_E_STATE, "read_ref_table: integer-bin contexts have no float table");
+    if (c->ring && (s_first + n - 1 > c->pushed || s_first + c->cap_w <= c->pushed + 1)) return fail(c, QLD_E_STATE, "read_ref_table: frames not in the ring");
+    if (!c->ring && s_first + n - 1 > c->N) return fail(c, QLD_E_INVAL, "read_ref_table: beyond the window");
+    CU(c, cudaStreamSynchronize(c->s_copy));
+    for (int i = 0; i < n; ++i) {
+        const int64_t e = (s_first + i) % c->cap_w;
+        float w[2];
+        CU(c, cudaMemcpy(w, static_cast<const float *>(c->wtab) + e * c->rows_pad + 2 * k, sizeof w, cudaMemcpyDeviceToHost));
+        if (sin_out) sin_out[i] = w[0];
+        if (cos_out) cos_out[i] = w[1];
+    }
+    return QLD_OK;
+}
+
+int qld_counters(const qld_ctx *c, int64_t *frames_pushed, int64_t *windows_done)
+{
+    if (!c) return QLD_E_INVAL;
+    if (frames_pushed) *frames_pushed = c->pushed;
+    if (windows_done) *windows_done = c->windows_done;
+    return QLD_OK;
+}
+
+int qld_sync(qld_ctx *c)
+{
+    if (!c) return QLD_E_INVAL;
+    CU(c, cudaStreamSynchronize(c->s_copy));
+    CU(c, cudaStreamSynchronize(c->s_comp));
+    c->push_pending = false;
+    return QLD_OK;
+}
+
+int qld_reset(qld_ctx *c)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    int rc = qld_sync(c);
+    if (rc) return rc;
+    c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
+    for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
+    if (c->external) c->frames = nullptr;
+    if (c->ring) {
+        rc = init_device_state(c);
+        if (rc) return rc;
+    }
+    return QLD_OK;
+}
+
+void qld_destroy(qld_ctx *c)
+{
+    if (!c) return;
+    if (c->s_copy) cudaStreamSynchronize(c->s_copy);
+    if (c->s_comp) cudaStreamSynchronize(c->s_comp);
+    for (int i = 0; i < N_PUSH_EVENTS; ++i) if (c->push_ev[i]) cudaEventDestroy(c->push_ev[i]);
+    for (int i = 0; i < N_DEMOD_EVENTS; ++i) if (c->demod_ev[i].ev) cudaEventDestroy(c->demod_ev[i].ev);
+    if (c->tables_ev) cudaEventDestroy(c->tables_ev);
+    if (c->own_comp && c->s_comp) cudaStreamDestroy(c->s_comp);
+    if (c->own_copy && c->s_copy) cudaStreamDestroy(c->s_copy);
+    if (c->own_ws && c->ws) cudaFree(c->ws);
+    (void)cudaGetLastError();
+    delete c;
+}
+
+const char *qld_last_error(const qld_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int64_t qld_kernel_launches(const qld_ctx *c) { return c ? c->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,82 @@
+// Internal declarations shared by the translation units of libqld.so (product side only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "qld.h"
+
+#define QLD_MAX_K 8
+#define QLD_MAX_ROWS 16
+
+// How one reference maps onto rows of the weight table.
+//  FP32     : 2 rows (sin, cos), float weights.
+//  INT_BINS : n_rows rows of int weights in {0, +1, -1}; I = sum_r row_r * sw[r], Q = sum_r row_r * cw[r].
+struct RefPlan {
+    double nu, phase;
+    int64_t num, den;
+    int32_t phase_quarter;
+    int32_t row_off, n_rows;
+    int32_t use_diff;  // even den: rows are B_r - B_{r+den/2}
+};
+
+// Epilogue (A4) parameters, passed by value to the kernels.
+struct FinParams {
+    int32_t K;
+    int32_t is_int;          // 1: rows are int32 bins, combine with sw/cw;  0: row_off = I sum, row_off+1 = Q sum
+    int32_t row_off[QLD_MAX_K];
+    int32_t n_rows[QLD_MAX_K];
+    double sw[QLD_MAX_ROWS]; // per row: sin(2 pi r/den + phase)
+    double cw[QLD_MAX_ROWS];
+    double scale;            // 1 (PAPER) or 2/N (AMPLITUDE)
+    float *I, *Q, *amp, *phase;   // [K][HW] or null
+};
+
+// One demodulation launch (whole window, ring aware).
+struct DemodParams {
+    const void *frames;      // frame store base
+    int64_t frame_stride;    // bytes between frames
+    int64_t HW;
+    int32_t cap;             // frame store capacity (frames); slot of frame s is (s-1) mod cap
+    int32_t slot0;           // slot of the first frame of the window
+    int32_t n;               // frames in the window
+    int32_t cap_w;           // weight table capacity; entry of frame s is s mod cap_w
+    int32_t w0;              // weight entry of the first frame
+    int32_t cum_lo, cum_hi;  // weight entries of frame (first-1) and of the last frame, for the pedestal sums
+    const void *wtab;        // [cap_w][ROWS] float or int32
+    const double *cum;       // [cap_w][ROWS] running sums of the float weights (FP32 only)
+    void *acc_out;           // optional [ROWS][HW]: double (FP32: pedestal-subtracted sums) or int32 (bins)
+    float *ped_out;          // optional [HW] pedestal used (FP32)
+    FinParams fin;
+};
+
+// One sliding update launch (A5).
+struct SlideParams {
+    const void *frames;
+    int64_t frame_stride;
+    int64_t HW;
+    int32_t cap, cap_w;
+    int32_t new_slot0, old_slot0;   // slots of the first new / first expired frame
+    int32_t new_w0, old_w0;         // weight entries of the same
+    int32_t hop;
+    int32_t cum_lo, cum_hi;         // entries of frame (window first - 1) and window last, after the update
+    const void *wtab;
+    const double *cum;
+    void *acc;                      // [ROWS][HW] double or int32, read-modify-write
+    const float *ped;               // [HW] (FP32)
+    FinParams fin;
+};
+
+struct TableFillParams {
+    int32_t K, is_int, rows;        // rows = padded row count (table row stride)
+    RefPlan ref[QLD_MAX_K];
+    int64_t s_first;
+    int32_t n, cap_w;
+    void *wtab;
+    double *cum;
+};
+
+// launchers (return cudaError_t of the launch)
+cudaError_t qld_launch_demod_whole(int dtype, int is_int, int rows, const DemodParams &p, cudaStream_t st);
+cudaError_t qld_launch_demod_slide(int dtype, int is_int, int rows, const SlideParams &p, cudaStream_t st);
+cudaError_t qld_launch_table_fill(const TableFillParams &p, cudaStream_t st);
+int qld_pixels_per_thread(int dtype, int rows, int64_t HW, const void *frames, int64_t frame_stride);

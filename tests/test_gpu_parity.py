@@ -1,0 +1,299 @@
+"""GPU parity: the CUDA path behind the C ABI against the CPU oracle, element by element, on the same bytes.
+
+Bars (BASELINE.json north_star): integer paths bit-exact; float paths within 1e-5 relative (floored at the
+map median).  Every call goes through paper_1511_03390_b200.qld (ctypes -> libqld.so).
+"""
+import numpy as np
+import pytest
+
+from _parity import check_float_maps, oracle_maps
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def Q():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_1511_03390_b200 import qld
+    qld.load_library()          # raises if libqld.so is missing: no fallback
+    return qld
+
+
+def _maps(ctx, k=0):
+    return tuple(None if m is None else m.cpu().numpy() for m in ctx.get_maps(k))
+
+
+def _rand_stack(rng, N, H, W, dtype, hi=None):
+    hi = hi or (256 if dtype == np.uint8 else 4096)
+    base = rng.integers(hi // 4, hi // 2, size=(1, H, W))
+    return np.clip(base + rng.normal(0, hi / 64, size=(N, H, W)), 0, hi - 1).astype(dtype)
+
+
+# ------------------------------------------------------------------------------------------------ A1
+@pytest.mark.parametrize("ref", [{"nu": 0.0937}, {"nu": 0.31, "phase": 1.1}, {"num": 1, "den": 6},
+                                 {"num": 3, "den": 16, "phase_quarter": 1}])
+def test_reference_tables_match_oracle(Q, oracle, ref):
+    N = 300
+    ctx = Q.QLD(4, 4, "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+    sn, cs = ctx.read_ref_table(0, 1, N)
+    osn, ocs = oracle.ref_tables(ref, 1, N)
+    # fp64 sincospi of an exactly reduced angle, rounded once to fp32: at most 1 ulp from the rounded oracle value
+    assert np.abs(sn.astype(np.float64) - osn).max() <= 2.0 ** -24 * 1.01
+    assert np.abs(cs.astype(np.float64) - ocs).max() <= 2.0 ** -24 * 1.01
+    assert (sn == osn.astype(np.float32)).mean() > 0.99 and (cs == ocs.astype(np.float32)).mean() > 0.99
+    ctx.destroy()
+
+
+def test_reference_tables_deep_in_a_stream(Q, oracle):
+    """Ring context: tables are filled per push by absolute frame index; check around frame 10^5."""
+    N, cap, H, W = 8, 64, 2, 8
+    ref = {"nu": 0.0937, "phase": 0.2}
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_FP32)
+    z = np.zeros((32, H, W), np.uint16)
+    pushed = 0
+    while pushed < 100000:
+        ctx.push_frames(z)
+        pushed += 32
+        if pushed % 32 == 0:
+            ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    sn, cs = ctx.read_ref_table(0, pushed - 31, 32)
+    osn, ocs = oracle.ref_tables(ref, pushed - 31, 32)
+    assert np.abs(sn - osn).max() < 1e-7 and np.abs(cs - ocs).max() < 1e-7
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ A3 / A4 / A6
+@pytest.mark.parametrize("H,W", [(1, 1), (3, 17), (17, 3), (64, 64), (5, 48)])
+@pytest.mark.parametrize("N", [1, 2, 5, 63, 64, 65, 200])
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
+def test_whole_window_fp32_shapes(Q, oracle, H, W, N, dtype):
+    rng = np.random.default_rng(H * 1000 + W * 10 + N)
+    x = _rand_stack(rng, N, H, W, dtype)
+    ref = {"nu": 0.0937, "phase": 0.3}
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), what=f"{H}x{W} N={N}")
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 8])
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
+def test_multi_reference_equals_single_runs(Q, oracle, K, dtype):
+    """A6 / G13: K references on shared loads == K independent QLDs."""
+    rng = np.random.default_rng(K)
+    H, W, N = 24, 40, 130
+    x = _rand_stack(rng, N, H, W, dtype)
+    refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FP32)
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    for k in range(K):
+        check_float_maps(_maps(ctx, k), oracle_maps(oracle, x, refs[k]), what=f"K={K} k={k}")
+    ctx.destroy()
+
+
+def test_normalisation_and_map_selection(Q, oracle):
+    rng = np.random.default_rng(3)
+    H, W, N = 16, 32, 64
+    x = _rand_stack(rng, N, H, W, np.uint16)
+    ref = {"nu": 0.125}
+    ctx = Q.QLD(H, W, "u16", N, [ref], accum=Q.QLD_ACC_FP32, norm=Q.QLD_NORM_AMPLITUDE, maps=Q.QLD_MAP_AMP)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    I, Qm, A, P = _maps(ctx)
+    assert I is None and Qm is None and P is None
+    check_float_maps((None, None, A, None), oracle_maps(oracle, x, ref, scale=2.0 / N))
+    ctx.destroy()
+
+
+def test_closed_form_tone_on_gpu(Q):
+    """A pure 100-count tone on a 1000-count pedestal at nu = 1/8, N = 256: R = A N/2 = 12800, phase = phi."""
+    N, H, W = 256, 4, 16
+    s = np.arange(1, N + 1)[:, None, None]
+    phi = np.linspace(-3, 3, H * W).reshape(1, H, W)
+    x = np.rint(1000 + 100 * np.sin(2 * np.pi * s / 8 + phi)).astype(np.uint16)
+    ctx = Q.QLD(H, W, "u16", N, [{"num": 1, "den": 8}], accum=Q.QLD_ACC_FP32)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    I, Qm, A, P = _maps(ctx)
+    assert np.abs(A - 12800).max() < 12800 * 2e-3          # rounding of the samples to integers, not the GPU
+    assert np.abs(np.remainder(P - phi[0] + np.pi, 2 * np.pi) - np.pi).max() < 3e-3
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ A3' integer paths
+@pytest.mark.parametrize("dtype,hi", [(np.uint8, 256), (np.uint16, 65536)])
+@pytest.mark.parametrize("H,W,N", [(64, 64, 64), (3, 17, 65), (16, 48, 1000)])
+def test_quarter_rate_integer_reference_bit_exact(Q, oracle, dtype, hi, H, W, N):
+    """nu = 1/4, phase 0: references are {0, +-1}; I, Q and the amplitude are bit-exact."""
+    rng = np.random.default_rng(N)
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    ref = {"num": 1, "den": 4}
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_INT_BINS)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    sn, cs = oracle.ref_tables(ref, 1, N)
+    oI, oQ = oracle.demod_int(x, sn.astype(np.int64), cs.astype(np.int64))
+    I, Qm, A, P = _maps(ctx)
+    assert np.array_equal(I, oI.astype(np.float32)) and np.array_equal(Qm, oQ.astype(np.float32))
+    p2 = (oI * oI + oQ * oQ)
+    assert p2.max() < 2 ** 53
+    assert np.array_equal(A, np.sqrt(p2.astype(np.float64)).astype(np.float32))
+    bins = ctx.get_bins(0).cpu().numpy()
+    assert np.array_equal(bins[0], oQ) and np.array_equal(bins[1], oI)       # D_0 = Q, D_1 = I (include/qld.h)
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("num,den", [(1, 6), (1, 8), (2, 5), (3, 16), (1, 3)])
+def test_phase_bins_bit_exact(Q, oracle, num, den):
+    rng = np.random.default_rng(den)
+    H, W, N = 20, 24, 257
+    x = rng.integers(0, 4096, size=(N, H, W)).astype(np.uint16)
+    ref = {"num": num, "den": den, "phase": 0.0}
+    ctx = Q.QLD(H, W, "u16", N, [ref], accum=Q.QLD_ACC_INT_BINS, max_value=4095)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    B = oracle.bins(x, num, den)
+    bins = ctx.get_bins(0).cpu().numpy()
+    if den % 2 == 0:
+        assert np.array_equal(bins, B[:den // 2] - B[den // 2:])
+    else:
+        assert np.array_equal(bins, B)
+    # maps: fp64 combination of exact integers, stored as fp32: 1e-6 relative to the map scale
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), rel=1e-6, what=f"bins {num}/{den}")
+    ctx.destroy()
+
+
+def test_auto_picks_bins_for_small_rational_and_fp32_otherwise(Q):
+    a = Q.QLD(8, 8, "u8", 64, [{"num": 1, "den": 4}])
+    b = Q.QLD(8, 8, "u16", 64, [{"nu": 0.0937}])
+    x = np.zeros((64, 8, 8), np.uint8)
+    a.push_frames(x); a.demod(); a.sync()
+    assert a.get_bins(0).shape[0] == 2
+    with pytest.raises(Q.QLDError):
+        b.get_bins(0)
+    a.destroy(); b.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ A5 sliding window
+@pytest.mark.parametrize("accum_name", ["INT_BINS", "FP32"])
+@pytest.mark.parametrize("hop,cap", [(8, 72), (8, 77), (5, 70), (64, 130)])
+def test_sliding_equals_direct_recompute(Q, oracle, accum_name, hop, cap):
+    """Every window equals the oracle's direct recomputation; ring wrap-around, hop not dividing the ring,
+    partial pushes; the bins path is bit-exact at every hop."""
+    rng = np.random.default_rng(hop + cap)
+    H, W, N, T = 12, 16, 64, 400
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    ref = {"num": 1, "den": 6}
+    accum = getattr(Q, "QLD_ACC_" + accum_name)
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=accum, max_value=4095)
+    pushed, w = 0, 0
+    batch = 3 if hop == 5 else hop                         # pushes need not align with hops
+    while True:
+        # push as much as the ring allows, in `batch`-sized pieces
+        while pushed + batch <= T:
+            try:
+                ctx.push_frames(stream[pushed:pushed + batch])
+                pushed += batch
+            except Q.QLDError as e:
+                assert e.status == Q.QLD_E_OVERRUN
+                break
+        try:
+            ctx.demod(Q.QLD_SLIDE, hop)
+        except Q.QLDError as e:
+            assert e.status == Q.QLD_E_STATE
+            break
+        ctx.sync()
+        a = w * hop
+        ora = oracle_maps(oracle, stream[a:a + N], ref, s_first=a + 1)
+        if accum_name == "INT_BINS":
+            B = oracle.bins(stream[a:a + N], 1, 6, s_first=a + 1)
+            assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:3] - B[3:]), f"window {w}"
+            check_float_maps(_maps(ctx), ora, rel=1e-6, what=f"window {w}")
+        else:
+            check_float_maps(_maps(ctx), ora, what=f"window {w}")
+        w += 1
+    assert pushed + batch > T and w == (pushed - N) // hop + 1
+    ctx.destroy()
+
+
+def test_sliding_fp32_real_nu_with_resync(Q, oracle):
+    rng = np.random.default_rng(77)
+    H, W, N, hop, T = 8, 32, 128, 16, 1024
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    ref = {"nu": 0.0937}
+    for resync in (0, 7):
+        ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=N + 2 * hop, accum=Q.QLD_ACC_FP32, resync_hops=resync)
+        ctx.push_frames(stream[:N])
+        ctx.demod(Q.QLD_SLIDE, hop)
+        for w in range(1, (T - N) // hop + 1):
+            ctx.push_frames(stream[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+            if w % 9 == 0 or w == (T - N) // hop:
+                ctx.sync()
+                check_float_maps(_maps(ctx), oracle_maps(oracle, stream[w * hop:w * hop + N], ref, s_first=w * hop + 1),
+                                 what=f"resync={resync} window {w}")
+        ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ boundary behaviour on the device
+def test_state_errors_reset_and_attach(Q, oracle):
+    import torch
+    H, W, N = 8, 16, 32
+    rng = np.random.default_rng(1)
+    x = _rand_stack(rng, N, H, W, np.uint16)
+    ref = {"nu": 0.2}
+    ctx = Q.QLD(H, W, "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.demod()
+    assert e.value.status == Q.QLD_E_STATE
+    ctx.push_frames(x[:10])                                   # partial pushes
+    with pytest.raises(Q.QLDError):
+        ctx.demod()
+    ctx.push_frames(x[10:])
+    with pytest.raises(Q.QLDError) as e:
+        ctx.push_frames(x[:1])                                # store full
+    assert e.value.status == Q.QLD_E_OVERRUN
+    with pytest.raises(Q.QLDError) as e:
+        ctx.demod(Q.QLD_SLIDE, 4)                             # not a ring context
+    assert e.value.status == Q.QLD_E_STATE
+    ctx.demod(); ctx.sync()
+    first = _maps(ctx)
+    assert ctx.counters() == (N, 1) and ctx.kernel_launches() >= 2
+    ctx.reset()
+    assert ctx.counters() == (0, 0)
+    pinned = torch.from_numpy(x[::-1].copy()).pin_memory()    # pinned host buffer, reversed stack
+    ctx.push_frames(pinned)
+    assert ctx.push_done(block=True)
+    ctx.demod(); ctx.sync()
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x[::-1].copy(), ref))
+    # attach a device stack in place
+    ctx.reset()
+    dev = torch.from_numpy(x).cuda()
+    ctx.attach_frames_device(dev)
+    ctx.demod(); ctx.sync()
+    again = _maps(ctx)
+    assert all(np.array_equal(a, b) for a, b in zip(first, again))      # same bytes, same kernel: deterministic
+    host = torch.empty((H, W), dtype=torch.float32).pin_memory()
+    ctx.read_map(0, Q.QLD_MAP_AMP, host); ctx.sync()
+    assert np.array_equal(host.numpy(), again[2])
+    ctx.destroy(); ctx.destroy()                                         # double destroy is a no-op
+
+
+def test_device_generator_is_bit_identical_to_numpy(Q):
+    from paper_1511_03390_b200 import synth
+    for wl in (synth.cfg0(), synth.cfg1(H=60, W=80, N=16), synth.cfg2(H=64, W=80, N=16),
+               synth.cfg3(H=64, W=64, n_stream=48, N=16, hop=4, batch=4), synth.cfg4(H=64, W=64, N=16)):
+        n = min(16, wl.scene.n_frames)
+        dev = Q.synth_fill(wl.scene, 3 if wl.scene.n_frames > 20 else 1, n)
+        host = synth.frames(wl.scene, 3 if wl.scene.n_frames > 20 else 1, n)
+        assert np.array_equal(dev.cpu().numpy(), host), wl.name
