@@ -82,8 +82,10 @@ typedef struct {
     int32_t N;               /* window length in frames, >= 1 */
     int32_t K;               /* number of references, 1..8 */
     const qld_ref *refs;     /* K entries, copied by qld_create */
-    int32_t ring_frames;     /* 0: whole-window store of exactly N frames.  > 0: ring buffer for streaming,
-                                must be >= N + largest hop or push batch */
+    int32_t ring_frames;     /* 0: whole-window store of exactly N frames.  > 0: ring buffer for streaming (P:181-183),
+                                must be > N; a producer pushing batches of b frames and a consumer sliding by hop
+                                never stall each other when ring_frames >= N + hop + b - 1.
+                                -1: no store: frames are attached with qld_attach_frames_device */
     int32_t accum;           /* qld_accum */
     int32_t norm;            /* qld_norm */
     int32_t maps;            /* mask of QLD_MAP_*; 0 means QLD_MAP_ALL */

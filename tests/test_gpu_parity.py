@@ -123,8 +123,10 @@ def test_closed_form_tone_on_gpu(Q):
     ctx.demod()
     ctx.sync()
     I, Qm, A, P = _maps(ctx)
-    assert np.abs(A - 12800).max() < 12800 * 2e-3          # rounding of the samples to integers, not the GPU
-    assert np.abs(np.remainder(P - phi[0] + np.pi, 2 * np.pi) - np.pi).max() < 3e-3
+    # the samples are rounded to integers and the rounding error repeats with the 8-sample period, so it adds
+    # coherently: up to 0.5 * N/2 = 64 counts (0.5 %), not the GPU's doing
+    assert np.abs(A - 12800).max() < 64.5
+    assert np.abs(np.remainder(P - phi[0] + np.pi, 2 * np.pi) - np.pi).max() < 64.5 / 12800
     ctx.destroy()
 
 
@@ -186,7 +188,7 @@ def test_auto_picks_bins_for_small_rational_and_fp32_otherwise(Q):
 
 # ------------------------------------------------------------------------------------------------ A5 sliding window
 @pytest.mark.parametrize("accum_name", ["INT_BINS", "FP32"])
-@pytest.mark.parametrize("hop,cap", [(8, 72), (8, 77), (5, 70), (64, 130)])
+@pytest.mark.parametrize("hop,cap", [(8, 72), (8, 77), (5, 71), (64, 130)])   # cap >= N + hop + batch - 1
 def test_sliding_equals_direct_recompute(Q, oracle, accum_name, hop, cap):
     """Every window equals the oracle's direct recomputation; ring wrap-around, hop not dividing the ring,
     partial pushes; the bins path is bit-exact at every hop."""
