@@ -128,7 +128,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
-    ap.add_argument("--accum", default="auto", choices=["auto", "fp32", "bins"])
+    ap.add_argument("--accum", default="auto", choices=["auto", "fp32", "bins", "fixed"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-rows", type=int, default=0, help="rows of the frame the CPU oracle is timed / checked on "
                     "(0: sized for about 15 CPU-seconds of oracle work; 32 for --impl reference)")
@@ -158,7 +158,7 @@ def main():
     sc = wl.scene
     N, H, W, K = wl.N, sc.H, sc.W, len(wl.refs)
     bytes_per = 1 if sc.dtype == "u8" else 2
-    accum = {"auto": qld.QLD_ACC_AUTO, "fp32": qld.QLD_ACC_FP32, "bins": qld.QLD_ACC_INT_BINS}[args.accum]
+    accum = {"auto": qld.QLD_ACC_AUTO, "fp32": qld.QLD_ACC_FP32, "bins": qld.QLD_ACC_INT_BINS, "fixed": qld.QLD_ACC_FIXED}[args.accum]
 
     # ---- inputs: synthetic stack filled on the device, resident before the timed region -------------
     frames = qld.synth_fill(sc, 1, N, device=dev)
@@ -221,7 +221,7 @@ def main():
             traffic = None
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": algo_bytes,
-                "frac_of_nominal_8TBps": achieved / 8000.0, "kernel": "k_demod_whole"}
+                "frac_of_nominal_8TBps": achieved / 8000.0, "kernel": "k_demod_tc" if args.accum == "fixed" else "k_demod_whole"}
 
     # ---- end to end through host buffers (pinned): push + demod + read amplitude map back ------------
     e2e = None
@@ -289,9 +289,9 @@ def main():
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "int32 (phase bins)" if is_int else "f32", "data": "synthetic",
+                "dtype": "int32 (phase bins)" if is_int else ("int8 x int8 -> int32/int64 (tcgen05, Q1.30 references)" if args.accum == "fixed" else "f32"), "data": "synthetic",
                 "config": {"workload": args.workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype,
-                           "accum": "INT_BINS" if is_int else "FP32 (pedestal)", "maps": "I,Q,amplitude,phase",
+                           "accum": "INT_BINS" if is_int else ("FIXED (tensor cores)" if args.accum == "fixed" else "FP32 (pedestal)"), "maps": "I,Q,amplitude,phase",
                            "cache": f"input {samples_per_step * bytes_per / 1e6:.0f} MB per step "
                                     + ("> 126 MB L2: no flush needed" if samples_per_step * bytes_per > 3e8 else "<= L2: L2-resident, not an HBM number"),
                            "parallelism": f"{world} x independent stacks (pixels are independent; no collective)"},

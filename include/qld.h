@@ -58,15 +58,22 @@ typedef enum {
  *             in int32, exact; I, Q = sum_r B_r * sin/cos(2*pi*r/den + phase) in fp64.  For den = 4 and a
  *             phase that is a multiple of pi/2 the references are integers {0, +-1} and I, Q are exact
  *             integers ("integer-valued reference" path).  QLD_E_UNSUPPORTED if a bin could overflow int32.
+ *  FIXED    : fixed-point references R(s) = rint(2^30 * sin/cos(theta_s)) (Q1.30 integers; the table can also
+ *             be supplied, qld_set_ref_table_fixed).  I*2^30 = sum_s x_s R_sin(s), Q likewise, exact in int64:
+ *             computed on the tcgen05 tensor cores as a [pixel bytes x frames].[frames x reference digits]
+ *             int8 contraction (A6).  Bit-exact against an integer oracle with the same
+ *             table; |R*2^-30 - sin| <= 2^-31, so the maps also agree with the float definition to ~1e-9.
+ *             Whole-window stores only (ring_frames 0 or -1), H*W*bytes a multiple of 16, N <= 65536.
  *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds, else FP32. */
-typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2 } qld_accum;
+typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2, QLD_ACC_FIXED = 3 } qld_accum;
 
 typedef enum { QLD_NORM_PAPER = 0 /* no scaling (G3) */, QLD_NORM_AMPLITUDE = 1 /* I, Q, R times 2/N */ } qld_norm;
 
 typedef enum { QLD_WHOLE = 0, QLD_SLIDE = 1 } qld_mode;
 
 /* Which maps qld_demod produces (bit mask; unrequested maps are not computed or written). */
-enum { QLD_MAP_I = 1, QLD_MAP_Q = 2, QLD_MAP_AMP = 4, QLD_MAP_PHASE = 8, QLD_MAP_ALL = 15 };
+enum { QLD_MAP_I = 1, QLD_MAP_Q = 2, QLD_MAP_AMP = 4, QLD_MAP_PHASE = 8, QLD_MAP_ALL = 15,
+       QLD_MAP_SUMS_I64 = 16 /* FIXED only: also keep the exact int64 sums, see qld_get_sums_i64 */ };
 
 typedef struct {
     double nu;             /* f_mod/f_s in cycles per sample, 0 < nu < 0.5 (G18); ignored when den > 0 */
@@ -154,6 +161,16 @@ int qld_read_map(qld_ctx *ctx, int k, int which, float *host_dst);
 /* The reference table the kernels use: sin and cos of theta_{k,s} for s = s_first .. s_first+n-1, as float32
  * (FP32 accumulation) -- for inspection and tests.  Blocks until done.  Host pointers. */
 int qld_read_ref_table(qld_ctx *ctx, int k, int64_t s_first, int n, float *sin_out, float *cos_out);
+
+/* QLD_ACC_FIXED only.  Replace the Q1.30 reference table of reference k by caller-supplied integers (host
+ * arrays of n == N entries, entry i belongs to frame i+1, each in [-2^30, 2^30]); blocks until the device
+ * table is rebuilt.  qld_read_ref_table_fixed copies the table in use back to the host (blocks). */
+int qld_set_ref_table_fixed(qld_ctx *ctx, int k, const int32_t *sin_q30, const int32_t *cos_q30, int n);
+int qld_read_ref_table_fixed(qld_ctx *ctx, int k, int32_t *sin_q30, int32_t *cos_q30);
+
+/* QLD_ACC_FIXED with QLD_MAP_SUMS_I64: device pointers to the exact sums sum_s x_s R(s) of reference k,
+ * [H][W] int64 each (I*2^30 and Q*2^30 before normalisation), valid like the maps. */
+int qld_get_sums_i64(qld_ctx *ctx, int k, const int64_t **I, const int64_t **Q);
 
 /* Bookkeeping (host side, never blocks): frames pushed so far, windows produced so far. */
 int qld_counters(const qld_ctx *ctx, int64_t *frames_pushed, int64_t *windows_done);

@@ -9,6 +9,7 @@
 #include <string>
 
 #include "qld_internal.h"
+#include "qld_tc.h"
 
 namespace {
 
@@ -33,10 +34,17 @@ struct qld_ctx {
     uint32_t max_value;
     int cap, cap_w;          // frame store capacity, weight table capacity
     bool ring, external;     // ring buffer / frames attached by the caller
-    bool is_int;
+    bool is_int, is_fixed;
     int rows, rows_pad;
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
+    // tensor-core (FIXED) path
+    int32_t *rfix;           // [2K][N] Q30 references
+    int8_t *digits;          // digit tiles for the MMA B operand
+    int64_t *sums;           // optional [2K][HW] exact sums
+    alignas(64) unsigned char tmap[128];
+    bool tmap_valid;
+    int n_sms;
     // device memory
     void *ws;
     bool own_ws;
@@ -117,12 +125,12 @@ void exact_sincos(int64_t a, int64_t D, double extra, double *sn, double *cs)
 
 struct Plan {
     int H, W, dtype, bytes, N, K, accum, norm, maps, cap, cap_w, rows, rows_pad;
-    bool ring, external, is_int;
+    bool ring, external, is_int, is_fixed;
     int64_t HW;
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
     // workspace offsets
-    size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, total;
+    size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, off_rfix, off_digits, off_sums, total;
 };
 
 int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
@@ -135,12 +143,12 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     if (cfg->K < 1 || cfg->K > QLD_MAX_K || !cfg->refs) return bad(QLD_E_INVAL, "K must be 1..8 with refs given");
     if (cfg->ring_frames < -1 || (cfg->ring_frames > 0 && cfg->ring_frames <= cfg->N))
         return bad(QLD_E_INVAL, "ring_frames must be -1, 0, or > N");
-    if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_INT_BINS) return bad(QLD_E_INVAL, "unknown accum");
+    if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_FIXED) return bad(QLD_E_INVAL, "unknown accum");
     if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
-    if (cfg->maps & ~QLD_MAP_ALL) return bad(QLD_E_INVAL, "unknown bits in maps");
+    if (cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64)) return bad(QLD_E_INVAL, "unknown bits in maps");
     memset(pl, 0, sizeof *pl);
     pl->H = cfg->H; pl->W = cfg->W; pl->dtype = cfg->dtype; pl->bytes = cfg->dtype == QLD_U8 ? 1 : 2;
-    pl->N = cfg->N; pl->K = cfg->K; pl->norm = cfg->norm; pl->maps = cfg->maps ? cfg->maps : QLD_MAP_ALL;
+    pl->N = cfg->N; pl->K = cfg->K; pl->norm = cfg->norm; pl->maps = (cfg->maps & QLD_MAP_ALL) ? cfg->maps : (cfg->maps | QLD_MAP_ALL);
     pl->HW = (int64_t)cfg->H * cfg->W;
     pl->ring = cfg->ring_frames > 0; pl->external = cfg->ring_frames == -1;
     pl->cap = pl->ring ? cfg->ring_frames : cfg->N;
@@ -194,8 +202,15 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         if (!bins_rows(&rows)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
         if (!bins_fit()) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
     }
+    if (acc == QLD_ACC_FIXED) {
+        if (pl->ring) return bad(QLD_E_UNSUPPORTED, "FIXED (tensor-core) accumulation works on whole-window stores, not rings");
+        if ((pl->HW * pl->bytes) % 16 != 0) return bad(QLD_E_UNSUPPORTED, "FIXED: H*W*bytes_per_sample must be a multiple of 16 (TMA row pitch)");
+        if ((int64_t)cfg->N > 65536) return bad(QLD_E_UNSUPPORTED, "FIXED: N must be <= 65536 for exact int32 partial sums");
+    }
+    if ((pl->maps & QLD_MAP_SUMS_I64) && acc != QLD_ACC_FIXED) return bad(QLD_E_INVAL, "QLD_MAP_SUMS_I64 needs QLD_ACC_FIXED");
     pl->accum = acc;
     pl->is_int = acc == QLD_ACC_INT_BINS;
+    pl->is_fixed = acc == QLD_ACC_FIXED;
     FinParams &f = pl->fin;
     f.K = cfg->K; f.is_int = pl->is_int;
     f.scale = cfg->norm == QLD_NORM_AMPLITUDE ? 2.0 / (double)cfg->N : 1.0;
@@ -227,15 +242,19 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     // workspace layout
     size_t o = 0;
     pl->off_frames = o; if (!pl->external) o += align_up((size_t)pl->cap * pl->HW * pl->bytes);
-    pl->off_wtab = o; o += align_up((size_t)pl->cap_w * pl->rows_pad * 4);
-    pl->off_cum = o; o += align_up((size_t)pl->cap_w * pl->rows_pad * 8);
-    pl->off_acc = o; o += align_up((size_t)pl->rows_pad * pl->HW * (pl->is_int ? 4 : 8));
-    pl->off_ped = o; o += align_up((size_t)pl->HW * 4);
+    const bool cc = !pl->is_fixed;          // CUDA-core paths: weight tables, sliding accumulators, pedestal
+    pl->off_wtab = o; if (cc) o += align_up((size_t)pl->cap_w * pl->rows_pad * 4);
+    pl->off_cum = o; if (cc) o += align_up((size_t)pl->cap_w * pl->rows_pad * 8);
+    pl->off_acc = o; if (cc && (pl->ring || pl->is_int)) o += align_up((size_t)pl->rows_pad * pl->HW * (pl->is_int ? 4 : 8));
+    pl->off_ped = o; if (cc && pl->ring) o += align_up((size_t)pl->HW * 4);
     const size_t map = align_up((size_t)pl->K * pl->HW * 4);
     pl->off_I = o; if (pl->maps & QLD_MAP_I) o += map;
     pl->off_Q = o; if (pl->maps & QLD_MAP_Q) o += map;
     pl->off_A = o; if (pl->maps & QLD_MAP_AMP) o += map;
     pl->off_P = o; if (pl->maps & QLD_MAP_PHASE) o += map;
+    pl->off_rfix = o; if (pl->is_fixed) o += align_up((size_t)2 * pl->K * pl->N * 4);
+    pl->off_digits = o; if (pl->is_fixed) o += align_up(qld_tc_digit_bytes(pl->K, pl->N));
+    pl->off_sums = o; if (pl->is_fixed && (pl->maps & QLD_MAP_SUMS_I64)) o += align_up((size_t)2 * pl->K * pl->HW * 8);
     pl->total = o;
     return QLD_OK;
 }
@@ -255,9 +274,20 @@ int fill_tables(qld_ctx *c, int64_t s_first, int n, cudaStream_t st)
 int init_device_state(qld_ctx *c)
 {
     // tables zeroed (padding rows stay zero; cum entry of frame 0 is zero), then filled for the whole store
-    CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
-    CU(c, cudaMemsetAsync(c->cum, 0, (size_t)c->cap_w * c->rows_pad * 8, c->s_copy));
-    if (!c->ring) {
+    if (!c->is_fixed) {
+        CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
+        CU(c, cudaMemsetAsync(c->cum, 0, (size_t)c->cap_w * c->rows_pad * 8, c->s_copy));
+    }
+    if (c->is_fixed) {
+        TableFillParams tp;
+        memset(&tp, 0, sizeof tp);
+        tp.K = c->K;
+        for (int k = 0; k < c->K; ++k) tp.ref[k] = c->ref[k];
+        tp.s_first = 1; tp.n = c->N;
+        CU(c, qld_launch_fixed_table_fill(tp, c->rfix, c->N, c->s_copy));
+        CU(c, qld_launch_digit_pack(c->rfix, c->N, c->N, c->K, c->digits, c->s_copy));
+        c->launches += 2;
+    } else if (!c->ring) {
         int rc = fill_tables(c, 1, c->N, c->s_copy);
         if (rc) return rc;
     }
@@ -336,8 +366,25 @@ int record_demod(qld_ctx *c, int64_t oldest_read)
 }
 
 // whole-window kernel over absolute frames a+1 .. a+N; seeds the sliding accumulators when asked
+int run_whole_tc(qld_ctx *c)
+{
+    if (!c->tmap_valid) {
+        CU(c, qld_tc_encode_tmap(c->tmap, c->frames, c->HW * c->bytes, c->N));
+        c->tmap_valid = true;
+    }
+    TcParams p;
+    memset(&p, 0, sizeof p);
+    p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes;
+    p.digits = c->digits; p.sums_out = c->sums;
+    p.fin = fin_with_maps(c);
+    CU(c, qld_launch_demod_tc(c->tmap, p, c->n_sms, c->s_comp));
+    c->launches++;
+    return record_demod(c, 1);
+}
+
 int run_whole(qld_ctx *c, int64_t a, bool seed)
 {
+    if (c->is_fixed) return run_whole_tc(c);
     DemodParams p;
     memset(&p, 0, sizeof p);
     p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
@@ -406,7 +453,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     c->H = pl.H; c->W = pl.W; c->dtype = pl.dtype; c->bytes = pl.bytes; c->N = pl.N; c->K = pl.K;
     c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops > 0 ? cfg->resync_hops : 0;
     c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
-    c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
+    c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
     for (int k = 0; k < pl.K; ++k) c->ref[k] = pl.ref[k];
     c->fin = pl.fin;
     c->ws_bytes = pl.total;
@@ -430,6 +477,15 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     c->mapQ = (pl.maps & QLD_MAP_Q) ? reinterpret_cast<float *>(b + pl.off_Q) : nullptr;
     c->mapA = (pl.maps & QLD_MAP_AMP) ? reinterpret_cast<float *>(b + pl.off_A) : nullptr;
     c->mapP = (pl.maps & QLD_MAP_PHASE) ? reinterpret_cast<float *>(b + pl.off_P) : nullptr;
+    if (pl.is_fixed) {
+        c->rfix = reinterpret_cast<int32_t *>(b + pl.off_rfix);
+        c->digits = reinterpret_cast<int8_t *>(b + pl.off_digits);
+        c->sums = (pl.maps & QLD_MAP_SUMS_I64) ? reinterpret_cast<int64_t *>(b + pl.off_sums) : nullptr;
+        if ((reinterpret_cast<uintptr_t>(c->frames) & 15) != 0) { if (c->own_ws) cudaFree(c->ws); delete c; return fail(nullptr, QLD_E_NOMEM, "workspace not 16-byte aligned"); }
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
 
     c->s_comp = static_cast<cudaStream_t>(cfg->compute_stream);
     c->s_copy = static_cast<cudaStream_t>(cfg->copy_stream);
@@ -460,7 +516,9 @@ int qld_attach_frames_device(qld_ctx *c, const void *device_frames)
     if (c->sticky) return QLD_E_CUDA;
     if (!device_frames) return fail(c, QLD_E_INVAL, "attach: null buffer");
     if (c->ring) return fail(c, QLD_E_STATE, "attach: ring contexts copy their frames (use qld_push_frames_device)");
+    if (c->is_fixed && (reinterpret_cast<uintptr_t>(device_frames) & 15)) return fail(c, QLD_E_INVAL, "attach: FIXED accumulation needs a 16-byte aligned buffer");
     c->frames = const_cast<unsigned char *>(static_cast<const unsigned char *>(device_frames));
+    c->tmap_valid = false;
     c->pushed = c->N;
     return QLD_OK;
 }
@@ -550,7 +608,7 @@ int qld_read_map(qld_ctx *c, int k, int which, float *host_dst)
 int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out, float *cos_out)
 {
     if (!c || k < 0 || k >= c->K || n < 1 || s_first < 1) return c ? fail(c, QLD_E_INVAL, "read_ref_table: bad argument") : QLD_E_INVAL;
-    if (c->is_int) return fail(c, QLD_E_STATE, "read_ref_table: integer-bin contexts have no float table");
+    if (c->is_int || c->is_fixed) return fail(c, QLD_E_STATE, "read_ref_table: this context has no float table");
     if (c->ring && (s_first + n - 1 > c->pushed || s_first + c->cap_w <= c->pushed + 1)) return fail(c, QLD_E_STATE, "read_ref_table: frames not in the ring");
     if (!c->ring && s_first + n - 1 > c->N) return fail(c, QLD_E_INVAL, "read_ref_table: beyond the window");
     CU(c, cudaStreamSynchronize(c->s_copy));
@@ -561,6 +619,44 @@ int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out
         if (sin_out) sin_out[i] = w[0];
         if (cos_out) cos_out[i] = w[1];
     }
+    return QLD_OK;
+}
+
+int qld_set_ref_table_fixed(qld_ctx *c, int k, const int32_t *sin_q30, const int32_t *cos_q30, int n)
+{
+    if (!c || k < 0 || k >= c->K || !sin_q30 || !cos_q30) return c ? fail(c, QLD_E_INVAL, "set_ref_table_fixed: bad argument") : QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (!c->is_fixed) return fail(c, QLD_E_STATE, "set_ref_table_fixed: context does not use QLD_ACC_FIXED");
+    if (n != c->N) return fail(c, QLD_E_INVAL, "set_ref_table_fixed: n must equal N");
+    for (int i = 0; i < n; ++i)
+        if (sin_q30[i] > (1 << 30) || sin_q30[i] < -(1 << 30) || cos_q30[i] > (1 << 30) || cos_q30[i] < -(1 << 30))
+            return fail(c, QLD_E_INVAL, "set_ref_table_fixed: entries must lie in [-2^30, 2^30]");
+    int rc = qld_sync(c);
+    if (rc) return rc;
+    CU(c, cudaMemcpy(c->rfix + (size_t)(2 * k) * c->N, sin_q30, (size_t)n * 4, cudaMemcpyHostToDevice));
+    CU(c, cudaMemcpy(c->rfix + (size_t)(2 * k + 1) * c->N, cos_q30, (size_t)n * 4, cudaMemcpyHostToDevice));
+    CU(c, qld_launch_digit_pack(c->rfix, c->N, c->N, c->K, c->digits, c->s_comp));
+    c->launches++;
+    return QLD_OK;
+}
+
+int qld_read_ref_table_fixed(qld_ctx *c, int k, int32_t *sin_q30, int32_t *cos_q30)
+{
+    if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "read_ref_table_fixed: bad argument") : QLD_E_INVAL;
+    if (!c->is_fixed) return fail(c, QLD_E_STATE, "read_ref_table_fixed: context does not use QLD_ACC_FIXED");
+    int rc = qld_sync(c);
+    if (rc) return rc;
+    if (sin_q30) CU(c, cudaMemcpy(sin_q30, c->rfix + (size_t)(2 * k) * c->N, (size_t)c->N * 4, cudaMemcpyDeviceToHost));
+    if (cos_q30) CU(c, cudaMemcpy(cos_q30, c->rfix + (size_t)(2 * k + 1) * c->N, (size_t)c->N * 4, cudaMemcpyDeviceToHost));
+    return QLD_OK;
+}
+
+int qld_get_sums_i64(qld_ctx *c, int k, const int64_t **I, const int64_t **Q)
+{
+    if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "get_sums_i64: k out of range") : QLD_E_INVAL;
+    if (!c->sums) return fail(c, QLD_E_STATE, "get_sums_i64: needs QLD_ACC_FIXED and QLD_MAP_SUMS_I64");
+    if (I) *I = c->sums + (size_t)(2 * k) * c->HW;
+    if (Q) *Q = c->sums + (size_t)(2 * k + 1) * c->HW;
     return QLD_OK;
 }
 
@@ -589,7 +685,7 @@ int qld_reset(qld_ctx *c)
     if (rc) return rc;
     c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
-    if (c->external) c->frames = nullptr;
+    if (c->external) { c->frames = nullptr; c->tmap_valid = false; }
     if (c->ring) {
         rc = init_device_state(c);
         if (rc) return rc;

@@ -1,0 +1,23 @@
+// Tensor-core (tcgen05) demodulation path: declarations shared by qld_tc.cu and qld_api.cu.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "qld_internal.h"
+
+struct TcParams {
+    int64_t HW;
+    int64_t row_bytes;        // H*W*bytes: bytes of one frame
+    int32_t N;                // frames in the window
+    int32_t bytes;            // 1 (u8) or 2 (u16)
+    const int8_t *digits;     // digit tiles, see k_digit_pack
+    int64_t *sums_out;        // optional [2K][HW] exact fixed-point sums (Q30 references)
+    FinParams fin;
+};
+
+int qld_tc_columns(int K);                       // N columns of the MMA: 8 per reference, padded to 16
+size_t qld_tc_digit_bytes(int K, int N);
+cudaError_t qld_tc_encode_tmap(void *tmap_out /*128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames);
+cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st);
+cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
+cudaError_t qld_launch_demod_tc(const void *tmap, const TcParams &p, int n_sms, cudaStream_t st);

@@ -16,17 +16,17 @@ _LIB_PATH = os.path.join(_PKG, "libqld.so")
 
 QLD_U8, QLD_U16 = 0, 1
 QLD_OK, QLD_E_INVAL, QLD_E_NOMEM, QLD_E_CUDA, QLD_E_STATE, QLD_E_OVERRUN, QLD_E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
-QLD_ACC_AUTO, QLD_ACC_FP32, QLD_ACC_INT_BINS = 0, 1, 2
+QLD_ACC_AUTO, QLD_ACC_FP32, QLD_ACC_INT_BINS, QLD_ACC_FIXED = 0, 1, 2, 3
 QLD_NORM_PAPER, QLD_NORM_AMPLITUDE = 0, 1
 QLD_WHOLE, QLD_SLIDE = 0, 1
-QLD_MAP_I, QLD_MAP_Q, QLD_MAP_AMP, QLD_MAP_PHASE, QLD_MAP_ALL = 1, 2, 4, 8, 15
+QLD_MAP_I, QLD_MAP_Q, QLD_MAP_AMP, QLD_MAP_PHASE, QLD_MAP_ALL, QLD_MAP_SUMS_I64 = 1, 2, 4, 8, 15, 16
 _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", -4: "QLD_E_STATE", -5: "QLD_E_OVERRUN",
            -6: "QLD_E_UNSUPPORTED"}
 
 # every symbol include/qld.h declares (tests check that the library exports each of them)
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
            "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
-           "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches",
+           "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches",
            "qld_synth_fill"]
 
 
@@ -82,6 +82,9 @@ def load_library():
     l.qld_get_bins.argtypes = [vp, i, pf, C.POINTER(C.c_int)]
     l.qld_read_map.argtypes = [vp, i, i, vp]
     l.qld_read_ref_table.argtypes = [vp, i, i64, i, vp, vp]
+    l.qld_set_ref_table_fixed.argtypes = [vp, i, vp, vp, i]
+    l.qld_read_ref_table_fixed.argtypes = [vp, i, vp, vp]
+    l.qld_get_sums_i64.argtypes = [vp, i, pf, pf]
     l.qld_counters.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     l.qld_sync.argtypes = [vp]
     l.qld_reset.argtypes = [vp]
@@ -167,7 +170,7 @@ class QLD:
         if self._ws is not None:
             off = ptr - self._ws.data_ptr()
             return self._ws[off:off + n * itemsize].view(dtype).view(*shape)
-        iface = {"shape": tuple(shape), "typestr": {torch.float32: "<f4", torch.int32: "<i4"}[dtype], "data": (ptr, False), "version": 2}
+        iface = {"shape": tuple(shape), "typestr": {torch.float32: "<f4", torch.int32: "<i4", torch.int64: "<i8"}[dtype], "data": (ptr, False), "version": 2}
         holder = type("_Dev", (), {"__cuda_array_interface__": iface})()
         return torch.as_tensor(holder, device=self.device)
 
@@ -224,6 +227,24 @@ class QLD:
         cs = np.empty(n, dtype=np.float32)
         self._check(self.lib.qld_read_ref_table(self._ctx, int(k), int(s_first), int(n), sn.ctypes.data, cs.ctypes.data))
         return sn, cs
+
+    def set_ref_table_fixed(self, k: int, sin_q30, cos_q30) -> None:
+        import numpy as np
+        a = np.ascontiguousarray(sin_q30, dtype=np.int32)
+        b = np.ascontiguousarray(cos_q30, dtype=np.int32)
+        self._check(self.lib.qld_set_ref_table_fixed(self._ctx, int(k), a.ctypes.data, b.ctypes.data, int(a.size)))
+
+    def read_ref_table_fixed(self, k: int):
+        import numpy as np
+        a = np.empty(self.N, dtype=np.int32)
+        b = np.empty(self.N, dtype=np.int32)
+        self._check(self.lib.qld_read_ref_table_fixed(self._ctx, int(k), a.ctypes.data, b.ctypes.data))
+        return a, b
+
+    def get_sums_i64(self, k: int = 0):
+        p, q = C.c_void_p(), C.c_void_p()
+        self._check(self.lib.qld_get_sums_i64(self._ctx, int(k), C.byref(p), C.byref(q)))
+        return (self._view(p.value, (self.H, self.W), self._torch.int64), self._view(q.value, (self.H, self.W), self._torch.int64))
 
     def counters(self):
         a, b = C.c_int64(), C.c_int64()

@@ -1,0 +1,107 @@
+"""GPU parity of the tcgen05 (QLD_ACC_FIXED) path: exact int64 sums against the integer oracle with the same
+Q1.30 reference table (bit-exact), and the float maps against the fp64 definition."""
+import numpy as np
+import pytest
+
+from _parity import check_float_maps, oracle_maps
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def Q():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1511_03390_b200 import qld
+    qld.load_library()
+    return qld
+
+
+def _q30(oracle, ref, N):
+    sn, cs = oracle.ref_tables(ref, 1, N)
+    return np.rint(sn * 2.0 ** 30).astype(np.int64), np.rint(cs * 2.0 ** 30).astype(np.int64)
+
+
+def _maps(ctx, k=0):
+    return tuple(None if m is None else m.cpu().numpy() for m in ctx.get_maps(k))
+
+
+@pytest.mark.parametrize("ref", [{"nu": 0.0937}, {"nu": 0.4321, "phase": 2.0}, {"num": 1, "den": 4}, {"num": 1, "den": 6}])
+def test_fixed_table_matches_rounded_oracle(Q, oracle, ref):
+    N = 1000
+    ctx = Q.QLD(4, 8, "u16", N, [ref], accum=Q.QLD_ACC_FIXED)
+    gs, gc = ctx.read_ref_table_fixed(0)
+    os_, oc = _q30(oracle, ref, N)
+    assert np.abs(gs - os_).max() <= 1 and np.abs(gc - oc).max() <= 1           # a tie in rint can flip on the last bit of sin
+    assert (gs == os_).mean() > 0.999 and (gc == oc).mean() > 0.999
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("dtype,hi", [(np.uint8, 256), (np.uint16, 65536)])
+@pytest.mark.parametrize("H,W,N", [(1, 16, 1), (3, 16, 5), (4, 16, 63), (8, 24, 64), (8, 40, 65), (64, 64, 200), (37, 48, 129),
+                                   (128, 160, 70)])
+def test_fixed_sums_bit_exact(Q, oracle, dtype, hi, H, W, N):
+    """sum_s x_s R(s) with the oracle's own Q1.30 table handed to the library: bit-exact int64, full sample range."""
+    rng = np.random.default_rng(H * W + N)
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    ref = {"nu": 0.0937, "phase": 0.3}
+    isin, icos = _q30(oracle, ref, N)
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
+    ctx.set_ref_table_fixed(0, isin, icos)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    oI, oQ = oracle.demod_int(x, isin, icos)
+    gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(0)]
+    assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ)
+    I, Qm, A, P = _maps(ctx)
+    assert np.array_equal(I, (oI.astype(np.float64) * 2.0 ** -30).astype(np.float32))
+    assert np.array_equal(Qm, (oQ.astype(np.float64) * 2.0 ** -30).astype(np.float32))
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 5, 8])
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
+def test_fixed_multi_reference(Q, oracle, K, dtype):
+    rng = np.random.default_rng(K)
+    H, W, N = 40, 72, 300
+    hi = 256 if dtype == np.uint8 else 4096
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
+    tabs = [_q30(oracle, r, N) for r in refs]
+    for k in range(K):
+        ctx.set_ref_table_fixed(k, *tabs[k])
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    for k in range(K):
+        oI, oQ = oracle.demod_int(x, *tabs[k])
+        gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
+        assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"k={k}"
+        # and against the float definition: quantising the references to 2^-31 costs ~1e-9 relative
+        check_float_maps(_maps(ctx, k), oracle_maps(oracle, x, refs[k]), rel=1e-7, what=f"K={K} k={k}")
+    ctx.destroy()
+
+
+def test_fixed_own_table_meets_float_tolerance_on_cfg2_shape(Q, oracle):
+    from paper_1511_03390_b200 import synth
+    wl = synth.cfg2(H=64, W=160, N=1024)
+    x = synth.frames(wl.scene, 1, wl.N)
+    ref = dict(wl.refs[0])
+    ctx = Q.QLD(64, 160, "u16", wl.N, [ref], accum=Q.QLD_ACC_FIXED)
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    worst = check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), rel=1e-7, what="cfg2-shaped")
+    assert worst < 1e-5                                      # even the strict point-wise error
+    ctx.destroy()
+
+
+def test_fixed_rejects_what_it_cannot_do(Q):
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(3, 17, "u8", 16, [{"nu": 0.1}], accum=Q.QLD_ACC_FIXED)            # 51 bytes per frame: not a TMA pitch
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(4, 16, "u8", 16, [{"nu": 0.1}], ring_frames=40, accum=Q.QLD_ACC_FIXED)
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
