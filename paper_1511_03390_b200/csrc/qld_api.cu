@@ -42,6 +42,7 @@ struct qld_ctx {
     int32_t *rfix;           // [2K][N] Q30 references
     int8_t *digits;          // digit tiles for the MMA B operand
     int64_t *sums;           // optional [2K][HW] exact sums
+    unsigned int *tile_counter;
     alignas(64) unsigned char tmap[128];
     bool tmap_valid;
     int n_sms;
@@ -130,7 +131,7 @@ struct Plan {
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
     // workspace offsets
-    size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, off_rfix, off_digits, off_sums, total;
+    size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, off_rfix, off_digits, off_sums, off_counter, total;
 };
 
 int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
@@ -255,6 +256,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     pl->off_rfix = o; if (pl->is_fixed) o += align_up((size_t)2 * pl->K * pl->N * 4);
     pl->off_digits = o; if (pl->is_fixed) o += align_up(qld_tc_digit_bytes(pl->K, pl->N));
     pl->off_sums = o; if (pl->is_fixed && (pl->maps & QLD_MAP_SUMS_I64)) o += align_up((size_t)2 * pl->K * pl->HW * 8);
+    pl->off_counter = o; if (pl->is_fixed) o += 256;
     pl->total = o;
     return QLD_OK;
 }
@@ -375,7 +377,7 @@ int run_whole_tc(qld_ctx *c)
     TcParams p;
     memset(&p, 0, sizeof p);
     p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes;
-    p.digits = c->digits; p.sums_out = c->sums;
+    p.digits = c->digits; p.sums_out = c->sums; p.tile_counter = c->tile_counter;
     p.fin = fin_with_maps(c);
     CU(c, qld_launch_demod_tc(c->tmap, p, c->n_sms, c->s_comp));
     c->launches++;
@@ -481,6 +483,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
         c->rfix = reinterpret_cast<int32_t *>(b + pl.off_rfix);
         c->digits = reinterpret_cast<int8_t *>(b + pl.off_digits);
         c->sums = (pl.maps & QLD_MAP_SUMS_I64) ? reinterpret_cast<int64_t *>(b + pl.off_sums) : nullptr;
+        c->tile_counter = reinterpret_cast<unsigned int *>(b + pl.off_counter);
         if ((reinterpret_cast<uintptr_t>(c->frames) & 15) != 0) { if (c->own_ws) cudaFree(c->ws); delete c; return fail(nullptr, QLD_E_NOMEM, "workspace not 16-byte aligned"); }
         int dev = 0;
         cudaGetDevice(&dev);

@@ -21,6 +21,8 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
 
 #include "qld_internal.h"
 #include "qld_tc.h"
@@ -159,30 +161,36 @@ __global__ void k_digit_pack(const int32_t *rfix, int n_stride, int n, int rows,
 // ---------------------------------------------------------------------------------------------------
 // the contraction kernel
 // ---------------------------------------------------------------------------------------------------
-template <int NC, int T, int STAGES>
+// shared-memory carve-up for (NC columns, T spans per tile, STAGES pipeline stages)
 struct TcSmem {
-    static constexpr int A_SUB = KC * SUB_BYTES;               // 8 KB per 128-byte span per stage
-    static constexpr int A_STAGE = T * A_SUB;
-    static constexpr int B_STAGE = (KC / MMA_K) * NC * MMA_K;
-    static constexpr int OFF_B = STAGES * A_STAGE;
-    static constexpr int OFF_BAR = OFF_B + STAGES * B_STAGE;
-    static constexpr int TOTAL = OFF_BAR + (2 * STAGES + 4) * 8 + 16;
+    int a_sub, a_stage, b_stage, off_b, off_bar, total;
+    __host__ __device__ TcSmem(int nc, int t, int stages)
+    {
+        a_sub = KC * SUB_BYTES;                       // 8 KB per 128-byte span per stage
+        a_stage = t * a_sub;
+        b_stage = (KC / MMA_K) * nc * MMA_K;
+        off_b = stages * a_stage;
+        off_bar = off_b + stages * b_stage;
+        total = off_bar + (2 * stages + 4) * 8 + 16 + 48;
+    }
 };
 
-template <int NC, int T, int STAGES, int BYTES>
-__global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap, const TcParams p)
+template <int NC, int BYTES>
+__global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap, const TcParams p, const int T, const int STAGES)
 {
-    using SM = TcSmem<NC, T, STAGES>;
+    const TcSmem SM(NC, T, STAGES);
     extern __shared__ unsigned char smem_raw[];
     // 128-byte-swizzled TMA/UMMA tiles need 1024-byte alignment in the shared window
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     unsigned char *sA = smem;
-    unsigned char *sB = smem + SM::OFF_B;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem + SM::OFF_BAR);
+    unsigned char *sB = smem + SM.off_b;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem + SM.off_bar);
     uint64_t *empty = full + STAGES;
     uint64_t *tfull = empty + STAGES;
     uint64_t *tempty = tfull + 2;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+    volatile int *tile_q = reinterpret_cast<volatile int *>(tmem_slot + 2);      // [8] tile ids, producer -> MMA warp
+    volatile int *tbuf_tile = tile_q + 8;                                        // [2] tile id per accumulator buffer
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (p.N + KC - 1) / KC;
@@ -195,7 +203,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
             mbar_init(&empty[i], 1);
         }
         for (int i = 0; i < 2; ++i) {
-            mbar_init(&tfull[i], 1);
+            mbar_init(&tfull[i], 2);
             mbar_init(&tempty[i], 128);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -210,20 +218,30 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
-        // ===== TMA producer =====
+        // ===== TMA producer + tile scheduler =====
+        // Tiles are claimed from a global counter: under HBM contention SMs progress at very different rates
+        // (ncu: fastest SM done in 56 % of the time with a static split), so the split must be dynamic.
         if (lane == 0) {
-            int stage = 0;
+            int stage = 0, it = 0;
             uint32_t phase = 0;
-            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+            for (;; ++it) {
+                int tile = (int)atomicAdd(p.tile_counter, 1u);
+                if (tile >= n_tiles) tile = -1;
+                tile_q[it & 7] = tile;                       // published by the next arrive on full[stage]
+                if (tile < 0) {                              // end of work: an empty stage carries the sentinel
+                    mbar_wait(&empty[stage], phase ^ 1);
+                    mbar_arrive(&full[stage]);
+                    break;
+                }
                 const int sub0 = tile * T;
                 const int nv = min(T, n_sub - sub0);
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&empty[stage], phase ^ 1);
-                    mbar_expect_tx(&full[stage], (uint32_t)(nv * SM::A_SUB + SM::B_STAGE));
+                    mbar_expect_tx(&full[stage], (uint32_t)(nv * SM.a_sub + SM.b_stage));
                     for (int t = 0; t < nv; ++t)
-                        tma_load_2d(sA + stage * SM::A_STAGE + t * SM::A_SUB, &tmap, &full[stage], (sub0 + t) * SUB_BYTES, c * KC,
+                        tma_load_2d(sA + stage * SM.a_stage + t * SM.a_sub, &tmap, &full[stage], (sub0 + t) * SUB_BYTES, c * KC,
                                     0x12F0000000000000ull /* evict first: every sample is read once */);
-                    bulk_load(sB + stage * SM::B_STAGE, p.digits + (size_t)c * SM::B_STAGE, SM::B_STAGE, &full[stage]);
+                    bulk_load(sB + stage * SM.b_stage, p.digits + (size_t)c * SM.b_stage, SM.b_stage, &full[stage]);
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -232,30 +250,40 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
         // ===== MMA issuer =====
         // instruction descriptor (cute::UMMA::InstrDescriptor): D = s32, A = u8 MN-major, B = s8 K-major, M = 128, N = NC
         constexpr uint32_t idesc = (2u << 4) | (0u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((uint32_t)(NC >> 3) << 17) | ((128u >> 4) << 24);
-        int stage = 0, it = 0;
+        int stage = 0;
         uint32_t phase = 0;
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-            const int nv = min(T, n_sub - tile * T);
+        for (int it = 0;; ++it) {
             const int buf = it & 1;
-            mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
+            mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);     // epilogue has drained this accumulator buffer
             tc_fence_after();
+            mbar_wait(&full[stage], phase);                   // first chunk of the tile (or the sentinel) has landed
+            const int tile = tile_q[it & 7];
+            if (lane == 0) tbuf_tile[buf] = tile;
+            if (tile < 0) {
+                if (lane == 0) { mbar_arrive(&tfull[buf]); mbar_arrive(&tfull[buf]); }
+                break;
+            }
+            const int nv = min(T, n_sub - tile * T);
             for (int c = 0; c < n_chunks; ++c) {
-                mbar_wait(&full[stage], phase);
+                if (c > 0) mbar_wait(&full[stage], phase);
                 tc_fence_after();
                 if (lane == 0) {
-                    const uint32_t a0 = smem_u32(sA + stage * SM::A_STAGE), b0 = smem_u32(sB + stage * SM::B_STAGE);
+                    const uint32_t a0 = smem_u32(sA + stage * SM.a_stage), b0 = smem_u32(sB + stage * SM.b_stage);
                     for (int t = 0; t < nv; ++t) {
 #pragma unroll
                         for (int ks = 0; ks < KC / MMA_K; ++ks) {
                             // A: MN-major, 128-byte swizzle: rows of 128 pixel bytes, 8-frame atoms 1024 B apart (SBO)
-                            const uint64_t ad = smem_desc(a0 + t * SM::A_SUB + ks * MMA_K * SUB_BYTES, SM::A_SUB, 1024, 2);
+                            const uint64_t ad = smem_desc(a0 + t * SM.a_sub + ks * MMA_K * SUB_BYTES, SM.a_sub, 1024, 2);
                             // B: K-major, no swizzle: K halves 128 B apart (LBO), 8-column groups 256 B apart (SBO)
                             const uint64_t bd = smem_desc(b0 + ks * NC * MMA_K, 128, 256, 0);
                             tc_mma_i8(tmem_base + (uint32_t)(buf * T * NC + t * NC), ad, bd, idesc, (c | ks) ? 1u : 0u);
                         }
                     }
                     tc_commit(&empty[stage]);                 // frees the stage when these MMAs have read it
-                    if (c == n_chunks - 1) tc_commit(&tfull[buf]);
+                    if (c == n_chunks - 1) {
+                        tc_commit(&tfull[buf]);               // arrival 1 of 2: the accumulators are complete
+                        mbar_arrive(&tfull[buf]);             // arrival 2 of 2: releases tbuf_tile[buf]
+                    }
                 }
                 __syncwarp();
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -265,11 +293,12 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
         // ===== epilogue: TMEM -> registers -> exact int64 sums -> A4 finalise =====
         const int q = warp & 3;                         // TMEM lane quarter this warp may read
         const int m = q * 32 + lane;                    // accumulator row = byte index inside the 128-byte span
-        int it = 0;
-        for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-            const int nv = min(T, n_sub - tile * T);
+        for (int it = 0;; ++it) {
             const int buf = it & 1;
             mbar_wait(&tfull[buf], (it >> 1) & 1);
+            const int tile = tbuf_tile[buf];
+            if (tile < 0) break;
+            const int nv = min(T, n_sub - tile * T);
             tc_fence_after();
             for (int t = 0; t < nv; ++t) {
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * T * NC + t * NC);
@@ -329,19 +358,29 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     }
 }
 
-template <int NC, int T, int STAGES, int BYTES>
+template <int NC, int BYTES>
 cudaError_t launch_tc(const CUtensorMap &tmap, const TcParams &p, int n_sms, cudaStream_t st)
 {
-    using SM = TcSmem<NC, T, STAGES>;
-    static_assert(2 * T * NC <= 512, "TMEM columns");
-    static_assert(SM::TOTAL + 1024 <= 227 * 1024, "shared memory");
-    auto kern = k_demod_tc<NC, T, STAGES, BYTES>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM::TOTAL + 1024);
+    // tile shape: T spans (T*128 contiguous bytes of every frame per CTA), accumulators double buffered in the
+    // 512 TMEM columns; as many 64-frame stages as fit in shared memory
+    int T = 512 / (2 * NC);
+    if (T > 4) T = 4;                                     // 512-byte spans: small tiles keep the tail short
+    int stages = (220 * 1024) / TcSmem(NC, T, 1).off_bar;
+    if (const char *e = getenv("QLD_TC_TILE")) {          // tuning override: "T,STAGES"
+        int t = 0, s2 = 0;
+        if (sscanf(e, "%d,%d", &t, &s2) == 2 && t >= 1 && 2 * t * NC <= 512 && s2 >= 2 && TcSmem(NC, t, s2).total + 1024 <= 227 * 1024) { T = t; stages = s2; }
+    }
+    if (stages > 8) stages = 8;
+    const TcSmem SM(NC, T, stages);
+    auto kern = k_demod_tc<NC, BYTES>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 1024);
     if (e != cudaSuccess) return e;
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + T - 1) / T;
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
-    kern<<<grid, 192, SM::TOTAL + 1024, st>>>(tmap, p);
+    e = cudaMemsetAsync(p.tile_counter, 0, sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, 192, SM.total + 1024, st>>>(tmap, p, T, stages);
     return cudaGetLastError();
 }
 
@@ -401,17 +440,17 @@ cudaError_t qld_launch_demod_tc(const void *tmap, const TcParams &p, int n_sms, 
     const int nc = qld_tc_columns(p.fin.K);
     if (p.bytes == 2) {
         switch (nc) {
-        case 16: return launch_tc<16, 8, 3, 2>(tm, p, n_sms, st);
-        case 32: return launch_tc<32, 8, 3, 2>(tm, p, n_sms, st);
-        case 48: return launch_tc<48, 4, 5, 2>(tm, p, n_sms, st);
-        case 64: return launch_tc<64, 4, 5, 2>(tm, p, n_sms, st);
+        case 16: return launch_tc<16, 2>(tm, p, n_sms, st);
+        case 32: return launch_tc<32, 2>(tm, p, n_sms, st);
+        case 48: return launch_tc<48, 2>(tm, p, n_sms, st);
+        case 64: return launch_tc<64, 2>(tm, p, n_sms, st);
         }
     } else {
         switch (nc) {
-        case 16: return launch_tc<16, 8, 3, 1>(tm, p, n_sms, st);
-        case 32: return launch_tc<32, 8, 3, 1>(tm, p, n_sms, st);
-        case 48: return launch_tc<48, 4, 5, 1>(tm, p, n_sms, st);
-        case 64: return launch_tc<64, 4, 5, 1>(tm, p, n_sms, st);
+        case 16: return launch_tc<16, 1>(tm, p, n_sms, st);
+        case 32: return launch_tc<32, 1>(tm, p, n_sms, st);
+        case 48: return launch_tc<48, 1>(tm, p, n_sms, st);
+        case 64: return launch_tc<64, 1>(tm, p, n_sms, st);
         }
     }
     return cudaErrorInvalidValue;

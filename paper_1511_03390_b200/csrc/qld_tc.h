@@ -12,6 +12,7 @@ struct TcParams {
     int32_t bytes;            // 1 (u8) or 2 (u16)
     const int8_t *digits;     // digit tiles, see k_digit_pack
     int64_t *sums_out;        // optional [2K][HW] exact fixed-point sums (Q30 references)
+    unsigned int *tile_counter; // device counter for the dynamic tile scheduler, zeroed by the launcher
     FinParams fin;
 };
 
