@@ -226,7 +226,7 @@ def main():
     # ---- end to end through host buffers (pinned): push + demod + read amplitude map back ------------
     e2e = None
     parity = None
-    if rank == 0 or world > 1:
+    if (rank == 0 or world > 1) and args.e2e_steps > 0:
         host = torch.empty((N, H, W), dtype=frames.dtype).pin_memory()
         host.copy_(frames)
         amp_host = torch.empty((K, H, W), dtype=torch.float32).pin_memory()

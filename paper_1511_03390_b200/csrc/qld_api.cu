@@ -9,6 +9,7 @@
 #include <string>
 
 #include "qld_internal.h"
+#include "qld_stream.h"
 #include "qld_tc.h"
 
 namespace {
@@ -43,9 +44,13 @@ struct qld_ctx {
     int8_t *digits;          // digit tiles for the MMA B operand
     int64_t *sums;           // optional [2K][HW] exact sums
     unsigned int *tile_counter;
-    alignas(64) unsigned char tmap[128];
+    alignas(64) unsigned char tmap[256];   // two CUtensorMap (qld_tc_encode_tmap)
     bool tmap_valid;
     int n_sms;
+    // TMA-fed CUDA-core path (qld_stream.cu)
+    alignas(64) unsigned char stream_tmap[128];
+    const void *stream_tmap_frames;   // frame store the map was encoded for (NULL: none yet)
+    StreamShape stream_shape;
     // device memory
     void *ws;
     bool own_ws;
@@ -256,7 +261,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     pl->off_rfix = o; if (pl->is_fixed) o += align_up((size_t)2 * pl->K * pl->N * 4);
     pl->off_digits = o; if (pl->is_fixed) o += align_up(qld_tc_digit_bytes(pl->K, pl->N));
     pl->off_sums = o; if (pl->is_fixed && (pl->maps & QLD_MAP_SUMS_I64)) o += align_up((size_t)2 * pl->K * pl->HW * 8);
-    pl->off_counter = o; if (pl->is_fixed) o += 256;
+    pl->off_counter = o; o += 256;            // tile counter of the persistent kernels
     pl->total = o;
     return QLD_OK;
 }
@@ -371,7 +376,7 @@ int record_demod(qld_ctx *c, int64_t oldest_read)
 int run_whole_tc(qld_ctx *c)
 {
     if (!c->tmap_valid) {
-        CU(c, qld_tc_encode_tmap(c->tmap, c->frames, c->HW * c->bytes, c->N));
+        CU(c, qld_tc_encode_tmap(c->tmap, c->frames, c->HW * c->bytes, c->N, c->K, c->n_sms));
         c->tmap_valid = true;
     }
     TcParams p;
@@ -397,7 +402,18 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.acc_out = (seed || c->is_int) ? c->acc : nullptr;
     p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
     p.fin = fin_with_maps(c);
-    CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+    // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    if (sh.seg > 0) {
+        if (c->stream_tmap_frames != c->frames || sh.seg != c->stream_shape.seg || sh.kc != c->stream_shape.kc) {
+            CU(c, qld_stream_encode_tmap(c->stream_tmap, c->frames, c->HW * c->bytes, c->cap, sh));
+            c->stream_tmap_frames = c->frames;
+            c->stream_shape = sh;
+        }
+        CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+    } else {
+        CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+    }
     c->launches++;
     return record_demod(c, a + 1);
 }
@@ -479,15 +495,17 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     c->mapQ = (pl.maps & QLD_MAP_Q) ? reinterpret_cast<float *>(b + pl.off_Q) : nullptr;
     c->mapA = (pl.maps & QLD_MAP_AMP) ? reinterpret_cast<float *>(b + pl.off_A) : nullptr;
     c->mapP = (pl.maps & QLD_MAP_PHASE) ? reinterpret_cast<float *>(b + pl.off_P) : nullptr;
+    c->tile_counter = reinterpret_cast<unsigned int *>(b + pl.off_counter);
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     if (pl.is_fixed) {
         c->rfix = reinterpret_cast<int32_t *>(b + pl.off_rfix);
         c->digits = reinterpret_cast<int8_t *>(b + pl.off_digits);
         c->sums = (pl.maps & QLD_MAP_SUMS_I64) ? reinterpret_cast<int64_t *>(b + pl.off_sums) : nullptr;
-        c->tile_counter = reinterpret_cast<unsigned int *>(b + pl.off_counter);
         if ((reinterpret_cast<uintptr_t>(c->frames) & 15) != 0) { if (c->own_ws) cudaFree(c->ws); delete c; return fail(nullptr, QLD_E_NOMEM, "workspace not 16-byte aligned"); }
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, dev);
     }
 
     c->s_comp = static_cast<cudaStream_t>(cfg->compute_stream);

@@ -1,0 +1,174 @@
+// Device helpers shared by the demodulation kernels (qld_kernels.cu, qld_stream.cu): sample unpacking, the
+// per-frame multiply-accumulate ("multiplied by two numbers ... accumulated"), and the A4 epilogue.
+#pragma once
+#include <type_traits>
+
+#include "qld_internal.h"
+
+namespace qld_dev {
+
+// ---------------------------------------------------------------------------------------------------
+// streaming loads of V samples of type T (V * sizeof(T) bytes <= 16)
+// ---------------------------------------------------------------------------------------------------
+template <typename T, int V>
+struct Pix {
+    static constexpr int VB = V * (int)sizeof(T);
+    static constexpr int NW = (VB + 3) / 4;
+    static_assert(VB == 1 || VB == 2 || VB == 4 || VB == 8 || VB == 16, "vector width");
+
+    __device__ __forceinline__ static void load(const unsigned char *ptr, uint32_t (&w)[NW])
+    {
+        if constexpr (VB == 16) {
+            asm("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "l"(ptr));
+        } else if constexpr (VB == 8) {
+            asm("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(w[0]), "=r"(w[1]) : "l"(ptr));
+        } else if constexpr (VB == 4) {
+            asm("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(w[0]) : "l"(ptr));
+        } else if constexpr (VB == 2) {
+            w[0] = *reinterpret_cast<const unsigned short *>(ptr);
+        } else {
+            w[0] = *ptr;
+        }
+    }
+    // the same V samples from shared memory (TMA-staged tiles)
+    __device__ __forceinline__ static void load_shared(const unsigned char *ptr, uint32_t (&w)[NW])
+    {
+        if constexpr (VB == 16) {
+            const uint4 t = *reinterpret_cast<const uint4 *>(ptr);
+            w[0] = t.x; w[1] = t.y; w[2] = t.z; w[3] = t.w;
+        } else if constexpr (VB == 8) {
+            const uint2 t = *reinterpret_cast<const uint2 *>(ptr);
+            w[0] = t.x; w[1] = t.y;
+        } else if constexpr (VB == 4) {
+            w[0] = *reinterpret_cast<const uint32_t *>(ptr);
+        } else if constexpr (VB == 2) {
+            w[0] = *reinterpret_cast<const unsigned short *>(ptr);
+        } else {
+            w[0] = *ptr;
+        }
+    }
+    // sample j as an unsigned integer
+    __device__ __forceinline__ static uint32_t geti(const uint32_t (&w)[NW], int j)
+    {
+        if constexpr (sizeof(T) == 2) return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
+        else return (w[j >> 2] >> (8 * (j & 3))) & 0xffu;
+    }
+    // sample j as the float 2^23 + x (one byte-permute: the integer lands in the mantissa of 0x4B000000)
+    __device__ __forceinline__ static float getf_biased(const uint32_t (&w)[NW], int j)
+    {
+        uint32_t r;
+        if constexpr (sizeof(T) == 2) r = __byte_perm(w[j >> 1], 0x4B000000u, (j & 1) ? 0x7632u : 0x7610u);
+        else r = __byte_perm(w[j >> 2], 0x4B000000u, 0x7650u | (uint32_t)(j & 3));
+        return __uint_as_float(r);
+    }
+};
+
+// weights of one frame: ROWS values, identical for every thread (broadcast load through L1)
+template <typename ACC, int ROWS>
+__device__ __forceinline__ void load_weights(const ACC *row, ACC (&wt)[ROWS])
+{
+    if constexpr (ROWS % 4 == 0) {
+#pragma unroll
+        for (int q = 0; q < ROWS / 4; ++q) {
+            int4 t = __ldg(reinterpret_cast<const int4 *>(row) + q);
+            wt[4 * q + 0] = *reinterpret_cast<ACC *>(&t.x);
+            wt[4 * q + 1] = *reinterpret_cast<ACC *>(&t.y);
+            wt[4 * q + 2] = *reinterpret_cast<ACC *>(&t.z);
+            wt[4 * q + 3] = *reinterpret_cast<ACC *>(&t.w);
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < ROWS / 2; ++q) {
+            int2 t = __ldg(reinterpret_cast<const int2 *>(row) + q);
+            wt[2 * q + 0] = *reinterpret_cast<ACC *>(&t.x);
+            wt[2 * q + 1] = *reinterpret_cast<ACC *>(&t.y);
+        }
+    }
+}
+
+// the same from a shared-memory copy of the rows
+template <typename ACC, int ROWS>
+__device__ __forceinline__ void load_weights_shared(const ACC *row, ACC (&wt)[ROWS])
+{
+    if constexpr (ROWS % 4 == 0) {
+#pragma unroll
+        for (int q = 0; q < ROWS / 4; ++q) {
+            const int4 t = reinterpret_cast<const int4 *>(row)[q];
+            wt[4 * q + 0] = *reinterpret_cast<const ACC *>(&t.x);
+            wt[4 * q + 1] = *reinterpret_cast<const ACC *>(&t.y);
+            wt[4 * q + 2] = *reinterpret_cast<const ACC *>(&t.z);
+            wt[4 * q + 3] = *reinterpret_cast<const ACC *>(&t.w);
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < ROWS / 2; ++q) {
+            const int2 t = reinterpret_cast<const int2 *>(row)[q];
+            wt[2 * q + 0] = *reinterpret_cast<const ACC *>(&t.x);
+            wt[2 * q + 1] = *reinterpret_cast<const ACC *>(&t.y);
+        }
+    }
+}
+
+// acc[r][v] += x_v * w_r for one frame.  Float: x is pedestal-subtracted exactly, (2^23+x) - (2^23+ped).
+template <typename T, typename ACC, int ROWS, int V>
+__device__ __forceinline__ void accumulate(const uint32_t (&w)[Pix<T, V>::NW], const ACC (&wt)[ROWS], const float (&pedm)[V],
+                                           ACC (&acc)[ROWS][V])
+{
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        if constexpr (std::is_same<ACC, float>::value) {
+            float x = Pix<T, V>::getf_biased(w, v) - pedm[v];
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) acc[r][v] = fmaf(x, wt[r], acc[r][v]);
+        } else {
+            int x = (int)Pix<T, V>::geti(w, v);
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) acc[r][v] += x * wt[r];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// A4: finalise one pixel from its ROWS sums (already including the pedestal term), all in fp64.
+// ---------------------------------------------------------------------------------------------------
+template <int ROWS>
+__device__ __forceinline__ void finalise_pixel(const FinParams &f, const double (&val)[ROWS], int64_t pixel, int64_t HW)
+{
+    for (int k = 0; k < f.K; ++k) {
+        double S = 0.0, C = 0.0;
+        if (f.is_int) {
+            const int off = f.row_off[k], end = off + f.n_rows[k];
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r)
+                if (r >= off && r < end) {
+                    S += val[r] * f.sw[r];
+                    C += val[r] * f.cw[r];
+                }
+        } else {
+#pragma unroll
+            for (int r = 0; r + 1 < ROWS; r += 2)
+                if (r == 2 * k) {
+                    S = val[r];
+                    C = val[r + 1];
+                }
+        }
+        S *= f.scale;
+        C *= f.scale;
+        const int64_t o = (int64_t)k * HW + pixel;
+        if (f.I) f.I[o] = (float)S;
+        if (f.Q) f.Q[o] = (float)C;
+        if (f.amp) f.amp[o] = (float)sqrt(S * S + C * C);
+        if (f.phase) f.phase[o] = (S == 0.0 && C == 0.0) ? 0.0f : (float)atan2(C, S);
+    }
+}
+
+// pixels per thread for a (dtype, rows) pair: at most 16 bytes per load and at most 64 accumulators
+constexpr int pick_v(int bytes, int rows)
+{
+    int v = 16 / bytes;
+    while (v * rows > 64 && v > 1) v /= 2;
+    return v;
+}
+
+}  // namespace qld_dev

@@ -4,8 +4,8 @@
 // integers (kind::i8, int32 accumulators in TMEM).
 //
 // Why this shape.  The frame stack is frame-major, so for a fixed frame the bytes of adjacent pixels are
-// contiguous: the A operand [M = pixel bytes][K = frames] is "MN-major" and a TMA box {128 bytes, KC frames}
-// with 128-byte swizzle lands in shared memory in exactly the canonical layout tcgen05.mma reads -- the raw
+// contiguous: the A operand [M = pixel bytes][K = frames] is "MN-major" and TMA boxes of {128 bytes, 8 frames}
+// with 128-byte swizzle land in shared memory in exactly the canonical layout tcgen05.mma reads -- the raw
 // camera bytes go global -> shared -> tensor core with no conversion pass and no CUDA-core instruction per
 // sample.  A uint16 sample x = lo + 256*hi occupies two M rows (its two little-endian bytes); a reference
 // R = sum_j d_j 256^j is split into four signed base-256 digits d_j in [-128, 127] (four N columns).  The MMA
@@ -25,53 +25,21 @@
 #include <stdlib.h>
 
 #include "qld_internal.h"
+#include "qld_ptx.cuh"
 #include "qld_tc.h"
+
+using namespace qld_ptx;
 
 namespace {
 
-constexpr int KC = 64;            // frames per pipeline stage
+constexpr int KC_PAD = 64;        // the digit tiles are padded to a multiple of this many frames
 constexpr int SUB_BYTES = 128;    // pixel bytes per MMA M tile
 constexpr int MMA_K = 32;         // frames per tcgen05.mma (8-bit operands)
+constexpr int GRP = 8;            // frames per 128-byte-swizzle atom (8 rows of 128 bytes = 1 KB)
 
 // ---------------------------------------------------------------------------------------------------
 // PTX wrappers
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P1;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra WAIT_DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "WAIT_DONE:\n\t"
-        "}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, uint64_t hint)
-{
-    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4}], [%2], %5;"
-                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "l"(hint) : "memory");
-}
-__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint64_t *bar)
@@ -163,12 +131,11 @@ __global__ void k_digit_pack(const int32_t *rfix, int n_stride, int n, int rows,
 // ---------------------------------------------------------------------------------------------------
 // shared-memory carve-up for (NC columns, T spans per tile, STAGES pipeline stages)
 struct TcSmem {
-    int a_sub, a_stage, b_stage, off_b, off_bar, total;
-    __host__ __device__ TcSmem(int nc, int t, int stages)
+    int a_stage, b_stage, off_b, off_bar, total;
+    __host__ __device__ TcSmem(int nc, int t, int stages, int kc)
     {
-        a_sub = KC * SUB_BYTES;                       // 8 KB per 128-byte span per stage
-        a_stage = t * a_sub;
-        b_stage = (KC / MMA_K) * nc * MMA_K;
+        a_stage = t * kc * SUB_BYTES;                 // [kc/8 frame groups][t spans][8 frames][128 bytes]
+        b_stage = (kc / MMA_K) * nc * MMA_K;
         off_b = stages * a_stage;
         off_bar = off_b + stages * b_stage;
         total = off_bar + (2 * stages + 4) * 8 + 16 + 48;
@@ -176,9 +143,10 @@ struct TcSmem {
 };
 
 template <int NC, int BYTES>
-__global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap, const TcParams p, const int T, const int STAGES)
+__global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap2, const __grid_constant__ CUtensorMap tmap4,
+                                                     const TcParams p, const int T, const int STAGES, const int KC, const int use4d)
 {
-    const TcSmem SM(NC, T, STAGES);
+    const TcSmem SM(NC, T, STAGES, KC);
     extern __shared__ unsigned char smem_raw[];
     // 128-byte-swizzled TMA/UMMA tiles need 1024-byte alignment in the shared window
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -194,6 +162,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (p.N + KC - 1) / KC;
+    const int n_full = p.N / GRP * GRP;               // frames covered by whole 8-frame groups (the 4-D map's extent)
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + T - 1) / T;
 
@@ -235,12 +204,26 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
                 }
                 const int sub0 = tile * T;
                 const int nv = min(T, n_sub - sub0);
+                const uint64_t hint = 0x12F0000000000000ull;     // evict first: every sample is read once
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&empty[stage], phase ^ 1);
-                    mbar_expect_tx(&full[stage], (uint32_t)(nv * SM.a_sub + SM.b_stage));
-                    for (int t = 0; t < nv; ++t)
-                        tma_load_2d(sA + stage * SM.a_stage + t * SM.a_sub, &tmap, &full[stage], (sub0 + t) * SUB_BYTES, c * KC,
-                                    0x12F0000000000000ull /* evict first: every sample is read once */);
+                    unsigned char *dst = sA + stage * SM.a_stage;
+                    if (use4d && (c + 1) * KC <= n_full) {
+                        // one 4-D box {128 B, 8 frames, T spans, KC/8 groups}: the TMA walks the T adjacent spans of a
+                        // frame back to back, so DRAM sees T*128 contiguous bytes per frame (the probe: 2 KB segments
+                        // reach 7.0 TB/s where isolated 128-byte rows stop at 6.0)
+                        mbar_expect_tx(&full[stage], (uint32_t)(SM.a_stage + SM.b_stage));
+                        tma_load_4d(dst, &tmap4, &full[stage], 0, 0, sub0, c * (KC / GRP), hint);
+                    } else {
+                        // ragged tail in time (or a row pitch that is not a multiple of 128 B): 1 KB boxes, zero filled
+                        // beyond the last frame / last byte
+                        // groups wholly beyond the last frame are skipped: their digits are zero and integer 0 * stale = 0
+                        const int ng = min(KC / GRP, (p.N - c * KC + GRP - 1) / GRP);
+                        mbar_expect_tx(&full[stage], (uint32_t)(nv * ng * GRP * SUB_BYTES + SM.b_stage));
+                        for (int g = 0; g < ng; ++g)
+                            for (int t = 0; t < nv; ++t)
+                                tma_load_2d(dst + (g * T + t) * (GRP * SUB_BYTES), &tmap2, &full[stage], (sub0 + t) * SUB_BYTES, c * KC + g * GRP, hint);
+                    }
                     bulk_load(sB + stage * SM.b_stage, p.digits + (size_t)c * SM.b_stage, SM.b_stage, &full[stage]);
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
@@ -270,10 +253,9 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
                 if (lane == 0) {
                     const uint32_t a0 = smem_u32(sA + stage * SM.a_stage), b0 = smem_u32(sB + stage * SM.b_stage);
                     for (int t = 0; t < nv; ++t) {
-#pragma unroll
                         for (int ks = 0; ks < KC / MMA_K; ++ks) {
-                            // A: MN-major, 128-byte swizzle: rows of 128 pixel bytes, 8-frame atoms 1024 B apart (SBO)
-                            const uint64_t ad = smem_desc(a0 + t * SM.a_sub + ks * MMA_K * SUB_BYTES, SM.a_sub, 1024, 2);
+                            // A: MN-major, 128-byte swizzle: rows of 128 pixel bytes, 8-frame atoms T KB apart (SBO)
+                            const uint64_t ad = smem_desc(a0 + (ks * (MMA_K / GRP) * T + t) * (GRP * SUB_BYTES), T * GRP * SUB_BYTES, T * GRP * SUB_BYTES, 2);
                             // B: K-major, no swizzle: K halves 128 B apart (LBO), 8-column groups 256 B apart (SBO)
                             const uint64_t bd = smem_desc(b0 + ks * NC * MMA_K, 128, 256, 0);
                             tc_mma_i8(tmem_base + (uint32_t)(buf * T * NC + t * NC), ad, bd, idesc, (c | ks) ? 1u : 0u);
@@ -358,29 +340,50 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     }
 }
 
-template <int NC, int BYTES>
-cudaError_t launch_tc(const CUtensorMap &tmap, const TcParams &p, int n_sms, cudaStream_t st)
+// Tile shape for (NC columns, frame size): T spans (T*128 contiguous bytes of every frame per CTA tile; the wider,
+// the friendlier to DRAM), accumulators double buffered in the 512 TMEM columns; KC frames per stage; as many
+// stages as fit in shared memory.
+struct TcShape { int T, kc, stages, use4d; };
+
+TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms)
 {
-    // tile shape: T spans (T*128 contiguous bytes of every frame per CTA), accumulators double buffered in the
-    // 512 TMEM columns; as many 64-frame stages as fit in shared memory
-    int T = 512 / (2 * NC);
-    if (T > 4) T = 4;                                     // 512-byte spans: small tiles keep the tail short
-    int stages = (220 * 1024) / TcSmem(NC, T, 1).off_bar;
-    if (const char *e = getenv("QLD_TC_TILE")) {          // tuning override: "T,STAGES"
-        int t = 0, s2 = 0;
-        if (sscanf(e, "%d,%d", &t, &s2) == 2 && t >= 1 && 2 * t * NC <= 512 && s2 >= 2 && TcSmem(NC, t, s2).total + 1024 <= 227 * 1024) { T = t; stages = s2; }
+    TcShape sh;
+    const int n_sub = (int)((row_bytes + SUB_BYTES - 1) / SUB_BYTES);
+    // Measured on cfg2 (B200): the tensor pipe takes about 200 cycles to fetch one MN-major 8-bit A tile (128 bytes x
+    // 32 frames) from shared memory whatever N is, i.e. about 21 B/clk/SM = 6.1 TB/s over 148 SMs -- that, not HBM,
+    // bounds this kernel.  64-frame stages (two MMAs per span per barrier round trip) and 1 KB of contiguous
+    // bytes per frame were the best point of the sweep (T,stages,KC = 8,3,64: 6.17 TB/s; 16,3,32: 5.05; 4,6,64: 5.78).
+    int T = 512 / (2 * nc);
+    if (T > 8) T = 8;
+    while (T & (T - 1)) --T;                                        // power of two
+    while (T > 1 && (n_sub + T - 1) / T < 2 * n_sms) T /= 2;      // small frames: keep every SM busy
+    sh.T = T;
+    sh.kc = 64;
+    sh.stages = (200 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
+    if (const char *e = getenv("QLD_TC_TILE")) {          // tuning override: "T,STAGES,KC"
+        int t = 0, s2 = 0, kc = 0;
+        if (sscanf(e, "%d,%d,%d", &t, &s2, &kc) == 3 && t >= 1 && 2 * t * nc <= 512 && s2 >= 2 && (kc == 32 || kc == 64) &&
+            TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
     }
-    if (stages > 8) stages = 8;
-    const TcSmem SM(NC, T, stages);
+    if (sh.stages > 12) sh.stages = 12;
+    sh.use4d = (row_bytes % SUB_BYTES == 0 && N >= GRP) ? 1 : 0;
+    return sh;
+}
+
+template <int NC, int BYTES>
+cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
+{
+    const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms);
+    const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
     auto kern = k_demod_tc<NC, BYTES>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 1024);
     if (e != cudaSuccess) return e;
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
-    const int n_tiles = (n_sub + T - 1) / T;
+    const int n_tiles = (n_sub + sh.T - 1) / sh.T;
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
     e = cudaMemsetAsync(p.tile_counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) return e;
-    kern<<<grid, 192, SM.total + 1024, st>>>(tmap, p, T, stages);
+    kern<<<grid, 192, SM.total + 1024, st>>>(tmaps[0], tmaps[1], p, sh.T, sh.stages, sh.kc, sh.use4d);
     return cudaGetLastError();
 }
 
@@ -394,11 +397,15 @@ int qld_tc_columns(int K) { const int c = 8 * K; return (c + 15) / 16 * 16; }
 
 size_t qld_tc_digit_bytes(int K, int N)
 {
-    const int n_chunks = (N + KC - 1) / KC;
-    return (size_t)n_chunks * (KC / MMA_K) * qld_tc_columns(K) * MMA_K;
+    const int n_chunks = (N + KC_PAD - 1) / KC_PAD;
+    return (size_t)n_chunks * (KC_PAD / MMA_K) * qld_tc_columns(K) * MMA_K;
 }
 
-cudaError_t qld_tc_encode_tmap(void *tmap_out, const void *frames, int64_t row_bytes, int n_frames)
+// Two tensor maps over the frame stack, written to tmaps_out[0..1]:
+//  [0] 2-D {row bytes, frames}, box {128 B, 8 frames}: one swizzle atom, any shape (zero fill beyond the edges);
+//  [1] 4-D {128 B, 8 frames, spans, frame groups}, box {128, 8, T, KC/8}: a whole pipeline stage in one copy,
+//      spans innermost in the walk.  Only valid (and only used) when row_bytes % 128 == 0 and N >= 8.
+cudaError_t qld_tc_encode_tmap(void *tmaps_out, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms)
 {
     static EncodeTiledFn fn = nullptr;
     if (!fn) {
@@ -409,14 +416,31 @@ cudaError_t qld_tc_encode_tmap(void *tmap_out, const void *frames, int64_t row_b
         if (!sym || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
         fn = reinterpret_cast<EncodeTiledFn>(sym);
     }
-    const cuuint64_t dims[2] = {(cuuint64_t)row_bytes, (cuuint64_t)n_frames};
-    const cuuint64_t strides[1] = {(cuuint64_t)row_bytes};
-    const cuuint32_t box[2] = {SUB_BYTES, KC};
-    const cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(reinterpret_cast<CUtensorMap *>(tmap_out), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(frames), dims, strides, box,
-                    estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+    CUtensorMap *tm = reinterpret_cast<CUtensorMap *>(tmaps_out);
+    {
+        const cuuint64_t dims[2] = {(cuuint64_t)row_bytes, (cuuint64_t)n_frames};
+        const cuuint64_t strides[1] = {(cuuint64_t)row_bytes};
+        const cuuint32_t box[2] = {SUB_BYTES, GRP};
+        const cuuint32_t estr[2] = {1, 1};
+        CUresult r = fn(&tm[0], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void *>(frames), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    const TcShape sh = tc_shape(qld_tc_columns(K), row_bytes, n_frames, n_sms);
+    if (sh.use4d) {
+        const cuuint64_t dims[4] = {SUB_BYTES, GRP, (cuuint64_t)(row_bytes / SUB_BYTES), (cuuint64_t)(n_frames / GRP)};
+        const cuuint64_t strides[3] = {(cuuint64_t)row_bytes, SUB_BYTES, (cuuint64_t)row_bytes * GRP};
+        const cuuint32_t box[4] = {SUB_BYTES, GRP, (cuuint32_t)sh.T, (cuuint32_t)(sh.kc / GRP)};
+        const cuuint32_t estr[4] = {1, 1, 1, 1};
+        CUresult r = fn(&tm[1], CU_TENSOR_MAP_DATA_TYPE_UINT8, 4, const_cast<void *>(frames), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    } else {
+        tm[1] = tm[0];
+    }
+    return cudaSuccess;
 }
 
 cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st)
@@ -428,15 +452,15 @@ cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix,
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st)
 {
     const int nc = qld_tc_columns(K);
-    const int n_steps = (N + KC - 1) / KC * (KC / MMA_K);
+    const int n_steps = (N + KC_PAD - 1) / KC_PAD * (KC_PAD / MMA_K);
     const int64_t total = (int64_t)n_steps * nc * MMA_K;
     k_digit_pack<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(rfix, n_stride, N, 2 * K, nc, n_steps, digits);
     return cudaGetLastError();
 }
 
-cudaError_t qld_launch_demod_tc(const void *tmap, const TcParams &p, int n_sms, cudaStream_t st)
+cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
-    const CUtensorMap &tm = *reinterpret_cast<const CUtensorMap *>(tmap);
+    const CUtensorMap *tm = reinterpret_cast<const CUtensorMap *>(tmaps);
     const int nc = qld_tc_columns(p.fin.K);
     if (p.bytes == 2) {
         switch (nc) {

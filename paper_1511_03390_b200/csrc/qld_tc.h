@@ -18,7 +18,7 @@ struct TcParams {
 
 int qld_tc_columns(int K);                       // N columns of the MMA: 8 per reference, padded to 16
 size_t qld_tc_digit_bytes(int K, int N);
-cudaError_t qld_tc_encode_tmap(void *tmap_out /*128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames);
+cudaError_t qld_tc_encode_tmap(void *tmaps_out /*2 x 128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms);
 cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st);
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
-cudaError_t qld_launch_demod_tc(const void *tmap, const TcParams &p, int n_sms, cudaStream_t st);
+cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);

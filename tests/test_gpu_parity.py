@@ -299,3 +299,90 @@ def test_device_generator_is_bit_identical_to_numpy(Q):
         dev = Q.synth_fill(wl.scene, 3 if wl.scene.n_frames > 20 else 1, n)
         host = synth.frames(wl.scene, 3 if wl.scene.n_frames > 20 else 1, n)
         assert np.array_equal(dev.cpu().numpy(), host), wl.name
+
+
+# ------------------------------------------------------------------------------------------------ TMA-fed kernel
+# k_demod_stream takes over for large frames; QLD_STREAM_TILE = "SEG,KC" forces it (and its tile shape) on small ones.
+STREAM_TILES = ["512,16", "1024,16", "2048,16", "2048,32", "256,32", "1024,64"]
+
+
+@pytest.mark.parametrize("tile", STREAM_TILES)
+@pytest.mark.parametrize("H,W,N,dtype", [(16, 200, 70, np.uint16), (9, 136, 16, np.uint16), (50, 128, 9, np.uint8), (37, 48, 129, np.uint16),
+                                         (25, 64, 3, np.uint16), (33, 256, 100, np.uint8), (128, 320, 40, np.uint16)])
+def test_stream_kernel_fp32_tiles(Q, oracle, monkeypatch, tile, H, W, N, dtype):
+    """Every tile shape (column groups x time slices), ragged last tile, ragged last stage, fewer frames than a stage."""
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(H + W + N)
+    x = _rand_stack(rng, N, H, W, dtype)
+    ref = {"nu": 0.0937, "phase": 0.3}
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.demod(Q.QLD_WHOLE)             # second launch: cached tensor map, tile counter reset
+    ctx.sync()
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), what=f"stream {tile} {H}x{W} N={N}")
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("tile", ["512,16", "2048,16"])
+@pytest.mark.parametrize("K", [2, 3, 8])
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
+def test_stream_kernel_multi_reference(Q, oracle, monkeypatch, tile, K, dtype):
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(K)
+    H, W, N = 24, 256, 130
+    x = _rand_stack(rng, N, H, W, dtype)
+    refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FP32)
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    for k in range(K):
+        check_float_maps(_maps(ctx, k), oracle_maps(oracle, x, refs[k]), what=f"stream K={K} k={k}")
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("tile", ["512,16", "2048,16", "1024,32"])
+@pytest.mark.parametrize("den,dtype", [(4, np.uint8), (6, np.uint16), (8, np.uint8), (5, np.uint16), (16, np.uint16)])
+def test_stream_kernel_integer_bins_bit_exact(Q, oracle, monkeypatch, tile, den, dtype):
+    """A3' through the TMA-fed kernel: int32 phase bins bit-exact against the int64 oracle."""
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(den)
+    H, W, N = 20, 192, 150
+    hi = 256 if dtype == np.uint8 else 65536
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    ref = {"num": 1, "den": den}
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_INT_BINS)
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    rows = ctx.get_bins(0).cpu().numpy().astype(np.int64)
+    bins = oracle.bins(x, 1, den)
+    if den % 2 == 0:
+        exp = bins[: den // 2] - bins[den // 2:]
+    else:
+        exp = bins
+    assert np.array_equal(rows, exp)
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), rel=1e-6, what=f"stream bins den={den}")
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("tile", ["512,16", "2048,16"])
+def test_stream_kernel_ring_wraparound(Q, oracle, monkeypatch, tile):
+    """QLD_WHOLE on a ring whose window straddles the wrap: two runs of slots, weights by absolute frame index."""
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(7)
+    H, W, N, cap = 16, 128, 40, 56
+    total = 152
+    x = _rand_stack(rng, total, H, W, np.uint16)
+    ref = {"nu": 0.0937, "phase": 0.3}
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_FP32)
+    pushed = 0
+    for b in (40, 8, 16, 8, 16, 16, 16, 16, 16):
+        ctx.push_frames(x[pushed:pushed + b])
+        pushed += b
+        ctx.demod(Q.QLD_WHOLE)
+        ctx.sync()
+        win = x[pushed - N:pushed]
+        check_float_maps(_maps(ctx), oracle_maps(oracle, win, ref, s_first=pushed - N + 1), what=f"ring whole at {pushed}")
+    ctx.destroy()

@@ -84,6 +84,55 @@ def test_fixed_multi_reference(Q, oracle, K, dtype):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("tile", ["16,3,32", "8,6,32", "4,6,64", "2,8,64", "1,8,32"])
+@pytest.mark.parametrize("H,W,N,dtype", [(16, 200, 70, np.uint16), (16, 200, 64, np.uint16), (50, 128, 9, np.uint8), (37, 48, 129, np.uint16),
+                                         (25, 64, 7, np.uint16), (33, 256, 100, np.uint8)])
+def test_fixed_tile_shapes_bit_exact(Q, oracle, monkeypatch, tile, H, W, N, dtype):
+    """Every tile shape the launcher can pick (T spans x KC frames per stage), forced through the tuning override, on
+    stacks with a ragged last tile, a ragged last 8-frame group, fewer than 8 frames, and a row pitch that is not a
+    multiple of 128 bytes (the 1 KB-box path): bit-exact int64 sums."""
+    monkeypatch.setenv("QLD_TC_TILE", tile)
+    rng = np.random.default_rng(H + W + N)
+    hi = 256 if dtype == np.uint8 else 65536
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    refs = [{"nu": 0.0937, "phase": 0.3}, {"num": 1, "den": 6}]
+    tabs = [_q30(oracle, r, N) for r in refs]
+    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
+    for k in range(2):
+        ctx.set_ref_table_fixed(k, *tabs[k])
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.demod()                                              # a second launch reuses the tensor maps and the tile counter
+    ctx.sync()
+    for k in range(2):
+        oI, oQ = oracle.demod_int(x, *tabs[k])
+        gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
+        assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"k={k}"
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("K", [1, 3, 8])
+def test_fixed_wide_tiles_large_frame(Q, oracle, K):
+    """A frame large enough that the launcher itself picks the widest tiles (T = 16 / 8 / 4 spans for K = 1 / 3 / 8),
+    with a ragged last tile (4810 spans) and a ragged last frame group (N = 70)."""
+    rng = np.random.default_rng(K)
+    H, W, N = 481, 640, 70
+    x = rng.integers(0, 4096, size=(N, H, W)).astype(np.uint16)
+    refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
+    tabs = [_q30(oracle, r, N) for r in refs]
+    ctx = Q.QLD(H, W, "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_AMP | Q.QLD_MAP_SUMS_I64)
+    for k in range(K):
+        ctx.set_ref_table_fixed(k, *tabs[k])
+    ctx.push_frames(x)
+    ctx.demod()
+    ctx.sync()
+    for k in range(K):
+        oI, oQ = oracle.demod_int(x, *tabs[k])
+        gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
+        assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"k={k}"
+    ctx.destroy()
+
+
 def test_fixed_own_table_meets_float_tolerance_on_cfg2_shape(Q, oracle):
     from paper_1511_03390_b200 import synth
     wl = synth.cfg2(H=64, W=160, N=1024)
