@@ -4,10 +4,14 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A step is one pass of the hot path over one window of synthetic frames of the named BASELINE.json config:
-qld_demod (reference tables were built by qld_create, A1) = A3/A3'/A6 demodulation + A4 finalise, with the
-frames resident in HBM (`value`), and the same through host buffers -- qld_push_frames from pinned memory (A2),
-qld_demod, qld_read_map of the amplitude map back to the host -- for `e2e`.  Prints ONE JSON line (rank 0).
+A step is one pass of the hot path over one batch of synthetic frames of the named BASELINE.json config.
+Whole-window workloads (cfg0, cfg1, cfg2, cfg4): one window of N frames -> qld_demod(QLD_WHOLE) = A3/A3'/A6
+demodulation + A4 finalise (reference tables, A1, were built by qld_create).  Streaming workload (cfg3): one
+batch of `hop` new frames -> qld_commit_frames (A1 table extension + A2 without a copy: frames are resident)
+-> qld_demod(QLD_SLIDE) = A5 update + A4.  `value` has the frames resident in HBM; `e2e` runs the same step
+from pinned host buffers: qld_push_frames (A2), qld_demod, qld_read_map of the amplitude map(s) to the host.
+Prints ONE JSON line (rank 0).  With the default flags at N = 1 the line also carries, under "also", a short
+run of the other large configs (cfg4 on the tensor cores, cfg3 sliding) so one run covers every row of 8(a).
 """
 from __future__ import annotations
 
@@ -107,13 +111,16 @@ def run_reference(args, rank, world):
     t = 0.0
     for _ in range(args.steps):
         t += oracle_on_rows(wl, x, refs, nt)[1]
-    samples = float(x.size) * args.steps
+    # streaming workload: a step is one hop; the oracle recomputes the whole window for it (never incremental)
+    per_step = float(wl.hop * rows * sc.W) if args.workload == "cfg3" else float(x.size)
+    samples = per_step * args.steps
     val = samples / t
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f80 (x87 long double) / int64", "data": "synthetic",
             "config": {"workload": args.workload, "H": sc.H, "W": sc.W, "N": wl.N, "K": len(refs),
-                       "sample": f"first {rows} rows x {sc.W} cols x {wl.N} frames per step"},
+                       "sample": f"first {rows} rows x {sc.W} cols x {wl.N} frames per step"
+                                 + (f" (one window recomputed per hop of {wl.hop} frames; value counts the hop's new samples)" if args.workload == "cfg3" else "")},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": nt, "kind": "oracle",
                              "sample": f"{rows} rows x {sc.W} x {wl.N} frames ({x.size} samples) per step"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -121,119 +128,138 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg4"])
-    ap.add_argument("--accum", default="auto", choices=["auto", "fp32", "bins", "fixed"])
-    ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--ref-rows", type=int, default=0, help="rows of the frame the CPU oracle is timed / checked on "
-                    "(0: sized for about 15 CPU-seconds of oracle work; 32 for --impl reference)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
-        run_reference(args, rank, world)
-        return
 
-    import numpy as np
-    import torch
-    import torch.distributed as dist
-    from paper_1511_03390_b200 import qld, synth
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+ACCUM_NAMES = {"auto": 0, "fp32": 1, "bins": 2, "fixed": 3}
 
-    wl = build_workload(args.workload, rank)
+
+class Env:
+    """Rank / device / barrier plumbing shared by the workload runners."""
+
+    def __init__(self, args):
+        import torch
+        self.torch = torch
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+        torch.cuda.set_device(self.local_rank)
+        self.dev = torch.device("cuda", self.local_rank)
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            dist.init_process_group("nccl", device_id=self.dev)
+            self.dist = dist
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        t = self.torch.tensor([x], device=self.dev, dtype=self.torch.float64)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def timed(self, step, steps: int, warmup: int, keep_busy=None, counter=None):
+        """warmup untimed steps, then exactly `steps` steps between CUDA events on the launching stream (torch's
+        current stream is the context's compute stream), barrier + synchronize on both sides, max over ranks.
+        `counter()` (kernel launches so far) is read on both sides of the timed region.
+        Returns (ms, clocks, launches)."""
+        torch = self.torch
+        for _ in range(warmup):
+            step()
+        self.barrier()
+        sampler = ClockSampler(self.local_rank)
+        sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.barrier()
+        c0 = counter() if counter else 0
+        ev0.record()
+        for _ in range(steps):
+            step()
+        ev1.record()
+        self.barrier()
+        ms = ev0.elapsed_time(ev1)
+        launches = (counter() - c0) if counter else None
+        # keep the GPU busy a little longer if the region was too short for a clock sample
+        t_end = time.time() + 0.25
+        while keep_busy is not None and len(sampler.samples) < 8 and time.time() < t_end:
+            keep_busy()
+            torch.cuda.synchronize()
+        sampler.stop_flag = True
+        sampler.join()
+        return self.max_over_ranks(ms), sampler.result(), launches
+
+
+def load_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` summaries (profiles/traffic.json, written by hand from profiles/*.md); None if absent."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(tpath)).get(workload, {}).get(kernel)
+    except Exception:
+        return None
+
+
+def roofline_hbm(algo_bytes: float, ms_per_launch: float, workload: str, kernel: str, notes=None):
+    peak, peak_src = load_peaks()
+    achieved = algo_bytes / (ms_per_launch * 1e-3) / 1e9
+    r = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+         "traffic": load_traffic(workload, kernel), "peak_source": peak_src, "algorithmic_bytes_per_launch": algo_bytes,
+         "frac_of_nominal_8TBps": achieved / 8000.0, "kernel": kernel}
+    if notes:
+        r["note"] = notes
+    return r
+
+
+def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warmup: int, e2e_steps: int, with_cpu: bool):
+    """Whole-window workloads (8(a) rows A1, A3/A3'/A6, A4; A2 in the e2e leg)."""
+    torch = env.torch
+    from paper_1511_03390_b200 import qld
+    wl = build_workload(workload, env.rank)
     sc = wl.scene
     N, H, W, K = wl.N, sc.H, sc.W, len(wl.refs)
-    bytes_per = 1 if sc.dtype == "u8" else 2
-    accum = {"auto": qld.QLD_ACC_AUTO, "fp32": qld.QLD_ACC_FP32, "bins": qld.QLD_ACC_INT_BINS, "fixed": qld.QLD_ACC_FIXED}[args.accum]
-
-    # ---- inputs: synthetic stack filled on the device, resident before the timed region -------------
-    frames = qld.synth_fill(sc, 1, N, device=dev)
+    b = 1 if sc.dtype == "u8" else 2
+    refs = [dict(r) for r in wl.refs]
+    accum = ACCUM_NAMES[accum_name]
+    # inputs: the synthetic stack, filled on the device, resident before the timed region
+    frames = qld.synth_fill(sc, 1, N, device=env.dev)
     torch.cuda.synchronize()
-    ctx = qld.QLD(H, W, sc.dtype, N, [dict(r) for r in wl.refs], ring_frames=-1, accum=accum, maps=qld.QLD_MAP_ALL,
-                  max_value=sc.maxval)
+    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=-1, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval)
     ctx.attach_frames_device(frames)
-    is_int = False
-    try:
-        ctx.get_bins(0)
-        is_int = True
-    except qld.QLDError:
-        pass
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
+    def step():
         ctx.demod(qld.QLD_WHOLE)
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    l0 = ctx.kernel_launches()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    for _ in range(args.steps):
-        ctx.demod(qld.QLD_WHOLE)
-    ev1.record()
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    launches = ctx.kernel_launches() - l0
-    # keep the GPU busy a little longer if the region was too short for a clock sample
-    t_end = time.time() + 0.25
-    while len(sampler.samples) < 8 and time.time() < t_end:
-        ctx.demod(qld.QLD_WHOLE)
-        torch.cuda.synchronize()
-    sampler.stop_flag = True
-    sampler.join()
-    if world > 1:
-        t = torch.tensor([ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    samples_per_step = float(N) * H * W
-    value = world * samples_per_step * args.steps / (ms * 1e-3)
 
-    # ---- roofline of the dominant kernel (the demodulation kernel is the only launch of a step) -----
-    n_maps = 4
-    algo_bytes = samples_per_step * bytes_per + n_maps * K * H * W * 4.0
-    peak, peak_src = load_peaks()
-    achieved = algo_bytes / (ms * 1e-3 / args.steps) / 1e9
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
-    if os.path.exists(tpath):
-        try:
-            traffic = json.load(open(tpath)).get(args.workload)
-        except Exception:
-            traffic = None
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": algo_bytes,
-                "frac_of_nominal_8TBps": achieved / 8000.0, "kernel": "k_demod_tc" if args.accum == "fixed" else "k_demod_whole"}
+    ms, clocks, launches = env.timed(step, steps, warmup, keep_busy=step, counter=ctx.kernel_launches)
+    kernel = ctx.last_kernel()
+    mode = ctx.accum_name()
+    samples = float(N) * H * W
+    res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
+           "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel}
+    res["gpu_launches"] = int(launches)
+    algo = samples * b + 4.0 * K * H * W * 4.0               # every sample once + four fp32 maps per reference
+    in_l2 = samples * b <= 126e6
+    res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
+                                   "input fits the 126 MB L2 and is re-read every step: L2-resident, not an HBM number" if in_l2 else None)
+    res["dtype"] = {"INT_BINS": "int32", "FIXED": "int8 x int8 -> int32 -> int64 (tcgen05)", "FP32": "f32"}[mode]
+    res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype, "accum": mode,
+                     "maps": "I,Q,amplitude,phase", "step": "qld_demod(QLD_WHOLE) over the resident stack",
+                     "cache": f"input {samples * b / 1e6:.0f} MB per step " + ("<= 126 MB L2: L2-resident" if in_l2 else "> 126 MB L2: no flush needed"),
+                     "parallelism": f"{env.world} x independent stacks (pixels are independent; no collective)"}
 
-    # ---- end to end through host buffers (pinned): push + demod + read amplitude map back ------------
-    e2e = None
-    parity = None
-    if (rank == 0 or world > 1) and args.e2e_steps > 0:
+    # ---- end to end through host buffers (pinned): push + demod + read amplitude maps back ---------
+    if e2e_steps > 0:
         host = torch.empty((N, H, W), dtype=frames.dtype).pin_memory()
         host.copy_(frames)
         amp_host = torch.empty((K, H, W), dtype=torch.float32).pin_memory()
         torch.cuda.synchronize()
-        ectx = qld.QLD(H, W, sc.dtype, N, [dict(r) for r in wl.refs], ring_frames=0, accum=accum, maps=qld.QLD_MAP_ALL,
-                       max_value=sc.maxval)
-        chunk = max(1, min(N, (256 << 20) // (H * W * bytes_per)))       # pushes of about 256 MiB
+        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=0, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval)
+        chunk = max(1, min(N, (256 << 20) // (H * W * b)))       # pushes of about 256 MiB
 
         def e2e_step():
             ectx.reset()
@@ -245,62 +271,236 @@ def main():
             ectx.sync()
 
         e2e_step()
-        barrier()
+        env.barrier()
         t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
+        for _ in range(e2e_steps):
             e2e_step()
-        barrier()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * samples_per_step * args.e2e_steps / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(samples_per_step * bytes_per), "d2h_bytes_per_step": int(K * H * W * 4),
-               "ms_per_step": 1e3 * dt / args.e2e_steps, "h2d_GBps": samples_per_step * bytes_per * args.e2e_steps / dt / 1e9,
-               "steps": args.e2e_steps, "note": "pinned host stack -> qld_push_frames -> qld_demod -> qld_read_map(amp) -> host"}
+        env.barrier()
+        dt = env.max_over_ranks(time.perf_counter() - t0)
+        res["e2e"] = {"value": env.world * samples * e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(samples * b),
+                      "d2h_bytes_per_step": int(K * H * W * 4), "ms_per_step": 1e3 * dt / e2e_steps,
+                      "h2d_GBps": samples * b * e2e_steps / dt / 1e9, "steps": e2e_steps,
+                      "note": "pinned host stack -> qld_push_frames -> qld_demod -> qld_read_map(amp) -> host"}
         ectx.destroy()
         del host
 
-    # ---- CPU baseline (the oracle, as it stands) + parity of the timed configuration on the same rows -
-    cpu = None
-    if rank == 0 and not args.no_cpu_baseline:
+    # ---- CPU baseline (the oracle, as it stands) + parity of the timed configuration on the same rows
+    if with_cpu and env.rank == 0:
         import oracle
         from _parity import check_float_maps
-        # about 15 CPU-seconds of oracle work at ~9e7 sample-references per second per core
-        rows = max(1, min(H, args.ref_rows or -(-int(1.35e9) // (K * N * W))))
+        nt = oracle.max_threads()
+        # about 15 s of oracle work at ~1.4e8 sample-references per second per core
+        rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (K * N * W))))
         r0 = (H // 2 - rows // 2)
         sub = frames[:, r0:r0 + rows, :].contiguous().cpu().numpy()
-        nt = oracle.max_threads()
-        refs = [dict(r) for r in wl.refs]
         oracle_on_rows(wl, sub[:8], refs[:1], nt)                      # thread pool warm-up
         out, secs = oracle_on_rows(wl, sub, refs, nt)
-        cpu = {"value": float(sub.size) / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
-               "sample": f"rows {r0}..{r0 + rows - 1} x {W} cols x {N} frames x {K} refs = {sub.size} samples, {secs:.2f} s"}
+        res["cpu_baseline"] = {"value": float(sub.size) / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
+                               "sample": f"rows {r0}..{r0 + rows - 1} x {W} cols x {N} frames x {K} refs = {sub.size} samples, {secs:.2f} s"}
         ctx.demod(qld.QLD_WHOLE)
         ctx.sync()
         worst = 0.0
+        tol = 1e-6 if mode == "INT_BINS" else 1e-5
         for k in range(K):
             got = tuple(m[r0:r0 + rows].cpu().numpy() for m in ctx.get_maps(k))
-            worst = max(worst, check_float_maps(got, out[k], rel=(1e-6 if is_int else 1e-5), what=f"bench parity k={k}"))
-        parity = {"rows_checked": rows, "refs_checked": K, "tolerance": "1e-6 (bins, fp64 combine)" if is_int else "1e-5 floored at map median",
-                  "strict_max_rel_err_amp": worst, "ok": True}
-
-    if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "int32 (phase bins)" if is_int else ("int8 x int8 -> int32/int64 (tcgen05, Q1.30 references)" if args.accum == "fixed" else "f32"), "data": "synthetic",
-                "config": {"workload": args.workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype,
-                           "accum": "INT_BINS" if is_int else ("FIXED (tensor cores)" if args.accum == "fixed" else "FP32 (pedestal)"), "maps": "I,Q,amplitude,phase",
-                           "cache": f"input {samples_per_step * bytes_per / 1e6:.0f} MB per step "
-                                    + ("> 126 MB L2: no flush needed" if samples_per_step * bytes_per > 3e8 else "<= L2: L2-resident, not an HBM number"),
-                           "parallelism": f"{world} x independent stacks (pixels are independent; no collective)"},
-                "maps_per_s": value / samples_per_step, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
-                "gpu_launches": int(launches), "clocks": sampler.result(), "parity": parity}
-        print(json.dumps(line), flush=True)
+            worst = max(worst, check_float_maps(got, out[k], rel=tol, what=f"bench parity k={k}"))
+        res["parity"] = {"rows_checked": rows, "refs_checked": K, "tolerance": f"{tol:g} relative, floored at the map median",
+                         "strict_max_rel_err_amp": worst, "ok": True}
     ctx.destroy()
-    if world > 1:
-        dist.destroy_process_group()
+    del frames
+    torch.cuda.empty_cache()
+    return res
+
+
+def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warmup: int, e2e_steps: int, with_cpu: bool):
+    """Streaming workload cfg3 (8(a) rows A1, A2, A5, A4): one step = one batch of `hop` new frames -> one map."""
+    torch = env.torch
+    from paper_1511_03390_b200 import qld, synth
+    wl = build_workload(workload, env.rank)
+    sc = wl.scene
+    N, H, W, K, hop = wl.N, sc.H, sc.W, len(wl.refs), wl.hop
+    b = 1 if sc.dtype == "u8" else 2
+    tdt = torch.uint8 if b == 1 else torch.uint16
+    refs = [dict(r) for r in wl.refs]
+    accum = ACCUM_NAMES[accum_name]
+    maps = qld.QLD_MAP_AMP                                   # BASELINE.json configs[3]: one amplitude map per hop
+    # inputs resident in HBM: the first T frames of the stream, written in place into the (external) ring
+    n_hops = warmup + steps
+    T = min(sc.n_frames, N + n_hops * hop)
+    ring = torch.empty((T, H, W), dtype=tdt, device=env.dev)
+    for a in range(0, T, 256):
+        qld.synth_fill(sc, a + 1, min(256, T - a), out=ring[a:a + 256])
+    torch.cuda.synchronize()
+    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=maps, max_value=sc.maxval, external_store=True)
+    ctx.attach_frames_device(ring)
+    ctx.commit_frames(N)
+    ctx.demod(qld.QLD_SLIDE, hop)                            # window 0: whole-window kernel seeds the accumulators
+    ctx.sync()
+    seed_kernel = ctx.last_kernel()
+
+    def step():                                              # past frame T the ring wraps: same bytes, same traffic
+        ctx.commit_frames(hop)
+        ctx.demod(qld.QLD_SLIDE, hop)
+
+    ms, clocks, launches = env.timed(step, steps, warmup, keep_busy=step, counter=ctx.kernel_launches)
+    kernel = ctx.last_kernel()
+    mode = ctx.accum_name()
+    n_rows = ctx.get_bins(0).shape[0] if mode == "INT_BINS" else 2 * K
+    acc_bytes = 4 if mode == "INT_BINS" else 8
+    samples = float(hop) * H * W                              # new pixel-samples consumed per step
+    res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
+           "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel, "gpu_launches": int(launches),
+           "window_samples_per_s": env.world * float(N) * H * W * steps / (ms * 1e-3)}
+    # per pixel: hop new + hop expired samples, accumulators read-modify-write, one amplitude map
+    algo = H * W * (2.0 * hop * b + 2.0 * n_rows * acc_bytes + 4.0 * K)
+    res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
+                                   f"per pixel 2*hop*{b} B of frames + {n_rows} x {acc_bytes} B accumulators read and written + 4 B map; "
+                                   f"a recompute would read {N * b} B")
+    res["dtype"] = {"INT_BINS": "int32", "FP32": "f32"}[mode]
+    res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "hop": hop, "K": K, "input_dtype": sc.dtype, "accum": mode,
+                     "maps": "amplitude", "step": "qld_commit_frames(hop) + qld_demod(QLD_SLIDE, hop) over the resident ring",
+                     "ring_frames": T, "seed_kernel": seed_kernel,
+                     "cache": f"{2 * hop * H * W * b / 1e6:.0f} MB of frames per step, each read once > 126 MB L2: no flush needed"
+                              if 2 * hop * H * W * b > 126e6 else f"{2 * hop * H * W * b / 1e6:.0f} MB of frames per step; new frames were "
+                              "written N/hop steps (> L2) earlier, so both reads miss L2",
+                     "parallelism": f"{env.world} x independent streams (pixels are independent; no collective)"}
+
+    # ---- CPU baseline + parity: windows recomputed directly by the oracle on a band of rows ---------
+    if with_cpu and env.rank == 0:
+        import oracle
+        from _parity import check_float_maps
+        nt = oracle.max_threads()
+        n_win = 4
+        rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (n_win * K * N * W))))
+        r0 = H // 2 - rows // 2                               # the moving disk crosses these rows
+        pctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval, external_store=True)
+        pctx.attach_frames_device(ring)
+        pctx.commit_frames(N)
+        pctx.demod(qld.QLD_SLIDE, hop)
+        last_w = min((T - N) // hop, warmup + steps)
+        check_at = sorted(set([0, 1, last_w // 2, last_w]))[:n_win]
+        secs, worst, done = 0.0, 0.0, 0
+        for w in range(0, last_w + 1):
+            if w > 0:
+                pctx.commit_frames(hop)
+                pctx.demod(qld.QLD_SLIDE, hop)
+            if w in check_at:
+                pctx.sync()
+                sub = ring[w * hop:w * hop + N, r0:r0 + rows, :].contiguous().cpu().numpy()
+                t0 = time.perf_counter()
+                out = [oracle.qld(sub, r, s_first=w * hop + 1, nthreads=nt) for r in refs]
+                secs += time.perf_counter() - t0
+                done += 1
+                for k in range(K):
+                    got = tuple(None if m is None else m[r0:r0 + rows].cpu().numpy() for m in pctx.get_maps(k))
+                    worst = max(worst, check_float_maps(got, out[k], rel=1e-6 if mode == "INT_BINS" else 1e-5, what=f"bench parity cfg3 window {w}"))
+        res["cpu_baseline"] = {"value": done * float(hop) * rows * W / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
+                               "sample": f"{done} windows (w = {check_at}) recomputed directly from the definition on rows {r0}..{r0 + rows - 1}: "
+                                         f"{done} x {N} x {rows} x {W} sample-products, {secs:.2f} s; value counts hop x rows x W new samples per window",
+                               "window_samples_per_s": done * float(N) * rows * W / secs}
+        res["parity"] = {"rows_checked": rows, "windows_checked": check_at, "tolerance": "1e-6" if mode == "INT_BINS" else "1e-5 floored",
+                         "strict_max_rel_err_amp": worst, "ok": True}
+        pctx.destroy()
+    ctx.destroy()
+    del ring
+    torch.cuda.empty_cache()
+
+    # ---- end to end: pinned host batches -> qld_push_frames (ring owned by the library) -> slide -> amp to host
+    if e2e_steps > 0:
+        batch = wl.batch
+        n_rot = 4                                             # rotate over a few pinned batches (the stream is 34 GB)
+        host = torch.empty((n_rot, batch, H, W), dtype=tdt).pin_memory()
+        for i in range(n_rot):
+            host[i].copy_(qld.synth_fill(sc, 1 + i * batch, batch, device=env.dev))
+        amp_host = torch.empty((2, K, H, W), dtype=torch.float32).pin_memory()
+        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=N + hop + 2 * batch, accum=accum, maps=maps, max_value=sc.maxval)
+        for i in range(N // batch):
+            ectx.push_frames(host[i % n_rot])
+        ectx.demod(qld.QLD_SLIDE, hop)
+        ectx.sync()
+        it = [0]
+
+        def e2e_step():
+            i = it[0]
+            it[0] += 1
+            ectx.push_frames(host[i % n_rot])
+            ectx.demod(qld.QLD_SLIDE, hop)
+            for k in range(K):
+                ectx.read_map(k, qld.QLD_MAP_AMP, amp_host[i & 1, k])
+            if i & 1:
+                ectx.sync()                                   # a consumer looks at the maps every other hop
+
+        for _ in range(4):
+            e2e_step()
+        ectx.sync()
+        env.barrier()
+        n = max(e2e_steps, 64)
+        t0 = time.perf_counter()
+        for _ in range(n):
+            e2e_step()
+        ectx.sync()
+        env.barrier()
+        dt = env.max_over_ranks(time.perf_counter() - t0)
+        res["e2e"] = {"value": env.world * samples * n / dt, "unit": UNIT, "h2d_bytes_per_step": int(batch * H * W * b),
+                      "d2h_bytes_per_step": int(K * H * W * 4), "ms_per_step": 1e3 * dt / n, "h2d_GBps": batch * H * W * b * n / dt / 1e9,
+                      "maps_per_s": env.world * K * n / dt, "input_frames_per_s": env.world * hop * n / dt, "steps": n,
+                      "note": "pinned host batch -> qld_push_frames (copy stream) -> qld_demod(QLD_SLIDE) -> qld_read_map(amp) -> host; copies overlap the update"}
+        ectx.destroy()
+    return res
+
+
+RUNNERS = {"cfg0": bench_whole, "cfg1": bench_whole, "cfg2": bench_whole, "cfg3": bench_slide, "cfg4": bench_whole}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=sorted(RUNNERS))
+    ap.add_argument("--accum", default="auto", choices=sorted(ACCUM_NAMES))
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--ref-rows", type=int, default=0, help="rows of the frame the CPU oracle is timed / checked on "
+                    "(0: sized for about 15 s of oracle work on the host cores; 32 for --impl reference)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly and report under "
+                    "\"also\" (default: cfg4,cfg3,cfg1 when --workload is cfg2 on one GPU; 'none' to skip)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    if args.impl == "reference":
+        run_reference(args, int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")))
+        return
+
+    env = Env(args)
+    main_res = RUNNERS[args.workload](env, args, args.workload, args.accum, args.steps, args.warmup, args.e2e_steps,
+                                      not args.no_cpu_baseline)
+    also = {}
+    names = args.also
+    if names == "default":
+        names = "cfg4,cfg3,cfg1" if (args.workload == "cfg2" and env.world == 1 and args.accum == "auto") else "none"
+    if names != "none":
+        for w in [x for x in names.split(",") if x and x != args.workload]:
+            r = RUNNERS[w](env, args, w, "auto", min(args.steps, 50), 3, 0, not args.no_cpu_baseline)
+            also[w] = {k: r[k] for k in ("value", "ms_per_step", "maps_per_s", "kernel", "gpu_launches", "dtype", "roofline", "parity", "cpu_baseline", "clocks") if k in r}
+            also[w]["unit"] = UNIT
+            also[w]["config"] = {k: r["config"][k] for k in ("accum", "step", "cache", "N", "K") if k in r["config"]}
+
+    if env.rank == 0:
+        r = main_res
+        line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": env.world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": r["dtype"], "data": "synthetic", "config": r["config"], "maps_per_s": r["maps_per_s"],
+                "roofline": r["roofline"], "cpu_baseline": r.get("cpu_baseline"), "e2e": r.get("e2e"),
+                "gpu_launches": r["gpu_launches"], "clocks": r["clocks"], "parity": r.get("parity")}
+        if "window_samples_per_s" in r:
+            line["window_samples_per_s"] = r["window_samples_per_s"]
+        if also:
+            line["also"] = also
+        print(json.dumps(line), flush=True)
+    if env.dist is not None:
+        env.dist.destroy_process_group()
 
 
 if __name__ == "__main__":

@@ -99,6 +99,9 @@ typedef struct {
     uint32_t max_value;      /* largest sample value the caller guarantees (0 = type maximum); used only for
                                 the INT_BINS overflow bound */
     int32_t resync_hops;     /* SLIDE, FP32: recompute the window from the ring every this many hops (0 = never) */
+    int32_t external_store;  /* 1: the frame store (N frames, or ring_frames frames) is the caller's device buffer, given
+                                with qld_attach_frames_device; frames arrive in place and are announced with
+                                qld_commit_frames (zero-copy ingest).  ring_frames = -1 implies it. */
     void *workspace;         /* device memory of qld_workspace_bytes() bytes, 256-byte aligned, owned by the
                                 caller (e.g. a torch tensor) and kept alive until qld_destroy; NULL: the
                                 library allocates and frees it */
@@ -126,9 +129,22 @@ int qld_push_frames(qld_ctx *ctx, const void *host_frames, int n_frames);
 /* Same, for frames that are already in device memory (device -> device copy on the copy stream). */
 int qld_push_frames_device(qld_ctx *ctx, const void *device_frames, int n_frames);
 
-/* Whole-window store only: use the caller's device buffer of N frames in place (no copy).  The buffer
- * must stay valid and unchanged while demods that use it are in flight.  Counts as N frames pushed. */
+/* Use the caller's device buffer in place (no copy).  The buffer must stay valid, and frames a pending demod
+ * reads unchanged, while demods are in flight.
+ * Whole-window store (ring_frames 0 / -1; with 0 the library's own store is simply left unused): a buffer
+ * of N frames; counts as N frames pushed.
+ * Ring (ring_frames > 0, external_store = 1): a buffer of ring_frames frames; counts as no frames: announce
+ * them with qld_commit_frames as they arrive. */
 int qld_attach_frames_device(qld_ctx *ctx, const void *device_frames);
+
+/* Zero-copy ingest (A2 for producers that write device memory themselves: a capture card doing peer-to-peer
+ * DMA, a decode kernel, the synthetic filler).  external_store contexts only.  The caller has written -- or
+ * has enqueued on `producer_stream` (cudaStream_t, NULL = already complete) the work that writes -- the next
+ * n_frames frames, absolute indices pushed+1 .. pushed+n, in place: frame s lives at
+ * store + ((s-1) mod capacity) * H*W*bytes_per_sample, capacity = ring_frames (ring) or N (whole store).
+ * The call orders later demods after that work and extends the reference tables; it copies nothing.
+ * Errors as qld_push_frames (QLD_E_OVERRUN: those slots still belong to a window that was not produced yet). */
+int qld_commit_frames(qld_ctx *ctx, int n_frames, void *producer_stream);
 
 /* Have all pushes issued so far completed (host buffers reusable)?  block = 0: returns QLD_OK when done,
  * QLD_E_STATE when still in flight.  block = 1: waits, then QLD_OK. */
@@ -185,6 +201,12 @@ const char *qld_last_error(const qld_ctx *ctx);
 
 /* Launch statistics for benchmarks: kernels launched by this context so far. */
 int64_t qld_kernel_launches(const qld_ctx *ctx);
+
+/* Introspection for benchmarks and tests: the accumulation mode in use (a qld_accum other than AUTO; negative
+ * status if ctx is NULL), and the name of the kernel the last qld_demod launched ("" before the first):
+ * "k_demod_stream", "k_demod_whole", "k_demod_split", "k_demod_tc" or "k_demod_slide".  Never NULL. */
+int qld_accum_mode(const qld_ctx *ctx);
+const char *qld_last_kernel(const qld_ctx *ctx);
 
 /* ---- synthetic input filler (not part of the method; device twin of paper_1511_03390_b200/synth.py) ---- */
 typedef struct {

@@ -77,6 +77,7 @@ struct qld_ctx {
     int64_t win_start;       // 0-based offset a of the current window: frames a+1 .. a+N
     int64_t hops_since_seed;
     int64_t launches;
+    const char *last_kernel;
     bool sticky;
     std::string err;
 };
@@ -150,13 +151,14 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     if (cfg->ring_frames < -1 || (cfg->ring_frames > 0 && cfg->ring_frames <= cfg->N))
         return bad(QLD_E_INVAL, "ring_frames must be -1, 0, or > N");
     if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_FIXED) return bad(QLD_E_INVAL, "unknown accum");
+    if (cfg->external_store != 0 && cfg->external_store != 1) return bad(QLD_E_INVAL, "external_store must be 0 or 1");
     if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
     if (cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64)) return bad(QLD_E_INVAL, "unknown bits in maps");
     memset(pl, 0, sizeof *pl);
     pl->H = cfg->H; pl->W = cfg->W; pl->dtype = cfg->dtype; pl->bytes = cfg->dtype == QLD_U8 ? 1 : 2;
     pl->N = cfg->N; pl->K = cfg->K; pl->norm = cfg->norm; pl->maps = (cfg->maps & QLD_MAP_ALL) ? cfg->maps : (cfg->maps | QLD_MAP_ALL);
     pl->HW = (int64_t)cfg->H * cfg->W;
-    pl->ring = cfg->ring_frames > 0; pl->external = cfg->ring_frames == -1;
+    pl->ring = cfg->ring_frames > 0; pl->external = cfg->ring_frames == -1 || cfg->external_store == 1;
     pl->cap = pl->ring ? cfg->ring_frames : cfg->N;
     pl->cap_w = pl->cap + 1;
 
@@ -317,20 +319,16 @@ int wait_for_readers(qld_ctx *c, int64_t last_overwritten)
     return QLD_OK;
 }
 
+// src == NULL: the frames were written in place by the caller (qld_commit_frames); nothing is copied
 int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
 {
-    if (!c) return QLD_E_INVAL;
-    if (c->sticky) return QLD_E_CUDA;
-    if (!src || n < 1) return fail(c, QLD_E_INVAL, "push: null buffer or n_frames < 1");
-    if (c->external) return fail(c, QLD_E_STATE, "push: this context takes attached frames only (ring_frames = -1)");
-    if (n > c->cap) return fail(c, QLD_E_INVAL, "push: more frames than the store holds");
     const size_t fb = (size_t)c->HW * c->bytes;
     if (!c->ring) {
         if (c->pushed + n > c->N) return fail(c, QLD_E_OVERRUN, "push: whole-window store already holds N frames (qld_reset first)");
         // frames still being read by an earlier demod of the previous stack
         int rc = wait_for_readers(c, INT64_MAX);
         if (rc) return rc;
-        CU(c, cudaMemcpyAsync(c->frames + (size_t)c->pushed * fb, src, (size_t)n * fb, kind, c->s_copy));
+        if (src) CU(c, cudaMemcpyAsync(c->frames + (size_t)c->pushed * fb, src, (size_t)n * fb, kind, c->s_copy));
     } else {
         const int64_t first = c->pushed + 1, last = c->pushed + n;
         const int64_t oldest_needed = c->seeded ? c->win_start + 1 : 1;
@@ -341,8 +339,10 @@ int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
         }
         const int slot = (int)((first - 1) % c->cap);
         const int n1 = n < c->cap - slot ? n : c->cap - slot;
-        CU(c, cudaMemcpyAsync(c->frames + (size_t)slot * fb, src, (size_t)n1 * fb, kind, c->s_copy));
-        if (n1 < n) CU(c, cudaMemcpyAsync(c->frames, static_cast<const unsigned char *>(src) + (size_t)n1 * fb, (size_t)(n - n1) * fb, kind, c->s_copy));
+        if (src) {
+            CU(c, cudaMemcpyAsync(c->frames + (size_t)slot * fb, src, (size_t)n1 * fb, kind, c->s_copy));
+            if (n1 < n) CU(c, cudaMemcpyAsync(c->frames, static_cast<const unsigned char *>(src) + (size_t)n1 * fb, (size_t)(n - n1) * fb, kind, c->s_copy));
+        }
         int rc = fill_tables(c, first, n, c->s_copy);
         if (rc) return rc;
     }
@@ -386,6 +386,7 @@ int run_whole_tc(qld_ctx *c)
     p.fin = fin_with_maps(c);
     CU(c, qld_launch_demod_tc(c->tmap, p, c->n_sms, c->s_comp));
     c->launches++;
+    c->last_kernel = "k_demod_tc";
     return record_demod(c, 1);
 }
 
@@ -411,8 +412,10 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
             c->stream_shape = sh;
         }
         CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+        c->last_kernel = "k_demod_stream";
     } else {
         CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+        c->last_kernel = "k_demod_whole";
     }
     c->launches++;
     return record_demod(c, a + 1);
@@ -434,6 +437,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
     p.fin = fin_with_maps(c);
     CU(c, qld_launch_demod_slide(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
     c->launches++;
+    c->last_kernel = "k_demod_slide";
     return record_demod(c, a_old + 1);
 }
 
@@ -527,20 +531,46 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     return QLD_OK;
 }
 
-int qld_push_frames(qld_ctx *c, const void *host_frames, int n_frames) { return push_common(c, host_frames, n_frames, cudaMemcpyHostToDevice); }
+static int push_checked(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (!src || n < 1) return fail(c, QLD_E_INVAL, "push: null buffer or n_frames < 1");
+    if (c->external) return fail(c, QLD_E_STATE, "push: this context takes frames in place (external_store): attach + qld_commit_frames");
+    if (n > c->cap) return fail(c, QLD_E_INVAL, "push: more frames than the store holds");
+    return push_common(c, src, n, kind);
+}
 
-int qld_push_frames_device(qld_ctx *c, const void *device_frames, int n_frames) { return push_common(c, device_frames, n_frames, cudaMemcpyDeviceToDevice); }
+int qld_push_frames(qld_ctx *c, const void *host_frames, int n_frames) { return push_checked(c, host_frames, n_frames, cudaMemcpyHostToDevice); }
+
+int qld_push_frames_device(qld_ctx *c, const void *device_frames, int n_frames) { return push_checked(c, device_frames, n_frames, cudaMemcpyDeviceToDevice); }
+
+int qld_commit_frames(qld_ctx *c, int n_frames, void *producer_stream)
+{
+    if (!c) return QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (!c->external) return fail(c, QLD_E_STATE, "commit: context owns its frame store (use qld_push_frames)");
+    if (!c->frames) return fail(c, QLD_E_STATE, "commit: no frame store attached");
+    if (n_frames < 1 || n_frames > c->cap) return fail(c, QLD_E_INVAL, "commit: n_frames must be 1..capacity");
+    if (producer_stream) {
+        // tables and later demods are ordered after the producer's writes
+        CU(c, cudaEventRecord(c->tables_ev, static_cast<cudaStream_t>(producer_stream)));
+        CU(c, cudaStreamWaitEvent(c->s_copy, c->tables_ev, 0));
+    }
+    return push_common(c, nullptr, n_frames, cudaMemcpyDefault);
+}
 
 int qld_attach_frames_device(qld_ctx *c, const void *device_frames)
 {
     if (!c) return QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
     if (!device_frames) return fail(c, QLD_E_INVAL, "attach: null buffer");
-    if (c->ring) return fail(c, QLD_E_STATE, "attach: ring contexts copy their frames (use qld_push_frames_device)");
+    if (c->ring && !c->external) return fail(c, QLD_E_STATE, "attach: this ring context owns its frame store (create it with external_store = 1)");
+    if (c->pushed > 0 && c->ring) return fail(c, QLD_E_STATE, "attach: ring already holds frames (qld_reset first)");
     if (c->is_fixed && (reinterpret_cast<uintptr_t>(device_frames) & 15)) return fail(c, QLD_E_INVAL, "attach: FIXED accumulation needs a 16-byte aligned buffer");
     c->frames = const_cast<unsigned char *>(static_cast<const unsigned char *>(device_frames));
     c->tmap_valid = false;
-    c->pushed = c->N;
+    if (!c->ring) c->pushed = c->N;
     return QLD_OK;
 }
 
@@ -706,7 +736,7 @@ int qld_reset(qld_ctx *c)
     if (rc) return rc;
     c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
-    if (c->external) { c->frames = nullptr; c->tmap_valid = false; }
+    if (c->external && !c->ring) { c->frames = nullptr; c->tmap_valid = false; }   // an attached ring stays attached
     if (c->ring) {
         rc = init_device_state(c);
         if (rc) return rc;
@@ -732,5 +762,9 @@ void qld_destroy(qld_ctx *c)
 const char *qld_last_error(const qld_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 int64_t qld_kernel_launches(const qld_ctx *c) { return c ? c->launches : 0; }
+
+int qld_accum_mode(const qld_ctx *c) { return c ? c->accum : QLD_E_INVAL; }
+
+const char *qld_last_kernel(const qld_ctx *c) { return (c && c->last_kernel) ? c->last_kernel : ""; }
 
 }  // extern "C"

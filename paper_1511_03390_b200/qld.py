@@ -25,8 +25,8 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 
 # every symbol include/qld.h declares (tests check that the library exports each of them)
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
-           "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
-           "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches",
+           "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
+           "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel",
            "qld_synth_fill"]
 
 
@@ -38,7 +38,7 @@ class qld_ref(C.Structure):
 class qld_config(C.Structure):
     _fields_ = [("H", C.c_int32), ("W", C.c_int32), ("dtype", C.c_int32), ("N", C.c_int32), ("K", C.c_int32),
                 ("refs", C.POINTER(qld_ref)), ("ring_frames", C.c_int32), ("accum", C.c_int32), ("norm", C.c_int32),
-                ("maps", C.c_int32), ("max_value", C.c_uint32), ("resync_hops", C.c_int32),
+                ("maps", C.c_int32), ("max_value", C.c_uint32), ("resync_hops", C.c_int32), ("external_store", C.c_int32),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("compute_stream", C.c_void_p), ("copy_stream", C.c_void_p)]
 
@@ -76,6 +76,7 @@ def load_library():
     l.qld_push_frames.argtypes = [vp, vp, i]
     l.qld_push_frames_device.argtypes = [vp, vp, i]
     l.qld_attach_frames_device.argtypes = [vp, vp]
+    l.qld_commit_frames.argtypes = [vp, i, vp]
     l.qld_push_done.argtypes = [vp, i]
     l.qld_demod.argtypes = [vp, i, i]
     l.qld_get_maps.argtypes = [vp, i, pf, pf, pf, pf]
@@ -94,6 +95,9 @@ def load_library():
     l.qld_last_error.restype = C.c_char_p
     l.qld_kernel_launches.argtypes = [vp]
     l.qld_kernel_launches.restype = i64
+    l.qld_accum_mode.argtypes = [vp]
+    l.qld_last_kernel.argtypes = [vp]
+    l.qld_last_kernel.restype = C.c_char_p
     l.qld_synth_fill.argtypes = [C.POINTER(qld_synth_scene), i64, i, vp, vp]
     _lib = l
     return l
@@ -115,7 +119,8 @@ class QLD:
 
     def __init__(self, H: int, W: int, dtype, N: int, refs: Sequence[dict], ring_frames: int = 0,
                  accum: int = QLD_ACC_AUTO, norm: int = QLD_NORM_PAPER, maps: int = QLD_MAP_ALL, max_value: int = 0,
-                 resync_hops: int = 0, device=None, copy_stream=None, torch_workspace: bool = True):
+                 resync_hops: int = 0, device=None, copy_stream=None, torch_workspace: bool = True,
+                 external_store: bool = False):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -126,7 +131,7 @@ class QLD:
         cfg.H, cfg.W, cfg.dtype, cfg.N, cfg.K = self.H, self.W, self.dtype, self.N, self.K
         cfg.refs = C.cast(self._refs, C.POINTER(qld_ref))
         cfg.ring_frames, cfg.accum, cfg.norm, cfg.maps = int(ring_frames), int(accum), int(norm), int(maps)
-        cfg.max_value, cfg.resync_hops = int(max_value), int(resync_hops)
+        cfg.max_value, cfg.resync_hops, cfg.external_store = int(max_value), int(resync_hops), int(bool(external_store))
         self._ctx = C.c_void_p()
         nbytes = C.c_size_t()
         rc = self.lib.qld_workspace_bytes(C.byref(cfg), C.byref(nbytes))
@@ -197,6 +202,11 @@ class QLD:
         self._check(self.lib.qld_attach_frames_device(self._ctx, frames.data_ptr()))
         self._attached = frames
 
+    def commit_frames(self, n_frames: int, producer_stream=None) -> None:
+        """qld_commit_frames: n more frames were written in place into the attached store (zero-copy ingest)."""
+        h = 0 if producer_stream is None else (producer_stream.cuda_stream or 1)
+        self._check(self.lib.qld_commit_frames(self._ctx, int(n_frames), h))
+
     def push_done(self, block: bool = False) -> bool:
         rc = self.lib.qld_push_done(self._ctx, int(block))
         if rc == QLD_E_STATE:
@@ -259,6 +269,15 @@ class QLD:
 
     def kernel_launches(self) -> int:
         return int(self.lib.qld_kernel_launches(self._ctx))
+
+    def accum_mode(self) -> int:
+        return int(self.lib.qld_accum_mode(self._ctx))
+
+    def accum_name(self) -> str:
+        return {QLD_ACC_FP32: "FP32", QLD_ACC_INT_BINS: "INT_BINS", QLD_ACC_FIXED: "FIXED"}[self.accum_mode()]
+
+    def last_kernel(self) -> str:
+        return self.lib.qld_last_kernel(self._ctx).decode()
 
     def destroy(self) -> None:
         if getattr(self, "_ctx", None) is not None and self._ctx.value:

@@ -386,3 +386,58 @@ def test_stream_kernel_ring_wraparound(Q, oracle, monkeypatch, tile):
         win = x[pushed - N:pushed]
         check_float_maps(_maps(ctx), oracle_maps(oracle, win, ref, s_first=pushed - N + 1), what=f"ring whole at {pushed}")
     ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ A2 zero-copy ingest
+@pytest.mark.parametrize("accum_name", ["INT_BINS", "FP32"])
+def test_commit_frames_into_attached_ring(Q, oracle, accum_name):
+    """external_store ring: the producer writes frames in place on its own stream, qld_commit_frames announces
+    them; windows (with ring wrap-around) equal the oracle's direct recomputation; overrun and state errors."""
+    import torch
+    rng = np.random.default_rng(5)
+    H, W, N, hop, cap, T = 8, 32, 48, 8, 64, 200
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    dev_stream = torch.from_numpy(stream.view(np.int16)).cuda()
+    ring = torch.zeros((cap, H, W), dtype=torch.int16, device="cuda")
+    ref = {"num": 1, "den": 6}
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095,
+                external_store=True)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.commit_frames(4)                                   # nothing attached yet
+    assert e.value.status == Q.QLD_E_STATE
+    with pytest.raises(Q.QLDError) as e:
+        ctx.push_frames(stream[:4])                            # copies are refused on an external store
+    assert e.value.status == Q.QLD_E_STATE
+    ctx.attach_frames_device(ring)
+    producer = torch.cuda.Stream()
+
+    def produce(first, n):                                     # frames first+1 .. first+n written in place
+        with torch.cuda.stream(producer):
+            for s in range(first, first + n):
+                ring[s % cap].copy_(dev_stream[s], non_blocking=True)
+        ctx.commit_frames(n, producer)
+
+    produce(0, N)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.commit_frames(cap - N + 1)                         # would overwrite frame 1 before window 0 exists
+    assert e.value.status == Q.QLD_E_OVERRUN
+    ctx.demod(Q.QLD_SLIDE, hop)
+    pushed, w = N, 0
+    while True:
+        ctx.sync()
+        a = w * hop
+        check_float_maps(_maps(ctx), oracle_maps(oracle, stream[a:a + N], ref, s_first=a + 1),
+                         rel=1e-6 if accum_name == "INT_BINS" else 1e-5, what=f"window {w}")
+        if pushed + hop > T:
+            break
+        produce(pushed, hop)
+        pushed += hop
+        ctx.demod(Q.QLD_SLIDE, hop)
+        w += 1
+    assert w == (T - N) // hop and ctx.counters() == (pushed, w + 1)
+    ctx.reset()                                                # the ring stays attached
+    produce(0, N)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    check_float_maps(_maps(ctx), oracle_maps(oracle, stream[:N], ref), what="after reset")
+    ctx.destroy()
