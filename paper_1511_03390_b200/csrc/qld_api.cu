@@ -372,6 +372,30 @@ int record_demod(qld_ctx *c, int64_t oldest_read)
     return QLD_OK;
 }
 
+// frames first+1 .. first+n (0-based offset `first`) as runs of consecutive store slots; returns the new run count
+int add_runs(const qld_ctx *c, DemodRun *runs, int at, int64_t first, int n, int sign)
+{
+    const int slot = (int)(first % c->cap);
+    const int n0 = n < c->cap - slot ? n : c->cap - slot;
+    runs[at].slot0 = slot; runs[at].n = n0; runs[at].w0 = (int)((first + 1) % c->cap_w); runs[at].sign = sign;
+    ++at;
+    if (n0 < n) {
+        runs[at].slot0 = 0; runs[at].n = n - n0; runs[at].w0 = (int)((first + 1 + n0) % c->cap_w); runs[at].sign = sign;
+        ++at;
+    }
+    return at;
+}
+
+int stream_tmap_for(qld_ctx *c, const StreamShape &sh)
+{
+    if (c->stream_tmap_frames != c->frames || sh.seg != c->stream_shape.seg || sh.kc != c->stream_shape.kc) {
+        CU(c, qld_stream_encode_tmap(c->stream_tmap, c->frames, c->HW * c->bytes, c->cap, sh));
+        c->stream_tmap_frames = c->frames;
+        c->stream_shape = sh;
+    }
+    return QLD_OK;
+}
+
 // whole-window kernel over absolute frames a+1 .. a+N; seeds the sliding accumulators when asked
 int run_whole_tc(qld_ctx *c)
 {
@@ -403,14 +427,12 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.acc_out = (seed || c->is_int) ? c->acc : nullptr;
     p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
     p.fin = fin_with_maps(c);
+    p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
     if (sh.seg > 0) {
-        if (c->stream_tmap_frames != c->frames || sh.seg != c->stream_shape.seg || sh.kc != c->stream_shape.kc) {
-            CU(c, qld_stream_encode_tmap(c->stream_tmap, c->frames, c->HW * c->bytes, c->cap, sh));
-            c->stream_tmap_frames = c->frames;
-            c->stream_shape = sh;
-        }
+        int rc = stream_tmap_for(c, sh);
+        if (rc) return rc;
         CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
         c->last_kernel = "k_demod_stream";
     } else {
@@ -424,6 +446,28 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
 int run_slide(qld_ctx *c, int64_t a_old, int hop)
 {
     const int64_t a_new = a_old + hop;
+    // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    if (sh.seg > 0 && hop >= sh.kc) {
+        DemodParams p;
+        memset(&p, 0, sizeof p);
+        p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+        p.cap = c->cap; p.cap_w = c->cap_w;
+        p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
+        p.wtab = c->wtab; p.cum = c->cum;
+        p.acc_out = c->acc; p.acc_add = 1;
+        p.ped_in = c->is_int ? nullptr : c->ped;
+        p.fin = fin_with_maps(c);
+        int n = add_runs(c, p.run, 0, a_old, hop, -1);            // expired: frames a_old+1 .. a_old+hop
+        n = add_runs(c, p.run, n, a_old + c->N, hop, +1);        // new: frames a_old+N+1 .. a_old+N+hop
+        p.n_runs = n;
+        int rc = stream_tmap_for(c, sh);
+        if (rc) return rc;
+        CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+        c->launches++;
+        c->last_kernel = "k_demod_stream";
+        return record_demod(c, a_old + 1);
+    }
     SlideParams p;
     memset(&p, 0, sizeof p);
     p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;

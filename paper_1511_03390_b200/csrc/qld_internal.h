@@ -31,6 +31,16 @@ struct FinParams {
     float *I, *Q, *amp, *phase;   // [K][HW] or null
 };
 
+// A run of consecutive store slots (no wrap inside a run) whose frames enter the sums with weight sign * w:
+// a whole window is one or two runs with sign +1 (a ring wraps once); a sliding update (A5) is the expired
+// frames with sign -1 followed by the new frames with sign +1.  k_demod_stream walks runs; k_demod_whole uses
+// slot0 / n / w0.
+struct DemodRun {
+    int32_t slot0, n;        // first slot, number of frames
+    int32_t w0;              // weight entry of the first frame (entries wrap at cap_w)
+    int32_t sign;            // +1 or -1
+};
+
 // One demodulation launch (whole window, ring aware).
 struct DemodParams {
     const void *frames;      // frame store base
@@ -46,6 +56,11 @@ struct DemodParams {
     const double *cum;       // [cap_w][ROWS] running sums of the float weights (FP32 only)
     void *acc_out;           // optional [ROWS][HW]: double (FP32: pedestal-subtracted sums) or int32 (bins)
     float *ped_out;          // optional [HW] pedestal used (FP32)
+    // k_demod_stream only
+    int32_t n_runs;
+    int32_t acc_add;         // 1: acc_out holds the previous window's sums; this launch's sums are added to them
+    DemodRun run[4];
+    const float *ped_in;     // FP32: pedestal to subtract (the one acc_out was seeded with); NULL: the first sample
     FinParams fin;
 };
 

@@ -11,7 +11,12 @@
 // One persistent CTA per SM: warp 0 = producer (TMA + the stage's weight rows), warps 1..8 = consumers.  A tile is
 // SEG bytes of every frame of the window; tiles are claimed from a global counter.  Inside a tile, consumer warp w
 // owns column group (w % CG) -- 32 lanes x V pixels -- and time slice (w / CG): it takes every TS-th frame of each
-// stage.  Slices are combined through shared memory at the end of the tile (fp64 / int32), then the A4 epilogue.
+// stage.  Slices are combined through shared memory at the end of the tile (fp64 / int32), then the A4 epilogue
+// runs with consecutive threads on consecutive pixels (coalesced accumulator and map traffic).
+//
+// The frames of a launch are a list of runs (DemodRun): a whole window is one or two runs of weight +w, and the
+// sliding update of PAPER.md:181-183 (A5) is the same kernel over {expired frames, -w} + {new frames, +w} with the
+// sums added to the accumulators the previous window left in global memory.
 #include <stdio.h>
 #include <stdlib.h>
 
@@ -51,7 +56,14 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
 
     const int SEG = sh.seg, KC = sh.kc, STAGES = sh.stages;
     const int CG = SEG / (32 * VB), TS = NW / CG;          // column groups, time slices
-    const StreamSmem SM(SEG, KC, STAGES, ROWS, TS > 1 ? ROWS * V * CG * 32 * (int)sizeof(RED) : 0);
+    // combine buffer: [ROWS (+1: pedestal)][V][RS] RED cells, RS = column count padded so that the epilogue's
+    // pixel-order reads (v fastest) fall into distinct banks
+    constexpr int PAD = 128 / ((int)sizeof(RED) * V) > 0 ? 128 / ((int)sizeof(RED) * V) : 1;
+    constexpr int RROWS = ROWS + (IS_INT ? 0 : 1);
+    // pixels per thread whose stored sums are prefetched in a sliding update (registers: PFN * ROWS RED values)
+    constexpr int PFN = IS_INT ? (ROWS <= 4 ? 4 : (ROWS <= 8 ? 2 : 0)) : (ROWS <= 2 ? 4 : (ROWS <= 4 ? 2 : 0));
+    const int RS = CG * 32 + PAD;
+    const StreamSmem SM(SEG, KC, STAGES, ROWS, TS > 1 ? RROWS * V * RS * (int)sizeof(RED) : 0);
 
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
@@ -65,8 +77,6 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
     const int n_tiles = (int)((row_bytes + SEG - 1) / SEG);
-    // the window is at most two runs of consecutive slots of the frame store (a ring wraps once)
-    const int run0 = min(p.n, p.cap - p.slot0), run1 = p.n - run0;
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < STAGES; ++i) {
@@ -98,9 +108,9 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
                 }
                 break;
             }
-            int fi = 0;                                    // frame index inside the window of the chunk's first frame
-            for (int run = 0; run < 2; ++run) {
-                const int rn = run ? run1 : run0, rslot = run ? 0 : p.slot0;
+            for (int run = 0; run < p.n_runs; ++run) {
+                const int rn = p.run[run].n, rslot = p.run[run].slot0, rw0 = p.run[run].w0;
+                const ACC sgn = (ACC)p.run[run].sign;
                 for (int c0 = 0; c0 < rn; c0 += KC) {
                     const int nf = min(KC, rn - c0);
                     mbar_wait(&empty[stage], phase ^ 1);
@@ -112,13 +122,12 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
                     }
                     ACC *wdst = sW + (size_t)stage * KC * ROWS;
                     for (int i = lane; i < nf * ROWS; i += 32) {
-                        int e = p.w0 + fi + i / ROWS;
+                        int e = rw0 + c0 + i / ROWS;           // rw0 < cap_w and c0 + i / ROWS < cap_w
                         if (e >= p.cap_w) e -= p.cap_w;
-                        wdst[i] = __ldg(wtab + (int64_t)e * ROWS + (i % ROWS));
+                        wdst[i] = sgn * __ldg(wtab + (int64_t)e * ROWS + (i % ROWS));
                     }
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&full[stage]);
-                    fi += nf;
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -130,6 +139,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
     const int cw = warp - 1, cg = cw % CG, ts = cw / CG;
     const int col = (cg * 32 + lane) * VB;                 // byte offset of this thread's pixels inside the segment
     const int tcol = cg * 32 + lane;                       // thread column inside the tile
+    const int TP = SEG / (int)sizeof(T);                   // pixels per tile
     int stage = 0;
     uint32_t phase = 0;
     for (int it = 0;; ++it) {
@@ -147,10 +157,36 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
         float pedm[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) pedm[v] = 8388608.0f;
+        bool need_ped = !IS_INT;
+        if constexpr (!IS_INT) {
+            if (p.ped_in != nullptr) {                     // A5: the pedestal the accumulators were seeded with
+                need_ped = false;
+                if (active) {
+#pragma unroll
+                    for (int v = 0; v < V; ++v) pedm[v] = 8388608.0f + __ldg(p.ped_in + pix0 + v);
+                }
+            }
+        }
+
+        // A5: the previous window's sums of the pixels this thread finalises, requested now so that the loads
+        // complete under the frame loop
+        const int64_t tile_pix0 = (int64_t)tile * TP;
+        RED pf[PFN > 0 ? PFN : 1][ROWS];
+        const bool use_pf = PFN > 0 && p.acc_add && TS > 1 && TP <= PFN * NW * 32;
+        if (use_pf) {
+            const RED *accg = static_cast<const RED *>(p.acc_out);
+#pragma unroll
+            for (int i = 0; i < (PFN > 0 ? PFN : 1); ++i) {
+                const int q = cw * 32 + lane + i * NW * 32;
+                const bool ok = q < TP && tile_pix0 + q < p.HW;
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) pf[i][r] = ok ? accg[(int64_t)r * p.HW + tile_pix0 + q] : (RED)0;
+            }
+        }
 
         bool first = true;
-        for (int run = 0; run < 2; ++run) {
-            const int rn = run ? run1 : run0;
+        for (int run = 0; run < p.n_runs; ++run) {
+            const int rn = p.run[run].n;
             for (int c0 = 0; c0 < rn; c0 += KC) {
                 const int nf = min(KC, rn - c0);
                 if (!first) mbar_wait(&full[stage], phase);
@@ -158,7 +194,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
                 const ACC *wrow = sW + (size_t)stage * KC * ROWS;
                 if (first) {
                     first = false;
-                    if constexpr (!IS_INT) {
+                    if (need_ped) {
                         // pedestal = the pixel's first sample in the window (exact integer), DESIGN.md "Precision"
                         uint32_t w0[PX::NW];
                         PX::load_shared(d, w0);
@@ -195,63 +231,105 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
             }
         }
 
-        // ---- combine the TS time slices (fp64 / int32), then A4 ----
         if (TS > 1) {
-            for (int yy = 0; yy < TS; ++yy) {
-                if (ts == yy) {
+            // ---- combine the TS time slices (fp64 / int32).  The ROWS*V values of a thread are cut into NW chunks;
+            // in turn j slice ts adds the chunks c with c = ts + j (mod TS), so every slice works in every turn and
+            // no two slices touch a cell in the same turn.  Turn 0 stores (first touch), later turns add.
+            constexpr int CH = ROWS * V / NW;
+            static_assert(CH >= 1 && CH * NW == ROWS * V, "chunking");
+            for (int j = 0; j < TS; ++j) {
+                const int want = (ts + j) & (TS - 1);
 #pragma unroll
-                    for (int r = 0; r < ROWS; ++r)
+                for (int c = 0; c < NW; ++c) {
+                    if ((c & (TS - 1)) != want) continue;
+                    RED t[CH];
 #pragma unroll
-                        for (int v = 0; v < V; ++v) {
-                            RED *cell = &red[(r * V + v) * (CG * 32) + tcol];
-                            if (yy == 0) *cell = (RED)acc[r][v];
-                            else *cell += (RED)acc[r][v];
-                        }
+                    for (int e = 0; e < CH; ++e) {
+                        const int i = c * CH + e;
+                        t[e] = (j == 0) ? (RED)0 : red[(size_t)i * RS + tcol];
+                    }
+#pragma unroll
+                    for (int e = 0; e < CH; ++e) {
+                        const int i = c * CH + e;
+                        red[(size_t)i * RS + tcol] = t[e] + (RED)acc[i / V][i % V];
+                    }
+                }
+                if constexpr (!IS_INT) {
+                    if (j == 0 && ts == 0) {
+#pragma unroll
+                        for (int v = 0; v < V; ++v) red[(size_t)(ROWS * V + v) * RS + tcol] = (RED)(pedm[v] - 8388608.0f);
+                    }
                 }
                 named_barrier(1, NW * 32);
             }
-        }
-        if (active) {
-            for (int v = ts; v < V; v += TS) {
-                const int64_t pixel = pix0 + v;
+            // ---- A4, consecutive threads on consecutive pixels ----
+            auto finalise_q = [&](int q, int64_t pixel, const RED *prev) {
+                const int v = q % V, tc = q / V;
                 double val[ROWS];
-                RED a[ROWS];
-                if (TS > 1) {
+                RED *accg = static_cast<RED *>(p.acc_out);
+                double ped = 0.0;
+                if constexpr (!IS_INT) ped = red[(size_t)(ROWS * V + v) * RS + tc];
 #pragma unroll
-                    for (int r = 0; r < ROWS; ++r) a[r] = red[(r * V + v) * (CG * 32) + tcol];
-                } else {
-#pragma unroll
-                    for (int r = 0; r < ROWS; ++r) {
-                        // v is a runtime index: select without forcing acc[][] into local memory
-                        RED t = 0;
-#pragma unroll
-                        for (int vv = 0; vv < V; ++vv) t = (vv == v) ? (RED)acc[r][vv] : t;
-                        a[r] = t;
+                for (int r = 0; r < ROWS; ++r) {
+                    RED a = red[(size_t)(r * V + v) * RS + tc];
+                    if (p.acc_add) a += prev ? prev[r] : accg[(int64_t)r * p.HW + pixel];
+                    if (accg) accg[(int64_t)r * p.HW + pixel] = a;
+                    if constexpr (IS_INT) {
+                        val[r] = (double)a;
+                    } else {
+                        const double wsum = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
+                        val[r] = a + ped * wsum;           // sum x w = sum (x - ped) w + ped * sum w
                     }
                 }
+                if constexpr (!IS_INT) {
+                    if (p.ped_out) p.ped_out[pixel] = (float)ped;
+                }
+                finalise_pixel<ROWS>(p.fin, val, pixel, p.HW);
+            };
+            if (use_pf) {
+#pragma unroll
+                for (int i = 0; i < (PFN > 0 ? PFN : 1); ++i) {
+                    const int q = cw * 32 + lane + i * NW * 32;
+                    if (q < TP && tile_pix0 + q < p.HW) finalise_q(q, tile_pix0 + q, pf[i]);
+                }
+            } else {
+                for (int q = cw * 32 + lane; q < TP; q += NW * 32) {
+                    if (tile_pix0 + q >= p.HW) break;
+                    finalise_q(q, tile_pix0 + q, nullptr);
+                }
+            }
+            named_barrier(1, NW * 32);                     // red is free for the next tile
+        } else if (active) {
+            // one slice per column group (narrow vectors): every thread finalises its own V pixels
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const int64_t pixel = pix0 + v;
+                double val[ROWS];
                 if constexpr (IS_INT) {
+                    int *accg = static_cast<int *>(p.acc_out);
 #pragma unroll
                     for (int r = 0; r < ROWS; ++r) {
-                        val[r] = (double)a[r];
-                        if (p.acc_out) static_cast<int *>(p.acc_out)[(int64_t)r * p.HW + pixel] = a[r];
+                        int a = acc[r][v];
+                        if (p.acc_add) a += accg[(int64_t)r * p.HW + pixel];
+                        if (accg) accg[(int64_t)r * p.HW + pixel] = a;
+                        val[r] = (double)a;
                     }
                 } else {
-                    float pm = 0.f;
-#pragma unroll
-                    for (int vv = 0; vv < V; ++vv) pm = (vv == v) ? pedm[vv] : pm;
-                    const double ped = (double)(pm - 8388608.0f);
+                    double *accg = static_cast<double *>(p.acc_out);
+                    const double ped = (double)(pedm[v] - 8388608.0f);
 #pragma unroll
                     for (int r = 0; r < ROWS; ++r) {
-                        if (p.acc_out) static_cast<double *>(p.acc_out)[(int64_t)r * p.HW + pixel] = a[r];
+                        double a = (double)acc[r][v];
+                        if (p.acc_add) a += accg[(int64_t)r * p.HW + pixel];
+                        if (accg) accg[(int64_t)r * p.HW + pixel] = a;
                         const double wsum = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
-                        val[r] = a[r] + ped * wsum;     // sum x w = sum (x - ped) w + ped * sum w
+                        val[r] = a + ped * wsum;
                     }
                     if (p.ped_out) p.ped_out[pixel] = (float)ped;
                 }
                 finalise_pixel<ROWS>(p.fin, val, pixel, p.HW);
             }
         }
-        if (TS > 1) named_barrier(1, NW * 32);              // red is free for the next tile
     }
 }
 
@@ -262,7 +340,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
 int red_bytes_for(int seg, int vb, int rows, int v, bool is_int)
 {
     const int cg = seg / (32 * vb), ts = NW / cg;
-    return ts > 1 ? rows * v * cg * 32 * (is_int ? 4 : 8) : 0;
+    const int esz = is_int ? 4 : 8;
+    const int pad = 128 / (esz * v) > 0 ? 128 / (esz * v) : 1;
+    return ts > 1 ? (rows + (is_int ? 0 : 1)) * v * (cg * 32 + pad) * esz : 0;
 }
 
 template <typename T, typename ACC, int ROWS>

@@ -388,6 +388,38 @@ def test_stream_kernel_ring_wraparound(Q, oracle, monkeypatch, tile):
     ctx.destroy()
 
 
+@pytest.mark.parametrize("tile", ["512,16", "2048,16", "1024,32"])
+@pytest.mark.parametrize("accum_name,ref", [("INT_BINS", {"num": 1, "den": 6}), ("FP32", {"num": 1, "den": 6}), ("FP32", {"nu": 0.0937, "phase": 0.3}),
+                                            ("INT_BINS", {"num": 1, "den": 4})])
+@pytest.mark.parametrize("hop,cap", [(32, 170), (40, 173), (64, 192)])
+def test_stream_kernel_sliding_update(Q, oracle, monkeypatch, tile, accum_name, ref, hop, cap):
+    """A5 through the TMA-fed kernel: runs {expired, -w} + {new, +w} added to the stored accumulators; hops that are
+    and are not multiples of a stage, expired and new runs that wrap around the ring; bins bit-exact at every hop."""
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(hop + cap)
+    H, W, N, T = 12, 128, 96, 96 + 9 * hop
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095)
+    ctx.push_frames(stream[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    for w in range(0, (T - N) // hop + 1):
+        if w > 0:
+            ctx.push_frames(stream[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+            assert ctx.last_kernel() == "k_demod_stream"
+        ctx.sync()
+        a = w * hop
+        ora = oracle_maps(oracle, stream[a:a + N], ref, s_first=a + 1)
+        if accum_name == "INT_BINS":
+            den = ref["den"]
+            B = oracle.bins(stream[a:a + N], 1, den, s_first=a + 1)
+            assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:den // 2] - B[den // 2:]), f"window {w}"
+            check_float_maps(_maps(ctx), ora, rel=1e-6, what=f"window {w}")
+        else:
+            check_float_maps(_maps(ctx), ora, what=f"window {w}")
+    ctx.destroy()
+
+
 # ------------------------------------------------------------------------------------------------ A2 zero-copy ingest
 @pytest.mark.parametrize("accum_name", ["INT_BINS", "FP32"])
 def test_commit_frames_into_attached_ring(Q, oracle, accum_name):
