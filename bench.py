@@ -80,8 +80,8 @@ class ClockSampler(threading.Thread):
 
 
 def build_workload(name: str, rank: int):
-    from paper_1511_03390_b200 import synth
-    return synth.BUILDERS[name](seed=int(name[3]) + 1000 * rank)      # BASELINE.json seeds: cfgN -> seed N
+    from paper_1511_03390_b200 import shard, synth
+    return synth.BUILDERS[name](seed=shard.stream_seed(int(name[3]), rank))   # BASELINE.json seeds: cfgN -> seed N on rank 0
 
 
 def oracle_on_rows(wl, frames_rows_host, refs, nthreads):
