@@ -110,21 +110,55 @@ __device__ __forceinline__ void load_weights_shared(const ACC *row, ACC (&wt)[RO
     }
 }
 
+// packed fp32 pairs (Blackwell FADD2 / FFMA2: two IEEE fp32 operations per issued instruction, same rounding
+// as the scalar forms)
+__device__ __forceinline__ uint64_t pack2(float lo, float hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t p, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p)); }
+__device__ __forceinline__ uint64_t sub2(uint64_t a, uint64_t b)
+{
+    uint64_t r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c)
+{
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
 // acc[r][v] += x_v * w_r for one frame.  Float: x is pedestal-subtracted exactly, (2^23+x) - (2^23+ped).
 template <typename T, typename ACC, int ROWS, int V>
 __device__ __forceinline__ void accumulate(const uint32_t (&w)[Pix<T, V>::NW], const ACC (&wt)[ROWS], const float (&pedm)[V],
                                            ACC (&acc)[ROWS][V])
 {
+    if constexpr (std::is_same<ACC, float>::value && V % 2 == 0) {
 #pragma unroll
-    for (int v = 0; v < V; ++v) {
-        if constexpr (std::is_same<ACC, float>::value) {
-            float x = Pix<T, V>::getf_biased(w, v) - pedm[v];
+        for (int v = 0; v < V; v += 2) {
+            const uint64_t x = sub2(pack2(Pix<T, V>::getf_biased(w, v), Pix<T, V>::getf_biased(w, v + 1)), pack2(pedm[v], pedm[v + 1]));
 #pragma unroll
-            for (int r = 0; r < ROWS; ++r) acc[r][v] = fmaf(x, wt[r], acc[r][v]);
-        } else {
-            int x = (int)Pix<T, V>::geti(w, v);
+            for (int r = 0; r < ROWS; ++r) {
+                const uint64_t a = fma2(x, pack2(wt[r], wt[r]), pack2(acc[r][v], acc[r][v + 1]));
+                unpack2(a, acc[r][v], acc[r][v + 1]);
+            }
+        }
+    } else {
 #pragma unroll
-            for (int r = 0; r < ROWS; ++r) acc[r][v] += x * wt[r];
+        for (int v = 0; v < V; ++v) {
+            if constexpr (std::is_same<ACC, float>::value) {
+                float x = Pix<T, V>::getf_biased(w, v) - pedm[v];
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) acc[r][v] = fmaf(x, wt[r], acc[r][v]);
+            } else {
+                int x = (int)Pix<T, V>::geti(w, v);
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) acc[r][v] += x * wt[r];
+            }
         }
     }
 }
