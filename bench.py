@@ -229,7 +229,10 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     # inputs: the synthetic stack, filled on the device, resident before the timed region
     frames = qld.synth_fill(sc, 1, N, device=env.dev)
     torch.cuda.synchronize()
-    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=-1, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval)
+    # BASELINE.json configs[4] asks for the K amplitude maps only; the other configs produce all four maps
+    maps, map_names = (qld.QLD_MAP_AMP, "amplitude") if workload == "cfg4" else (qld.QLD_MAP_ALL, "I,Q,amplitude,phase")
+    n_maps = 1 if workload == "cfg4" else 4
+    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=-1, accum=accum, maps=maps, max_value=sc.maxval)
     ctx.attach_frames_device(frames)
 
     def step():
@@ -242,13 +245,13 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
            "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel}
     res["gpu_launches"] = int(launches)
-    algo = samples * b + 4.0 * K * H * W * 4.0               # every sample once + four fp32 maps per reference
+    algo = samples * b + n_maps * K * H * W * 4.0            # every sample once + the fp32 maps of every reference
     in_l2 = samples * b <= 126e6
     res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
                                    "input fits the 126 MB L2 and is re-read every step: L2-resident, not an HBM number" if in_l2 else None)
     res["dtype"] = {"INT_BINS": "int32", "FIXED": "int8 x int8 -> int32 -> int64 (tcgen05)", "FP32": "f32"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype, "accum": mode,
-                     "maps": "I,Q,amplitude,phase", "step": "qld_demod(QLD_WHOLE) over the resident stack",
+                     "maps": map_names, "step": "qld_demod(QLD_WHOLE) over the resident stack",
                      "cache": f"input {samples * b / 1e6:.0f} MB per step " + ("<= 126 MB L2: L2-resident" if in_l2 else "> 126 MB L2: no flush needed"),
                      "parallelism": f"{env.world} x independent stacks (pixels are independent; no collective)"}
 
@@ -258,7 +261,7 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
         host.copy_(frames)
         amp_host = torch.empty((K, H, W), dtype=torch.float32).pin_memory()
         torch.cuda.synchronize()
-        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=0, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval)
+        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=0, accum=accum, maps=maps, max_value=sc.maxval)
         chunk = max(1, min(N, (256 << 20) // (H * W * b)))       # pushes of about 256 MiB
 
         def e2e_step():
@@ -300,9 +303,9 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
         ctx.demod(qld.QLD_WHOLE)
         ctx.sync()
         worst = 0.0
-        tol = 1e-6 if mode == "INT_BINS" else 1e-5
+        tol = 1e-5 if mode == "FP32" else 1e-6
         for k in range(K):
-            got = tuple(m[r0:r0 + rows].cpu().numpy() for m in ctx.get_maps(k))
+            got = tuple(None if m is None else m[r0:r0 + rows].cpu().numpy() for m in ctx.get_maps(k))
             worst = max(worst, check_float_maps(got, out[k], rel=tol, what=f"bench parity k={k}"))
         res["parity"] = {"rows_checked": rows, "refs_checked": K, "tolerance": f"{tol:g} relative, floored at the map median",
                          "strict_max_rel_err_amp": worst, "ok": True}

@@ -64,7 +64,9 @@ typedef enum {
  *             int8 contraction (A6).  Bit-exact against an integer oracle with the same
  *             table; |R*2^-30 - sin| <= 2^-31, so the maps also agree with the float definition to ~1e-9.
  *             Whole-window stores only (ring_frames 0 or -1), H*W*bytes a multiple of 16, N <= 65536.
- *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds, else FP32. */
+ *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds; else FIXED for
+ *             K >= 4 references on a whole-window store that meets FIXED's conditions (the CUDA-core kernel is
+ *             instruction-bound there, the contraction is HBM-bound and more accurate than fp32); else FP32. */
 typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2, QLD_ACC_FIXED = 3 } qld_accum;
 
 typedef enum { QLD_NORM_PAPER = 0 /* no scaling (G3) */, QLD_NORM_AMPLITUDE = 1 /* I, Q, R times 2/N */ } qld_norm;

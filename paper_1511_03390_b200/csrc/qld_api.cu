@@ -203,7 +203,11 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     int acc = cfg->accum;
     int rows = 0;
     if (acc == QLD_ACC_AUTO) {
-        acc = (all_rational && max_den <= 16 && bins_rows(&rows) && bins_fit()) ? QLD_ACC_INT_BINS : QLD_ACC_FP32;
+        // bins when the references allow them (exact, cheapest); for K >= 4 float references on a whole-window
+        // store the CUDA-core kernel is instruction-issue bound (16+ FMA per sample) and the
+        // exact int8 contraction on the tensor cores is used; otherwise pedestal-subtracted fp32
+        const bool tc_ok = !pl->ring && cfg->K >= 4 && (pl->HW * pl->bytes) % 16 == 0 && cfg->N <= 65536 && !(cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64));
+        acc = (all_rational && max_den <= 16 && bins_rows(&rows) && bins_fit()) ? QLD_ACC_INT_BINS : (tc_ok ? QLD_ACC_FIXED : QLD_ACC_FP32);
     }
     if (acc == QLD_ACC_INT_BINS) {
         if (!all_rational) return bad(QLD_E_UNSUPPORTED, "INT_BINS needs every reference rational (den > 0)");
@@ -428,8 +432,9 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
     p.fin = fin_with_maps(c);
     p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
+    p.onehot = c->is_int && c->K == 1;
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->N);
     if (sh.seg > 0) {
         int rc = stream_tmap_for(c, sh);
         if (rc) return rc;
@@ -447,7 +452,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
 {
     const int64_t a_new = a_old + hop;
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, 2 * hop);
     if (sh.seg > 0 && hop >= sh.kc) {
         DemodParams p;
         memset(&p, 0, sizeof p);
@@ -456,6 +461,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
         p.wtab = c->wtab; p.cum = c->cum;
         p.acc_out = c->acc; p.acc_add = 1;
+        p.onehot = c->is_int && c->K == 1;
         p.ped_in = c->is_int ? nullptr : c->ped;
         p.fin = fin_with_maps(c);
         int n = add_runs(c, p.run, 0, a_old, hop, -1);            // expired: frames a_old+1 .. a_old+hop

@@ -58,6 +58,7 @@ struct DemodParams {
     float *ped_out;          // optional [HW] pedestal used (FP32)
     // k_demod_stream only
     int32_t n_runs;
+    int32_t onehot;          // integer bins, one reference: every weight row is one-hot (+-1 in one row)
     int32_t acc_add;         // 1: acc_out holds the previous window's sums; this launch's sums are added to them
     DemodRun run[4];
     const float *ped_in;     // FP32: pedestal to subtract (the one acc_out was seeded with); NULL: the first sample

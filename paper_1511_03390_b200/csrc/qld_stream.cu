@@ -30,6 +30,11 @@ using namespace qld_ptx;
 namespace {
 
 constexpr int NW = 8;                 // consumer warps
+// variants with at most 32 accumulators per thread get dedicated epilogue warps: A4 of tile i then overlaps the
+// frame loop of tile i + 1, which pays when a launch has few frames per pixel (sliding updates, short windows)
+constexpr bool stream_light(int bytes, int rows) { return rows * qld_dev::pick_v(bytes, rows) <= 32; }
+// four epilogue warps for the variants whose frame loop fits in 128 registers (13 warps per CTA)
+constexpr int stream_nepi(int bytes, int rows) { return stream_light(bytes, rows) ? 4 : 0; }
 constexpr int TQ = 16;                // tile-id queue entries (producer runs at most `stages` <= 12 tiles ahead)
 
 struct StreamSmem {
@@ -41,13 +46,13 @@ struct StreamSmem {
         off_w = stages * data_stage;
         off_red = off_w + stages * w_stage;
         off_bar = off_red + red_bytes;
-        total = off_bar + 2 * stages * 8 + TQ * 4 + 16;
+        total = off_bar + 2 * stages * 8 + TQ * 4 + 6 * 8 + 16;
     }
 };
 
-template <typename T, typename ACC, int ROWS, int V>
-__global__ void __launch_bounds__(32 * (NW + 1), 1)
-k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, const StreamShape sh, unsigned int *tile_counter)
+template <typename T, typename ACC, int ROWS, int V, int NWT, int NEPI>
+__global__ void __launch_bounds__(32 * (NWT + 1 + NEPI), 1)
+k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ DemodParams p, const StreamShape sh, unsigned int *tile_counter)
 {
     using PX = Pix<T, V>;
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
@@ -55,15 +60,19 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
     constexpr int VB = V * (int)sizeof(T);                 // bytes per thread per frame
 
     const int SEG = sh.seg, KC = sh.kc, STAGES = sh.stages;
-    const int CG = SEG / (32 * VB), TS = NW / CG;          // column groups, time slices
+    const int CG = SEG / (32 * VB), TS = NWT / CG;          // column groups, time slices
     // combine buffer: [ROWS (+1: pedestal)][V][RS] RED cells, RS = column count padded so that the epilogue's
     // pixel-order reads (v fastest) fall into distinct banks
     constexpr int PAD = 128 / ((int)sizeof(RED) * V) > 0 ? 128 / ((int)sizeof(RED) * V) : 1;
     constexpr int RROWS = ROWS + (IS_INT ? 0 : 1);
-    // pixels per thread whose stored sums are prefetched in a sliding update (registers: PFN * ROWS RED values)
-    constexpr int PFN = IS_INT ? (ROWS <= 4 ? 4 : (ROWS <= 8 ? 2 : 0)) : (ROWS <= 2 ? 4 : (ROWS <= 4 ? 2 : 0));
+    // pixels per thread whose stored sums are prefetched in a sliding update (about 32 registers)
+    constexpr int PFN_ = (IS_INT ? 32 : 16) / ROWS;
+    constexpr int PFN = PFN_ > 8 ? 8 : (PFN_ < 1 ? 1 : PFN_);
     const int RS = CG * 32 + PAD;
-    const StreamSmem SM(SEG, KC, STAGES, ROWS, TS > 1 ? RROWS * V * RS * (int)sizeof(RED) : 0);
+    // epilogue warps (NEPI > 0): the combine buffer is double buffered and finalised by them
+    const bool SPLIT = NEPI > 0 && TS > 1;
+    const int red_cells = RROWS * V * RS;
+    const StreamSmem SM(SEG, KC, STAGES, ROWS, TS > 1 ? (SPLIT ? 2 : 1) * red_cells * (int)sizeof(RED) : 0);
 
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
@@ -73,6 +82,8 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + SM.off_bar);
     uint64_t *empty = full + STAGES;
     volatile int *tile_q = reinterpret_cast<volatile int *>(empty + STAGES);
+    uint64_t *red_full = reinterpret_cast<uint64_t *>(const_cast<int *>(tile_q) + TQ);   // [2] consumers -> epilogue warps
+    uint64_t *red_empty = red_full + 2, *tile_known = red_full + 4;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
@@ -81,7 +92,12 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
     if (threadIdx.x == 0) {
         for (int i = 0; i < STAGES; ++i) {
             mbar_init(&full[i], 2);          // the producer's expect_tx arrival + its "weights written" arrival
-            mbar_init(&empty[i], NW);
+            mbar_init(&empty[i], NWT);
+        }
+        for (int i = 0; i < 2; ++i) {
+            mbar_init(&red_full[i], NWT * 32);
+            mbar_init(&red_empty[i], NEPI > 0 ? NEPI * 32 : 1);
+            mbar_init(&tile_known[i], 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -135,16 +151,98 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
         return;
     }
 
+    // ---- A4 for the pixels q0, q0 + qstride, ... of a tile whose combined sums sit in `redb` (consecutive threads on
+    // consecutive pixels: coalesced accumulator and map traffic).  prefetch_acc requests, ahead of time, the previous
+    // window's sums (A5) of the same pixels.
+    const int TP = SEG / (int)sizeof(T);                   // pixels per tile
+    auto prefetch_acc = [&](int tile, int q0, int qstride, RED (&pf)[PFN][ROWS]) {
+        const RED *accg = static_cast<const RED *>(p.acc_out);
+        const int64_t tile_pix0 = (int64_t)tile * TP;
+#pragma unroll
+        for (int i = 0; i < PFN; ++i) {
+            const int q = q0 + i * qstride;
+            const bool ok = q < TP && tile_pix0 + q < p.HW;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) pf[i][r] = ok ? accg[(int64_t)r * p.HW + tile_pix0 + q] : (RED)0;
+        }
+    };
+    auto finalise_tile = [&](const RED *redb, int tile, int q0, int qstride, const RED (&pf)[PFN][ROWS], bool use_pf) {
+        const int64_t tile_pix0 = (int64_t)tile * TP;
+        RowVals<double, ROWS> wsum;
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) wsum.a[r] = 0.0;
+        if constexpr (!IS_INT) {
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) wsum.a[r] = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
+        }
+        auto finalise_q = [&](int q, int64_t pixel, const RED *prev) {
+            const int v = q % V, tc = q / V;
+            RED *accg = static_cast<RED *>(p.acc_out);
+            double ped = 0.0;
+            if constexpr (!IS_INT) ped = redb[(size_t)(ROWS * V + v) * RS + tc];
+            RowVals<RED, ROWS> a;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) {
+                a.a[r] = redb[(size_t)(r * V + v) * RS + tc];
+                if (p.acc_add) a.a[r] += prev ? prev[r] : accg[(int64_t)r * p.HW + pixel];
+                if (accg) accg[(int64_t)r * p.HW + pixel] = a.a[r];
+            }
+            if constexpr (!IS_INT) {
+                if (p.ped_out) p.ped_out[pixel] = (float)ped;
+            }
+            finalise_pixel_nl<ROWS, IS_INT, RED>(&p.fin, a, ped, wsum, pixel, p.HW);   // sum x w = sum (x - ped) w + ped * sum w
+        };
+        if (use_pf) {
+#pragma unroll
+            for (int i = 0; i < PFN; ++i) {
+                const int q = q0 + i * qstride;
+                if (q < TP && tile_pix0 + q < p.HW) finalise_q(q, tile_pix0 + q, pf[i]);
+            }
+        } else {
+            for (int q = q0; q < TP; q += qstride) {
+                if (tile_pix0 + q >= p.HW) break;
+                finalise_q(q, tile_pix0 + q, nullptr);
+            }
+        }
+    };
+
+    if (warp > NWT) {
+        // ===== epilogue warps: finalise tile i from red[i & 1] while the consumers run the frame loop of tile i + 1 =====
+        if (!SPLIT) return;
+        const int et = (warp - 1 - NWT) * 32 + lane;
+        const bool use_pf = p.acc_add && TP <= PFN * NEPI * 32;
+        for (int it = 0;; ++it) {
+            const int buf = it & 1;
+            const uint32_t par = (uint32_t)(it >> 1) & 1u;
+            mbar_wait(&tile_known[buf], par);
+            const int tile = tile_q[it & (TQ - 1)];
+            if (tile < 0) break;
+            RED pf[PFN][ROWS];
+            if (use_pf) prefetch_acc(tile, et, NEPI * 32, pf);
+            mbar_wait(&red_full[buf], par);
+            finalise_tile(red + (size_t)buf * red_cells, tile, et, NEPI * 32, pf, use_pf);
+            mbar_arrive(&red_empty[buf]);
+        }
+        return;
+    }
+
     // ===== consumers =====
     const int cw = warp - 1, cg = cw % CG, ts = cw / CG;
     const int col = (cg * 32 + lane) * VB;                 // byte offset of this thread's pixels inside the segment
     const int tcol = cg * 32 + lane;                       // thread column inside the tile
-    const int TP = SEG / (int)sizeof(T);                   // pixels per tile
     int stage = 0;
     uint32_t phase = 0;
     for (int it = 0;; ++it) {
         mbar_wait(&full[stage], phase);
         const int tile = tile_q[it & (TQ - 1)];
+        const int buf = SPLIT ? (it & 1) : 0;
+        RED *redb = red + (size_t)buf * red_cells;
+        if (SPLIT) {
+            // red[buf] was last used by tile it - 2: wait until the epilogue warps are done with it, then tell them which
+            // tile comes next in this buffer (they prefetch its stored sums while the frame loop runs)
+            if (it >= 2) mbar_wait(&red_empty[buf], ((uint32_t)(it >> 1) & 1u) ^ 1u);
+            if (cw == 0 && lane == 0) mbar_arrive(&tile_known[buf]);
+        }
         if (tile < 0) break;
         const int64_t pix0 = ((int64_t)tile * SEG + col) / (int64_t)sizeof(T);
         const bool active = pix0 < p.HW;
@@ -168,21 +266,10 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
             }
         }
 
-        // A5: the previous window's sums of the pixels this thread finalises, requested now so that the loads
-        // complete under the frame loop
-        const int64_t tile_pix0 = (int64_t)tile * TP;
-        RED pf[PFN > 0 ? PFN : 1][ROWS];
-        const bool use_pf = PFN > 0 && p.acc_add && TS > 1 && TP <= PFN * NW * 32;
-        if (use_pf) {
-            const RED *accg = static_cast<const RED *>(p.acc_out);
-#pragma unroll
-            for (int i = 0; i < (PFN > 0 ? PFN : 1); ++i) {
-                const int q = cw * 32 + lane + i * NW * 32;
-                const bool ok = q < TP && tile_pix0 + q < p.HW;
-#pragma unroll
-                for (int r = 0; r < ROWS; ++r) pf[i][r] = ok ? accg[(int64_t)r * p.HW + tile_pix0 + q] : (RED)0;
-            }
-        }
+        // without epilogue warps the consumers finalise: request the stored sums now, under the frame loop
+        RED pf[PFN][ROWS];
+        const bool use_pf = !SPLIT && p.acc_add && TS > 1 && TP <= PFN * NWT * 32;
+        if (use_pf) prefetch_acc(tile, cw * 32 + lane, NWT * 32, pf);
 
         bool first = true;
         for (int run = 0; run < p.n_runs; ++run) {
@@ -214,7 +301,12 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
                             load_weights_shared<ACC, ROWS>(wrow + (f + u * TS) * ROWS, wt[u]);
                         }
 #pragma unroll
-                        for (int u = 0; u < 4; ++u) accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc);
+                        for (int u = 0; u < 4; ++u) {
+                            if constexpr (IS_INT) {
+                                if (p.onehot) { accumulate_onehot<T, ROWS, V>(w[u], wt[u], acc); continue; }
+                            }
+                            accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc);
+                        }
                     }
                 } else {
                     for (; f < nf; f += TS) {
@@ -222,6 +314,9 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
                         ACC wt[ROWS];
                         PX::load_shared(d + (size_t)f * SEG, w);
                         load_weights_shared<ACC, ROWS>(wrow + f * ROWS, wt);
+                        if constexpr (IS_INT) {
+                            if (p.onehot) { accumulate_onehot<T, ROWS, V>(w, wt, acc); continue; }
+                        }
                         accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc);
                     }
                 }
@@ -232,102 +327,66 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const DemodParams p, co
         }
 
         if (TS > 1) {
-            // ---- combine the TS time slices (fp64 / int32).  The ROWS*V values of a thread are cut into NW chunks;
+            // ---- combine the TS time slices (fp64 / int32).  The ROWS*V values of a thread are cut into NWT chunks;
             // in turn j slice ts adds the chunks c with c = ts + j (mod TS), so every slice works in every turn and
             // no two slices touch a cell in the same turn.  Turn 0 stores (first touch), later turns add.
-            constexpr int CH = ROWS * V / NW;
-            static_assert(CH >= 1 && CH * NW == ROWS * V, "chunking");
+            constexpr int CH = ROWS * V / NWT;
+            static_assert(CH >= 1 && CH * NWT == ROWS * V, "chunking");
             for (int j = 0; j < TS; ++j) {
                 const int want = (ts + j) & (TS - 1);
 #pragma unroll
-                for (int c = 0; c < NW; ++c) {
+                for (int c = 0; c < NWT; ++c) {
                     if ((c & (TS - 1)) != want) continue;
                     RED t[CH];
 #pragma unroll
                     for (int e = 0; e < CH; ++e) {
                         const int i = c * CH + e;
-                        t[e] = (j == 0) ? (RED)0 : red[(size_t)i * RS + tcol];
+                        t[e] = (j == 0) ? (RED)0 : redb[(size_t)i * RS + tcol];
                     }
 #pragma unroll
                     for (int e = 0; e < CH; ++e) {
                         const int i = c * CH + e;
-                        red[(size_t)i * RS + tcol] = t[e] + (RED)acc[i / V][i % V];
+                        redb[(size_t)i * RS + tcol] = t[e] + (RED)acc[i / V][i % V];
                     }
                 }
                 if constexpr (!IS_INT) {
                     if (j == 0 && ts == 0) {
 #pragma unroll
-                        for (int v = 0; v < V; ++v) red[(size_t)(ROWS * V + v) * RS + tcol] = (RED)(pedm[v] - 8388608.0f);
+                        for (int v = 0; v < V; ++v) redb[(size_t)(ROWS * V + v) * RS + tcol] = (RED)(pedm[v] - 8388608.0f);
                     }
                 }
-                named_barrier(1, NW * 32);
+                if (SPLIT && j == TS - 1) mbar_arrive(&red_full[buf]);   // every consumer thread: its cells are written
+                else named_barrier(1, NWT * 32);
             }
-            // ---- A4, consecutive threads on consecutive pixels ----
-            auto finalise_q = [&](int q, int64_t pixel, const RED *prev) {
-                const int v = q % V, tc = q / V;
-                double val[ROWS];
-                RED *accg = static_cast<RED *>(p.acc_out);
-                double ped = 0.0;
-                if constexpr (!IS_INT) ped = red[(size_t)(ROWS * V + v) * RS + tc];
+            if (!SPLIT) {
+                finalise_tile(redb, tile, cw * 32 + lane, NWT * 32, pf, use_pf);
+                named_barrier(1, NWT * 32);                 // red is free for the next tile
+            }
+        } else if (active) {
+            // one slice per column group (narrow vectors): every thread finalises its own V pixels
+            RowVals<double, ROWS> wsum;
+#pragma unroll
+            for (int r = 0; r < ROWS; ++r) wsum.a[r] = 0.0;
+            if constexpr (!IS_INT) {
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) wsum.a[r] = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
+            }
+            RED *accg = static_cast<RED *>(p.acc_out);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const int64_t pixel = pix0 + v;
+                const double ped = IS_INT ? 0.0 : (double)(pedm[v] - 8388608.0f);
+                RowVals<RED, ROWS> a;
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) {
-                    RED a = red[(size_t)(r * V + v) * RS + tc];
-                    if (p.acc_add) a += prev ? prev[r] : accg[(int64_t)r * p.HW + pixel];
-                    if (accg) accg[(int64_t)r * p.HW + pixel] = a;
-                    if constexpr (IS_INT) {
-                        val[r] = (double)a;
-                    } else {
-                        const double wsum = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
-                        val[r] = a + ped * wsum;           // sum x w = sum (x - ped) w + ped * sum w
-                    }
+                    a.a[r] = (RED)acc[r][v];
+                    if (p.acc_add) a.a[r] += accg[(int64_t)r * p.HW + pixel];
+                    if (accg) accg[(int64_t)r * p.HW + pixel] = a.a[r];
                 }
                 if constexpr (!IS_INT) {
                     if (p.ped_out) p.ped_out[pixel] = (float)ped;
                 }
-                finalise_pixel<ROWS>(p.fin, val, pixel, p.HW);
-            };
-            if (use_pf) {
-#pragma unroll
-                for (int i = 0; i < (PFN > 0 ? PFN : 1); ++i) {
-                    const int q = cw * 32 + lane + i * NW * 32;
-                    if (q < TP && tile_pix0 + q < p.HW) finalise_q(q, tile_pix0 + q, pf[i]);
-                }
-            } else {
-                for (int q = cw * 32 + lane; q < TP; q += NW * 32) {
-                    if (tile_pix0 + q >= p.HW) break;
-                    finalise_q(q, tile_pix0 + q, nullptr);
-                }
-            }
-            named_barrier(1, NW * 32);                     // red is free for the next tile
-        } else if (active) {
-            // one slice per column group (narrow vectors): every thread finalises its own V pixels
-#pragma unroll
-            for (int v = 0; v < V; ++v) {
-                const int64_t pixel = pix0 + v;
-                double val[ROWS];
-                if constexpr (IS_INT) {
-                    int *accg = static_cast<int *>(p.acc_out);
-#pragma unroll
-                    for (int r = 0; r < ROWS; ++r) {
-                        int a = acc[r][v];
-                        if (p.acc_add) a += accg[(int64_t)r * p.HW + pixel];
-                        if (accg) accg[(int64_t)r * p.HW + pixel] = a;
-                        val[r] = (double)a;
-                    }
-                } else {
-                    double *accg = static_cast<double *>(p.acc_out);
-                    const double ped = (double)(pedm[v] - 8388608.0f);
-#pragma unroll
-                    for (int r = 0; r < ROWS; ++r) {
-                        double a = (double)acc[r][v];
-                        if (p.acc_add) a += accg[(int64_t)r * p.HW + pixel];
-                        if (accg) accg[(int64_t)r * p.HW + pixel] = a;
-                        const double wsum = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
-                        val[r] = a + ped * wsum;
-                    }
-                    if (p.ped_out) p.ped_out[pixel] = (float)ped;
-                }
-                finalise_pixel<ROWS>(p.fin, val, pixel, p.HW);
+                finalise_pixel_nl<ROWS, IS_INT, RED>(&p.fin, a, ped, wsum, pixel, p.HW);
             }
         }
     }
@@ -337,29 +396,35 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-int red_bytes_for(int seg, int vb, int rows, int v, bool is_int)
+int red_bytes_for(int seg, int vb, int rows, int v, bool is_int, int nw, int nepi)
 {
-    const int cg = seg / (32 * vb), ts = NW / cg;
+    const int cg = seg / (32 * vb), ts = nw / cg;
     const int esz = is_int ? 4 : 8;
     const int pad = 128 / (esz * v) > 0 ? 128 / (esz * v) : 1;
-    return ts > 1 ? (rows + (is_int ? 0 : 1)) * v * (cg * 32 + pad) * esz : 0;
+    return ts > 1 ? (nepi > 0 ? 2 : 1) * (rows + (is_int ? 0 : 1)) * v * (cg * 32 + pad) * esz : 0;
 }
 
-template <typename T, typename ACC, int ROWS>
-cudaError_t launch_stream_t(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
+template <typename T, typename ACC, int ROWS, int NWT, int NEPI>
+cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
 {
     constexpr int V = pick_v(sizeof(T), ROWS);
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
-    const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT));
-    auto kern = k_demod_stream<T, ACC, ROWS, V>;
+    const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT, NWT, NEPI));
+    auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
     if (e != cudaSuccess) return e;
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
     const int n_tiles = (int)((row_bytes + sh.seg - 1) / sh.seg);
     e = cudaMemsetAsync(counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) return e;
-    kern<<<n_tiles < n_sms ? n_tiles : n_sms, 32 * (NW + 1), SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, counter);
+    kern<<<n_tiles < n_sms ? n_tiles : n_sms, 32 * (NWT + 1 + NEPI), SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, counter);
     return cudaGetLastError();
+}
+
+template <typename T, typename ACC, int ROWS>
+cudaError_t launch_stream_t(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
+{
+    return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS)>(tmap, p, sh, counter, n_sms, st);
 }
 
 template <typename T, typename ACC>
@@ -378,31 +443,33 @@ cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, co
 
 // Tile shape for this (dtype, rows, frame size), or seg = 0 when the streaming kernel does not apply (row pitch or
 // base not 16-byte aligned, or a frame too small to give every SM a tile: k_demod_whole handles those).
-StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms)
+StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int frames_per_pixel)
 {
-    StreamShape sh = {0, 0, 0};
+    StreamShape sh = {0, 0, 0, NW};
     const int bytes = dtype == QLD_U8 ? 1 : 2;
     const int v = pick_v(bytes, rows), vb = v * bytes;
     const int64_t row_bytes = HW * bytes;
     if (row_bytes % 16 != 0 || (reinterpret_cast<uintptr_t>(frames) & 15) != 0) return sh;
+    (void)frames_per_pixel;
+    const int nw = NW, mb = 1;
     int seg = 2048;                                        // TMA box: at most 256 8-byte elements per row
-    if (seg > NW * 32 * vb) seg = NW * 32 * vb;
+    if (seg > nw * 32 * vb) seg = nw * 32 * vb;
     while (seg > 32 * vb && (row_bytes + seg - 1) / seg < 4 * (int64_t)n_sms) seg /= 2;
     int kc = 16, stages = 0;
     bool forced = false;
     if (const char *e = getenv("QLD_STREAM_TILE")) {      // tuning / test override: "SEG,KC" (also lifts the size threshold)
         int s2 = 0, k2 = 0;
-        if (sscanf(e, "%d,%d", &s2, &k2) == 2 && s2 >= 32 * vb && s2 <= NW * 32 * vb && s2 <= 2048 && (s2 & (s2 - 1)) == 0 && k2 >= 4 && k2 <= 256) { seg = s2; kc = k2; forced = true; }
+        if (sscanf(e, "%d,%d", &s2, &k2) == 2 && s2 >= 32 * vb && s2 <= nw * 32 * vb && s2 <= 2048 && (s2 & (s2 - 1)) == 0 && k2 >= 4 && k2 <= 256) { seg = s2; kc = k2; forced = true; }
     }
     if (!forced && (row_bytes + seg - 1) / seg < n_sms) return sh;
-    const int ts = NW / (seg / (32 * vb));
+    const int ts = nw / (seg / (32 * vb));
     if (kc < 4 * ts) kc = 4 * ts;                          // every slice gets a multiple of four frames per stage
     kc = (kc + 4 * ts - 1) / (4 * ts) * (4 * ts);
-    const int red = red_bytes_for(seg, vb, rows, v, is_int != 0);
-    stages = (int)((200 * 1024 - red) / (seg * kc + kc * rows * 4));
+    const int red = red_bytes_for(seg, vb, rows, v, is_int != 0, nw, stream_nepi(bytes, rows));
+    stages = (int)((200 * 1024 / mb - red) / (seg * kc + kc * rows * 4));
     if (stages > 12) stages = 12;
-    if (stages < 2) return StreamShape{0, 0, 0};
-    sh.seg = seg; sh.kc = kc; sh.stages = stages;
+    if (stages < 2) return StreamShape{0, 0, 0, NW};
+    sh.seg = seg; sh.kc = kc; sh.stages = stages; sh.nw = nw;
     return sh;
 }
 

@@ -42,7 +42,7 @@ def _gpu_on_pixels(ctx, k, pix):
 
 @pytest.mark.parametrize("name,accum_name,kernel", [("cfg1", "AUTO", "k_demod_stream"), ("cfg1", "FP32", "k_demod_stream"),
                                                    ("cfg2", "AUTO", "k_demod_stream"), ("cfg2", "FIXED", "k_demod_tc"),
-                                                   ("cfg4", "AUTO", None), ("cfg4", "FP32", "k_demod_stream"), ("cfg4", "FIXED", "k_demod_tc")])
+                                                   ("cfg4", "AUTO", "k_demod_tc"), ("cfg4", "FP32", "k_demod_stream"), ("cfg4", "FIXED", "k_demod_tc")])
 def test_whole_window_full_size_sampled(Q, oracle, name, accum_name, kernel):
     import torch
     from paper_1511_03390_b200 import synth

@@ -154,3 +154,26 @@ def test_fixed_rejects_what_it_cannot_do(Q):
     with pytest.raises(Q.QLDError) as e:
         Q.QLD(4, 16, "u8", 16, [{"nu": 0.1}], ring_frames=40, accum=Q.QLD_ACC_FIXED)
     assert e.value.status == Q.QLD_E_UNSUPPORTED
+
+
+def test_auto_moves_k_ge_4_to_the_tensor_cores(Q, oracle):
+    """AUTO: K >= 4 float references on a whole-window store -> FIXED (k_demod_tc); on a ring, or for K < 4 -> FP32."""
+    rng = np.random.default_rng(11)
+    H, W, N = 16, 64, 96
+    x = rng.integers(0, 4096, size=(N, H, W)).astype(np.uint16)
+    refs = [{"nu": 0.07 + 0.09 * k, "phase": 0.2 * k} for k in range(4)]
+    ctx = Q.QLD(H, W, "u16", N, refs)
+    assert ctx.accum_name() == "FIXED"
+    ctx.push_frames(x); ctx.demod(Q.QLD_WHOLE); ctx.sync()
+    assert ctx.last_kernel() == "k_demod_tc"
+    for k in range(4):
+        got = tuple(m.cpu().numpy() for m in ctx.get_maps(k))
+        check_float_maps(got, oracle_maps(oracle, x, refs[k]), rel=1e-6, what=f"auto fixed k={k}")
+    ctx.destroy()
+    for kw, n_refs in ((dict(ring_frames=N + 16), 4), (dict(), 3)):
+        c2 = Q.QLD(H, W, "u16", N, refs[:n_refs], **kw)
+        assert c2.accum_name() == "FP32"
+        c2.destroy()
+    c3 = Q.QLD(3, 7, "u8", N, refs)              # 21-byte frames: not a TMA row pitch -> FP32
+    assert c3.accum_name() == "FP32"
+    c3.destroy()
