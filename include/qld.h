@@ -210,6 +210,15 @@ int64_t qld_kernel_launches(const qld_ctx *ctx);
 int qld_accum_mode(const qld_ctx *ctx);
 const char *qld_last_kernel(const qld_ctx *ctx);
 
+/* Contrast-to-noise ratio of a processed image (Eq. (1), Fig. 6; the paper's quality metric, the step
+ * after the path):  CNR = (mean_s - mean_surr) / sqrt( mean over the slice of (I(j,k) - mean_surr)^2 ), mean_s
+ * over the m x m source square with top-left pixel (y0, x0), the slice being the m-pixel wide square ring around
+ * it (8 m^2 pixels, which must lie inside the frame: QLD_E_INVAL otherwise).  map_device: row-major [H][W] float32
+ * in device memory (e.g. an amplitude map from qld_get_maps).  Enqueued on `stream` (cudaStream_t or NULL); writes
+ * out_device[0..3] = {CNR, mean_s, mean_surr, rms} (device memory, 4 doubles); fp64 arithmetic, IEEE inf / nan when
+ * the slice is flat. */
+int qld_cnr(const float *map_device, int32_t H, int32_t W, int32_t y0, int32_t x0, int32_t m, double *out_device, void *stream);
+
 /* ---- synthetic input filler (not part of the method; device twin of paper_1511_03390_b200/synth.py) ---- */
 typedef struct {
     int32_t H, W;

@@ -170,3 +170,33 @@ def qld_sliding(stream: np.ndarray, ref: dict, N: int, hop: int, nthreads: int =
     for w in (range(n_win) if windows is None else windows):
         a = w * hop
         yield (w,) + qld(stream[a:a + N], ref, s_first=a + 1, nthreads=nthreads)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Contrast-to-noise ratio (Eq. (1), Fig. 6) -- SURVEY.md 8(f1), the step after the path
+# ---------------------------------------------------------------------------------------------------
+def cnr_regions(H: int, W: int, y0: int, x0: int, m: int):
+    """Boolean masks (source, surround) of Fig. 6: the m x m source square with top-left corner
+    (y0, x0) and the m-pixel wide square slice around it, i.e. the 3m x 3m square minus the source: 8 m^2 pixels
+    (PAPER.md:109).  The slice must lie inside the frame."""
+    if m < 1 or y0 - m < 0 or x0 - m < 0 or y0 + 2 * m > H or x0 + 2 * m > W:
+        raise ValueError("cnr: the surrounding slice must lie inside the frame")
+    src = np.zeros((H, W), dtype=bool)
+    big = np.zeros((H, W), dtype=bool)
+    src[y0:y0 + m, x0:x0 + m] = True
+    big[y0 - m:y0 + 2 * m, x0 - m:x0 + 2 * m] = True
+    return src, big & ~src
+
+
+def cnr(image: np.ndarray, y0: int, x0: int, m: int):
+    """Eq. (1): CNR = (mean_s - mean_surr) / sqrt(mean over the slice of (I(j,k) - mean_surr)^2), fp64, term by term
+    as printed.  Returns (cnr, mean_s, mean_surr, rms); IEEE semantics when the slice is flat (rms = 0)."""
+    img = np.asarray(image, dtype=np.float64)
+    src, ring = cnr_regions(img.shape[0], img.shape[1], y0, x0, m)
+    mean_s = img[src].sum() / float(m * m)
+    r = img[ring]
+    mean_surr = r.sum() / float(8 * m * m)
+    rms = np.sqrt(((r - mean_surr) ** 2).sum() / float(8 * m * m))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ratio = np.float64(mean_s - mean_surr) / np.float64(rms)
+    return float(ratio), float(mean_s), float(mean_surr), float(rms)

@@ -434,7 +434,7 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
     p.onehot = c->is_int && c->K == 1;
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->N);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
     if (sh.seg > 0) {
         int rc = stream_tmap_for(c, sh);
         if (rc) return rc;
@@ -452,7 +452,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
 {
     const int64_t a_new = a_old + hop;
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, 2 * hop);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
     if (sh.seg > 0 && hop >= sh.kc) {
         DemodParams p;
         memset(&p, 0, sizeof p);

@@ -12,7 +12,10 @@
 // SEG bytes of every frame of the window; tiles are claimed from a global counter.  Inside a tile, consumer warp w
 // owns column group (w % CG) -- 32 lanes x V pixels -- and time slice (w / CG): it takes every TS-th frame of each
 // stage.  Slices are combined through shared memory at the end of the tile (fp64 / int32), then the A4 epilogue
-// runs with consecutive threads on consecutive pixels (coalesced accumulator and map traffic).
+// runs with consecutive threads on consecutive pixels (coalesced accumulator and map traffic).  Variants with at
+// most 32 accumulators per thread carry four more warps (10..13) that do nothing but this epilogue, out of a double
+// buffered combine buffer, so that A4 of tile i overlaps the frame loop of tile i + 1 (hand-off by mbarriers:
+// tile_known -> red_full -> red_empty).
 //
 // The frames of a launch are a list of runs (DemodRun): a whole window is one or two runs of weight +w, and the
 // sliding update of PAPER.md:181-183 (A5) is the same kernel over {expired frames, -w} + {new frames, +w} with the
@@ -443,15 +446,14 @@ cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, co
 
 // Tile shape for this (dtype, rows, frame size), or seg = 0 when the streaming kernel does not apply (row pitch or
 // base not 16-byte aligned, or a frame too small to give every SM a tile: k_demod_whole handles those).
-StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int frames_per_pixel)
+StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms)
 {
-    StreamShape sh = {0, 0, 0, NW};
+    StreamShape sh = {0, 0, 0};
     const int bytes = dtype == QLD_U8 ? 1 : 2;
     const int v = pick_v(bytes, rows), vb = v * bytes;
     const int64_t row_bytes = HW * bytes;
     if (row_bytes % 16 != 0 || (reinterpret_cast<uintptr_t>(frames) & 15) != 0) return sh;
-    (void)frames_per_pixel;
-    const int nw = NW, mb = 1;
+    const int nw = NW;
     int seg = 2048;                                        // TMA box: at most 256 8-byte elements per row
     if (seg > nw * 32 * vb) seg = nw * 32 * vb;
     while (seg > 32 * vb && (row_bytes + seg - 1) / seg < 4 * (int64_t)n_sms) seg /= 2;
@@ -466,10 +468,10 @@ StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const 
     if (kc < 4 * ts) kc = 4 * ts;                          // every slice gets a multiple of four frames per stage
     kc = (kc + 4 * ts - 1) / (4 * ts) * (4 * ts);
     const int red = red_bytes_for(seg, vb, rows, v, is_int != 0, nw, stream_nepi(bytes, rows));
-    stages = (int)((200 * 1024 / mb - red) / (seg * kc + kc * rows * 4));
+    stages = (int)((200 * 1024 - red) / (seg * kc + kc * rows * 4));
     if (stages > 12) stages = 12;
-    if (stages < 2) return StreamShape{0, 0, 0, NW};
-    sh.seg = seg; sh.kc = kc; sh.stages = stages; sh.nw = nw;
+    if (stages < 2) return StreamShape{0, 0, 0};
+    sh.seg = seg; sh.kc = kc; sh.stages = stages;
     return sh;
 }
 

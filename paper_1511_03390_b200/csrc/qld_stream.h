@@ -9,10 +9,9 @@ struct StreamShape {
     int32_t seg;      // contiguous bytes of every frame per tile (0: the streaming kernel does not apply)
     int32_t kc;       // frames per pipeline stage
     int32_t stages;   // shared-memory stages
-    int32_t nw;       // consumer warps per CTA: 8 (one CTA per SM) or 4 (two CTAs per SM)
 };
 
-StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int frames_per_pixel);
+StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms);
 cudaError_t qld_stream_encode_tmap(void *tmap_out /*128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int cap, const StreamShape &sh);
 cudaError_t qld_launch_demod_stream(int dtype, int is_int, int rows, const void *tmap, const DemodParams &p, const StreamShape &sh,
                                     unsigned int *counter, int n_sms, cudaStream_t st);

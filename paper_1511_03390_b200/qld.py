@@ -27,7 +27,7 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
            "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
            "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel",
-           "qld_synth_fill"]
+           "qld_cnr", "qld_synth_fill"]
 
 
 class qld_ref(C.Structure):
@@ -98,6 +98,7 @@ def load_library():
     l.qld_accum_mode.argtypes = [vp]
     l.qld_last_kernel.argtypes = [vp]
     l.qld_last_kernel.restype = C.c_char_p
+    l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
     l.qld_synth_fill.argtypes = [C.POINTER(qld_synth_scene), i64, i, vp, vp]
     _lib = l
     return l
@@ -289,6 +290,20 @@ class QLD:
             self.destroy()
         except Exception:
             pass
+
+
+def cnr(image, y0: int, x0: int, m: int):
+    """qld_cnr on a CUDA float32 map [H, W]: returns a CUDA tensor of 4 doubles {CNR, mean_s, mean_surr, rms}
+    (Eq. (1)), enqueued on torch's current stream."""
+    import torch
+    lib = load_library()
+    assert image.is_cuda and image.dtype == torch.float32 and image.is_contiguous() and image.dim() == 2
+    out = torch.empty(4, dtype=torch.float64, device=image.device)
+    rc = lib.qld_cnr(image.data_ptr(), int(image.shape[0]), int(image.shape[1]), int(y0), int(x0), int(m), out.data_ptr(),
+                     torch.cuda.current_stream(image.device).cuda_stream or 1)
+    if rc != QLD_OK:
+        raise QLDError(rc, "qld_cnr")
+    return out
 
 
 def synth_fill(scene, s_first: int, n_frames: int, out=None, device="cuda"):

@@ -315,3 +315,45 @@ def cfg4(H: int = 2048, W: int = 2048, N: int = 2048, K: int = 8, seed: int = 4)
 
 
 BUILDERS = {"cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4}
+
+
+# ----------------------------------------------------------------------------------------------
+# The paper's own numerical simulation (Fig. 1): SURVEY.md 8(f1), a second workload
+# ----------------------------------------------------------------------------------------------
+@dataclass
+class PaperSim:
+    """Frames of the five-source scene plus where the sources sit."""
+    frames: np.ndarray                        # [N, n, n] uint16
+    boxes: Tuple[Tuple[int, int], ...]        # top-left (y0, x0) of the five m x m sub-regions; the last one is constant
+    m: int
+    nus: Tuple[float, ...]                    # f_i / f_s of the four modulated sources
+    gain: float
+    X: float
+
+
+def paper_sim(n: int = 96, m: int = 8, N: int = 82, X: float = 5.0, nus: Sequence[float] = (0.20, 0.23, 0.26, 0.29),
+              seed: int = 7, gain: float = 1000.0) -> PaperSim:
+    """an n x n frame with five non-overlapping m x m sub-regions; in four of them the intensity is
+    (0.5 + sin(omega_i t_s)), t_s = s dt, s = 1..N, the fifth is held constant; every pixel of every frame gets an
+    independent random number uniform in [0, X] (X in 1..10 in the paper).
+    The paper does not give n, m, dt or the noise generator; the defaults here are this build's choice (DESIGN.md
+    reading G21): frequencies 20/23/26/29 Hz at an assumed 100 frames/s, N = 82
+    (PAPER.md:37).  Intensities are real numbers in the paper; the device path takes integers, so the frame is
+    x = rint(gain * (intensity + 0.5)) as uint16 -- an affine map, which leaves Eq. (1)'s CNR of a map that is linear
+    in the data unchanged and only adds the constant-background leakage of reading G9."""
+    assert n >= 9 * m and len(nus) == 4
+    # five boxes: four around the centre of each quadrant's inner half and one in the middle, each with room for
+    # the m-wide surround of Fig. 6
+    c = [(n // 4, n // 4), (n // 4, 3 * n // 4), (3 * n // 4, n // 4), (3 * n // 4, 3 * n // 4), (n // 2, n // 2)]
+    boxes = tuple((cy - m // 2, cx - m // 2) for cy, cx in c)
+    key = seed_key(seed, 1)
+    s = np.arange(1, N + 1, dtype=np.int64)[:, None]
+    p = np.arange(n * n, dtype=np.int64)[None, :]
+    u = unit_uniform(key, (s.astype(np.uint64) * np.uint64(n * n) + p.astype(np.uint64)))
+    inten = (X * u).reshape(N, n, n)
+    t = np.arange(1, N + 1, dtype=np.float64)
+    for i, (y0, x0) in enumerate(boxes):
+        src = (0.5 + np.sin(2.0 * np.pi * nus[i] * t)) if i < 4 else np.full(N, 1.5)
+        inten[:, y0:y0 + m, x0:x0 + m] += src[:, None, None]
+    x = np.clip(np.rint(gain * (inten + 0.5)), 0, 65535).astype(np.uint16)
+    return PaperSim(x, boxes, m, tuple(float(v) for v in nus), float(gain), float(X))
