@@ -64,6 +64,43 @@ struct Pix {
     }
 };
 
+// N consecutive values of type E (N * sizeof(E) a multiple of 16, pointer 16-byte aligned) as 16-byte accesses
+template <typename E, int N>
+__device__ __forceinline__ void load_vec(const E *ptr, E (&out)[N])
+{
+    constexpr int PER = 16 / (int)sizeof(E);
+    if constexpr (N % PER == 0) {
+#pragma unroll
+        for (int i = 0; i < N / PER; ++i) {
+            const int4 t = reinterpret_cast<const int4 *>(ptr)[i];
+            alignas(16) E tmp[PER];
+            *reinterpret_cast<int4 *>(tmp) = t;
+#pragma unroll
+            for (int j = 0; j < PER; ++j) out[i * PER + j] = tmp[j];
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) out[i] = ptr[i];
+    }
+}
+template <typename E, int N>
+__device__ __forceinline__ void store_vec(E *ptr, const E (&in)[N])
+{
+    constexpr int PER = 16 / (int)sizeof(E);
+    if constexpr (N % PER == 0) {
+#pragma unroll
+        for (int i = 0; i < N / PER; ++i) {
+            alignas(16) E tmp[PER];
+#pragma unroll
+            for (int j = 0; j < PER; ++j) tmp[j] = in[i * PER + j];
+            reinterpret_cast<int4 *>(ptr)[i] = *reinterpret_cast<const int4 *>(tmp);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < N; ++i) ptr[i] = in[i];
+    }
+}
+
 // weights of one frame: ROWS values, identical for every thread (broadcast load through L1)
 template <typename ACC, int ROWS>
 __device__ __forceinline__ void load_weights(const ACC *row, ACC (&wt)[ROWS])

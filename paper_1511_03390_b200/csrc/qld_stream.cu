@@ -35,7 +35,19 @@ namespace {
 constexpr int NW = 8;                 // consumer warps
 // variants with at most 32 accumulators per thread get dedicated epilogue warps: A4 of tile i then overlaps the
 // frame loop of tile i + 1, which pays when a launch has few frames per pixel (sliding updates, short windows)
-constexpr bool stream_light(int bytes, int rows) { return rows * qld_dev::pick_v(bytes, rows) <= 32; }
+// pixels per thread: at most QLD_STREAM_VB bytes of every frame.  16 (LDS.128) is the measured optimum: with 8 the
+// eight consumer warps of a 2 KB segment own eight distinct column groups (TS = 1, no slices to combine, every
+// thread finalises its own pixels from registers), but the per-frame overhead (weight loads, the one-hot branch) is
+// then spread over half as many pixels: cfg3 hop 41 -> 46 us, integer whole window 196 -> 272 us.
+#ifndef QLD_STREAM_VB
+#define QLD_STREAM_VB 16
+#endif
+constexpr int stream_v(int bytes, int rows)
+{
+    const int v = qld_dev::pick_v(bytes, rows), cap = QLD_STREAM_VB / bytes;
+    return v < cap ? v : cap;
+}
+constexpr bool stream_light(int bytes, int rows) { return rows * stream_v(bytes, rows) <= 32; }
 // four epilogue warps for the variants whose frame loop fits in 128 registers (13 warps per CTA)
 constexpr int stream_nepi(int bytes, int rows) { return stream_light(bytes, rows) ? 4 : 0; }
 constexpr int TQ = 16;                // tile-id queue entries (producer runs at most `stages` <= 12 tiles ahead)
@@ -274,6 +286,19 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
         const bool use_pf = !SPLIT && p.acc_add && TS > 1 && TP <= PFN * NWT * 32;
         if (use_pf) prefetch_acc(tile, cw * 32 + lane, NWT * 32, pf);
 
+        // one slice per column group: the thread finalises its own V pixels; their stored sums (A5) are requested now
+        // (a 2 KB segment has eight column groups only when a thread takes at most 8 bytes per frame)
+        constexpr bool CAN_OWN = VB <= 8;
+        RED prev[CAN_OWN ? ROWS : 1][CAN_OWN ? V : 1];
+        const bool own_prev = CAN_OWN && TS == 1 && p.acc_add && active;
+        if constexpr (CAN_OWN) {
+            if (own_prev) {
+                const RED *accg = static_cast<const RED *>(p.acc_out);
+#pragma unroll
+                for (int r = 0; r < ROWS; ++r) load_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, prev[r]);
+            }
+        }
+
         bool first = true;
         for (int run = 0; run < p.n_runs; ++run) {
             const int rn = p.run[run].n;
@@ -365,32 +390,61 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
                 finalise_tile(redb, tile, cw * 32 + lane, NWT * 32, pf, use_pf);
                 named_barrier(1, NWT * 32);                 // red is free for the next tile
             }
-        } else if (active) {
-            // one slice per column group (narrow vectors): every thread finalises its own V pixels
-            RowVals<double, ROWS> wsum;
-#pragma unroll
-            for (int r = 0; r < ROWS; ++r) wsum.a[r] = 0.0;
-            if constexpr (!IS_INT) {
-#pragma unroll
-                for (int r = 0; r < ROWS; ++r) wsum.a[r] = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
-            }
+        } else if (CAN_OWN && active) {
+          if constexpr (CAN_OWN) {
+            // one slice per column group: every thread finalises its own V pixels from registers, 16-byte accesses
             RED *accg = static_cast<RED *>(p.acc_out);
+            RED a[ROWS][V];
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-                const int64_t pixel = pix0 + v;
-                const double ped = IS_INT ? 0.0 : (double)(pedm[v] - 8388608.0f);
-                RowVals<RED, ROWS> a;
+            for (int r = 0; r < ROWS; ++r) {
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) {
-                    a.a[r] = (RED)acc[r][v];
-                    if (p.acc_add) a.a[r] += accg[(int64_t)r * p.HW + pixel];
-                    if (accg) accg[(int64_t)r * p.HW + pixel] = a.a[r];
-                }
-                if constexpr (!IS_INT) {
-                    if (p.ped_out) p.ped_out[pixel] = (float)ped;
-                }
-                finalise_pixel_nl<ROWS, IS_INT, RED>(&p.fin, a, ped, wsum, pixel, p.HW);
+                for (int v = 0; v < V; ++v) a[r][v] = (RED)acc[r][v] + (own_prev ? prev[r][v] : (RED)0);
+                if (accg) store_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, a[r]);
             }
+            float pedf[V];
+#pragma unroll
+            for (int v = 0; v < V; ++v) pedf[v] = pedm[v] - 8388608.0f;
+            if constexpr (!IS_INT) {
+                if (p.ped_out) store_vec<float, V>(p.ped_out + pix0, pedf);
+            }
+            const FinParams &f = p.fin;
+            for (int k = 0; k < f.K; ++k) {
+                float oI[V], oQ[V], oA[V], oP[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    double S = 0.0, C = 0.0;
+                    if constexpr (IS_INT) {
+                        const int off = f.row_off[k], end = off + f.n_rows[k];
+#pragma unroll
+                        for (int r = 0; r < ROWS; ++r)
+                            if (r >= off && r < end) {
+                                S = fma((double)a[r][v], f.sw[r], S);
+                                C = fma((double)a[r][v], f.cw[r], C);
+                            }
+                    } else {
+#pragma unroll
+                        for (int r = 0; r + 1 < ROWS; r += 2)
+                            if (r == 2 * k) {
+                                const double ws = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
+                                const double wc = p.cum[(int64_t)p.cum_hi * ROWS + r + 1] - p.cum[(int64_t)p.cum_lo * ROWS + r + 1];
+                                S = (double)a[r][v] + (double)pedf[v] * ws;          // sum x w = sum (x - ped) w + ped * sum w
+                                C = (double)a[r + 1][v] + (double)pedf[v] * wc;
+                            }
+                    }
+                    S *= f.scale;
+                    C *= f.scale;
+                    oI[v] = (float)S;
+                    oQ[v] = (float)C;
+                    oA[v] = f.amp ? (float)sqrt(S * S + C * C) : 0.0f;
+                    oP[v] = (f.phase && !(S == 0.0 && C == 0.0)) ? (float)atan2(C, S) : 0.0f;
+                }
+                const int64_t o = (int64_t)k * p.HW + pix0;
+                if (f.I) store_vec<float, V>(f.I + o, oI);
+                if (f.Q) store_vec<float, V>(f.Q + o, oQ);
+                if (f.amp) store_vec<float, V>(f.amp + o, oA);
+                if (f.phase) store_vec<float, V>(f.phase + o, oP);
+            }
+          }
         }
     }
 }
@@ -410,7 +464,7 @@ int red_bytes_for(int seg, int vb, int rows, int v, bool is_int, int nw, int nep
 template <typename T, typename ACC, int ROWS, int NWT, int NEPI>
 cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
 {
-    constexpr int V = pick_v(sizeof(T), ROWS);
+    constexpr int V = stream_v(sizeof(T), ROWS);
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
     const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT, NWT, NEPI));
     auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI>;
@@ -450,7 +504,7 @@ StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const 
 {
     StreamShape sh = {0, 0, 0};
     const int bytes = dtype == QLD_U8 ? 1 : 2;
-    const int v = pick_v(bytes, rows), vb = v * bytes;
+    const int v = stream_v(bytes, rows), vb = v * bytes;
     const int64_t row_bytes = HW * bytes;
     if (row_bytes % 16 != 0 || (reinterpret_cast<uintptr_t>(frames) & 15) != 0) return sh;
     const int nw = NW;
