@@ -44,8 +44,12 @@ constexpr int NW = 8;                 // consumer warps
 #endif
 constexpr int stream_v(int bytes, int rows)
 {
-    const int v = qld_dev::pick_v(bytes, rows), cap = QLD_STREAM_VB / bytes;
-    return v < cap ? v : cap;
+    int v = qld_dev::pick_v(bytes, rows);
+    const int cap = QLD_STREAM_VB / bytes;
+    if (v > cap) v = cap;
+    // prefer 32 accumulators (128 registers, room for the epilogue warps) as long as a thread keeps 8 bytes per frame
+    while (rows * v > 32 && v * bytes > 8) v /= 2;
+    return v;
 }
 constexpr bool stream_light(int bytes, int rows) { return rows * stream_v(bytes, rows) <= 32; }
 // four epilogue warps for the variants whose frame loop fits in 128 registers (13 warps per CTA)
@@ -510,8 +514,10 @@ StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const 
     const int nw = NW;
     int seg = 2048;                                        // TMA box: at most 256 8-byte elements per row
     if (seg > nw * 32 * vb) seg = nw * 32 * vb;
-    while (seg > 32 * vb && (row_bytes + seg - 1) / seg < 4 * (int64_t)n_sms) seg /= 2;
-    int kc = 16, stages = 0;
+    // small frames: at least two tiles per SM, but segments as wide as that allows (cfg1 sweep: 1 KB x 32 frames
+    // 41 us, 512 B x 32 frames 47 us: narrow rows cost more per byte and need more time slices to combine)
+    while (seg > 32 * vb && (row_bytes + seg - 1) / seg < 2 * (int64_t)n_sms) seg /= 2;
+    int kc = 32768 / seg > 16 ? 32768 / seg : 16, stages = 0;      // stages of at least 32 KB
     bool forced = false;
     if (const char *e = getenv("QLD_STREAM_TILE")) {      // tuning / test override: "SEG,KC" (also lifts the size threshold)
         int s2 = 0, k2 = 0;
