@@ -334,10 +334,12 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     for a in range(0, T, 256):
         qld.synth_fill(sc, a + 1, min(256, T - a), out=ring[a:a + 256])
     torch.cuda.synchronize()
-    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=maps, max_value=sc.maxval, external_store=True)
+    slide_hop = hop if args.block_partials else 0
+    ctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=maps, max_value=sc.maxval, external_store=True,
+                  slide_hop=slide_hop)
     ctx.attach_frames_device(ring)
     ctx.commit_frames(N)
-    ctx.demod(qld.QLD_SLIDE, hop)                            # window 0: whole-window kernel seeds the accumulators
+    ctx.demod(qld.QLD_SLIDE, hop)                            # window 0 seeds the accumulators (and the partial sums)
     ctx.sync()
     seed_kernel = ctx.last_kernel()
 
@@ -356,12 +358,18 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
            "window_samples_per_s": env.world * float(N) * H * W * steps / (ms * 1e-3)}
     # per pixel: hop new + hop expired samples, accumulators read-modify-write, one amplitude map
     algo = H * W * (2.0 * hop * b + 2.0 * n_rows * acc_bytes + 4.0 * K)
+    moved = H * W * (1.0 * hop * b + 4.0 * n_rows * acc_bytes + 4.0 * K) if slide_hop else algo
     res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
-                                   f"per pixel 2*hop*{b} B of frames + {n_rows} x {acc_bytes} B accumulators read and written + 4 B map; "
-                                   f"a recompute would read {N * b} B")
+                                   f"algorithmic bytes = SURVEY.md 8(a) A5: per pixel 2*hop*{b} B of frames (new + expired) + {n_rows} x {acc_bytes} B "
+                                   f"accumulators read and written + 4 B map; a recompute would read {N * b} B."
+                                   + (f" This run keeps per-batch partial sums (8(f3)) and reads only the new frames: it moves {moved / 1e6:.1f} MB "
+                                      f"per launch ({hop * b} B of frames + 2 x {n_rows} x {acc_bytes} B accumulators and partials read and written + 4 B), "
+                                      f"i.e. {moved / (ms / steps * 1e-3) / 1e9:.0f} GB/s of real traffic" if slide_hop else ""))
+    res["roofline"]["bytes_moved_per_launch"] = moved
     res["dtype"] = {"INT_BINS": "int32", "FP32": "f32"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "hop": hop, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": "amplitude", "step": "qld_commit_frames(hop) + qld_demod(QLD_SLIDE, hop) over the resident ring",
+                     "update": "block partial sums (cfg.slide_hop = hop): only the new frames are read" if slide_hop else "expired frames re-read",
                      "ring_frames": T, "seed_kernel": seed_kernel,
                      "cache": f"{2 * hop * H * W * b / 1e6:.0f} MB of frames per step, each read once > 126 MB L2: no flush needed"
                               if 2 * hop * H * W * b > 126e6 else f"{2 * hop * H * W * b / 1e6:.0f} MB of frames per step; new frames were "
@@ -376,7 +384,8 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
         n_win = 4
         rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (n_win * K * N * W))))
         r0 = H // 2 - rows // 2                               # the moving disk crosses these rows
-        pctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval, external_store=True)
+        pctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval, external_store=True,
+                       slide_hop=slide_hop)
         pctx.attach_frames_device(ring)
         pctx.commit_frames(N)
         pctx.demod(qld.QLD_SLIDE, hop)
@@ -416,7 +425,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
         for i in range(n_rot):
             host[i].copy_(qld.synth_fill(sc, 1 + i * batch, batch, device=env.dev))
         amp_host = torch.empty((2, K, H, W), dtype=torch.float32).pin_memory()
-        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=N + hop + 2 * batch, accum=accum, maps=maps, max_value=sc.maxval)
+        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=N + hop + 2 * batch, accum=accum, maps=maps, max_value=sc.maxval, slide_hop=slide_hop)
         for i in range(N // batch):
             ectx.push_frames(host[i % n_rot])
         ectx.demod(qld.QLD_SLIDE, hop)
@@ -467,6 +476,8 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=0, help="rows of the frame the CPU oracle is timed / checked on "
                     "(0: sized for about 15 s of oracle work on the host cores; 32 for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--block-partials", action="store_true", help="cfg3: keep per-batch partial sums (SURVEY.md 8(f3), cfg.slide_hop) "
+                    "instead of re-reading the expired frames (8(a) A5 as stated, the default: it is the faster one on B200)")
     ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly and report under "
                     "\"also\" (default: cfg4,cfg3,cfg1 when --workload is cfg2 on one GPU; 'none' to skip)")
     args = ap.parse_args()

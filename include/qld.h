@@ -104,6 +104,15 @@ typedef struct {
     int32_t external_store;  /* 1: the frame store (N frames, or ring_frames frames) is the caller's device buffer, given
                                 with qld_attach_frames_device; frames arrive in place and are announced with
                                 qld_commit_frames (zero-copy ingest).  ring_frames = -1 implies it. */
+    int32_t slide_hop;       /* > 0 (ring contexts): block-partial sliding (P:181-183 with a constant hop): the context keeps
+                                the N/slide_hop per-batch partial sums of the window (N/slide_hop x rows x H*W accumulators)
+                                and a QLD_SLIDE update reads only the slide_hop NEW frames: the expired batch's partial is
+                                taken off instead of re-reading its frames.  Needs N % slide_hop == 0, every
+                                qld_demod(QLD_SLIDE, hop) with hop == slide_hop, and frames the TMA kernel accepts
+                                (H*W*bytes a multiple of 16, at least one 2 KB segment per SM, slide_hop >= 16..64
+                                depending on the frame size): QLD_E_UNSUPPORTED otherwise.  Results are identical to the
+                                frame re-reading update (bit-exact for INT_BINS). */
+    int32_t reserved2;
     void *workspace;         /* device memory of qld_workspace_bytes() bytes, 256-byte aligned, owned by the
                                 caller (e.g. a torch tensor) and kept alive until qld_destroy; NULL: the
                                 library allocates and frees it */

@@ -60,6 +60,8 @@ struct qld_ctx {
     double *cum;
     void *acc;
     float *ped;
+    unsigned char *part;     // block-partial sliding: [M][rows_pad][HW] partial sums (int32 / double)
+    int slide_hop, n_part;   // hop of the partial mode (0: off), M = N / hop
     float *mapI, *mapQ, *mapA, *mapP;
     // streams and events
     cudaStream_t s_comp, s_copy;
@@ -137,6 +139,8 @@ struct Plan {
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
     // workspace offsets
+    int slide_hop;
+    size_t off_part;
     size_t off_frames, off_wtab, off_cum, off_acc, off_ped, off_I, off_Q, off_A, off_P, off_rfix, off_digits, off_sums, off_counter, total;
 };
 
@@ -152,6 +156,8 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         return bad(QLD_E_INVAL, "ring_frames must be -1, 0, or > N");
     if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_FIXED) return bad(QLD_E_INVAL, "unknown accum");
     if (cfg->external_store != 0 && cfg->external_store != 1) return bad(QLD_E_INVAL, "external_store must be 0 or 1");
+    if (cfg->slide_hop < 0 || cfg->slide_hop > cfg->N) return bad(QLD_E_INVAL, "slide_hop must be 0..N");
+    if (cfg->slide_hop > 0 && cfg->ring_frames <= 0) return bad(QLD_E_INVAL, "slide_hop needs a ring context");
     if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
     if (cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64)) return bad(QLD_E_INVAL, "unknown bits in maps");
     memset(pl, 0, sizeof *pl);
@@ -259,6 +265,13 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     pl->off_cum = o; if (cc) o += align_up((size_t)pl->cap_w * pl->rows_pad * 8);
     pl->off_acc = o; if (cc && (pl->ring || pl->is_int)) o += align_up((size_t)pl->rows_pad * pl->HW * (pl->is_int ? 4 : 8));
     pl->off_ped = o; if (cc && pl->ring) o += align_up((size_t)pl->HW * 4);
+    pl->slide_hop = cfg->slide_hop;
+    pl->off_part = o;
+    if (cfg->slide_hop > 0) {
+        if (cfg->N % cfg->slide_hop != 0) return bad(QLD_E_UNSUPPORTED, "slide_hop must divide N");
+        if ((pl->HW * pl->bytes) % 16 != 0) return bad(QLD_E_UNSUPPORTED, "slide_hop: H*W*bytes_per_sample must be a multiple of 16");
+        o += align_up((size_t)(cfg->N / cfg->slide_hop) * pl->rows_pad * pl->HW * (pl->is_int ? 4 : 8));
+    }
     const size_t map = align_up((size_t)pl->K * pl->HW * 4);
     pl->off_I = o; if (pl->maps & QLD_MAP_I) o += map;
     pl->off_Q = o; if (pl->maps & QLD_MAP_Q) o += map;
@@ -448,9 +461,57 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     return record_demod(c, a + 1);
 }
 
+// Block-partial mode (8(f3)): one launch over the frames of batch b of the window that starts at offset a.
+// sub = false: seeding (the slot is only written); sub = true: a sliding update (the slot's old content is the
+// expired batch: taken off the accumulators, then overwritten).
+int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool add, bool sub, bool first_of_seed)
+{
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
+    DemodParams p;
+    memset(&p, 0, sizeof p);
+    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+    p.cap = c->cap; p.cap_w = c->cap_w;
+    p.cum_lo = (int)(a_win % c->cap_w); p.cum_hi = (int)((a_win + c->N) % c->cap_w);
+    p.wtab = c->wtab; p.cum = c->cum;
+    p.acc_out = c->acc; p.acc_add = add ? 1 : 0;
+    p.onehot = c->is_int && c->K == 1;
+    p.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
+    p.part_sub = sub ? 1 : 0;
+    if (!c->is_int) {
+        if (first_of_seed) p.ped_out = c->ped; else p.ped_in = c->ped;
+    }
+    p.fin = fin_with_maps(c);
+    p.n_runs = add_runs(c, p.run, 0, first, c->slide_hop, +1);
+    int rc = stream_tmap_for(c, sh);
+    if (rc) return rc;
+    CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+    c->launches++;
+    c->last_kernel = "k_demod_stream";
+    return QLD_OK;
+}
+
+// window a+1 .. a+N from scratch: the sums, and (block-partial mode) the N/hop per-batch partials
+int seed_window(qld_ctx *c, int64_t a)
+{
+    if (c->slide_hop == 0) return run_whole(c, a, true);
+    for (int b = 0; b < c->n_part; ++b) {
+        int rc = run_partial_batch(c, a, a + (int64_t)b * c->slide_hop, b, b > 0, false, b == 0);
+        if (rc) return rc;
+    }
+    return record_demod(c, a + 1);
+}
+
 int run_slide(qld_ctx *c, int64_t a_old, int hop)
 {
     const int64_t a_new = a_old + hop;
+    if (c->slide_hop > 0) {
+        // the expired batch and the new one share a slot: batch j of the seeded window lives in slot j mod M
+        const int slot = (int)(c->hops_since_seed % c->n_part);
+        int rc = run_partial_batch(c, a_new, a_old + c->N, slot, true, true, false);
+        if (rc) return rc;
+        return record_demod(c, a_old + 1);                    // conservative: the whole window stays protected from overwriting
+    }
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
     if (sh.seg > 0 && hop >= sh.kc) {
@@ -545,6 +606,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     c->frames = pl.external ? nullptr : b + pl.off_frames;
     c->wtab = b + pl.off_wtab; c->cum = reinterpret_cast<double *>(b + pl.off_cum);
     c->acc = b + pl.off_acc; c->ped = reinterpret_cast<float *>(b + pl.off_ped);
+    c->part = b + pl.off_part; c->slide_hop = pl.slide_hop; c->n_part = pl.slide_hop > 0 ? pl.N / pl.slide_hop : 0;
     c->mapI = (pl.maps & QLD_MAP_I) ? reinterpret_cast<float *>(b + pl.off_I) : nullptr;
     c->mapQ = (pl.maps & QLD_MAP_Q) ? reinterpret_cast<float *>(b + pl.off_Q) : nullptr;
     c->mapA = (pl.maps & QLD_MAP_AMP) ? reinterpret_cast<float *>(b + pl.off_A) : nullptr;
@@ -646,7 +708,7 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (mode == QLD_WHOLE) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames stored");
         const int64_t a = c->ring ? c->pushed - c->N : 0;
-        int rc = run_whole(c, a, c->ring);
+        int rc = c->ring ? seed_window(c, a) : run_whole(c, a, false);
         if (rc) return rc;
         if (c->ring) { c->seeded = true; c->win_start = a; c->hops_since_seed = 0; }
         c->windows_done++;
@@ -655,16 +717,17 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (!c->ring) return fail(c, QLD_E_STATE, "demod: QLD_SLIDE needs a ring context (ring_frames > N)");
     if (!c->seeded) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames pushed");
-        int rc = run_whole(c, 0, true);
+        int rc = seed_window(c, 0);
         if (rc) return rc;
         c->seeded = true; c->win_start = 0; c->hops_since_seed = 0; c->windows_done++;
         return QLD_OK;
     }
     if (hop < 1 || hop > c->N) return fail(c, QLD_E_INVAL, "demod: hop must be 1..N");
+    if (c->slide_hop > 0 && hop != c->slide_hop) return fail(c, QLD_E_INVAL, "demod: this context slides by cfg.slide_hop only");
     if (c->pushed < c->win_start + hop + c->N) return fail(c, QLD_E_STATE, "demod: fewer than hop new frames pushed");
     int rc;
     if (!c->is_int && c->resync_hops > 0 && c->hops_since_seed + 1 >= c->resync_hops) {
-        rc = run_whole(c, c->win_start + hop, true);
+        rc = seed_window(c, c->win_start + hop);
         c->hops_since_seed = 0;
     } else {
         rc = run_slide(c, c->win_start, hop);

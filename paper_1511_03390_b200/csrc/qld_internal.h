@@ -61,6 +61,9 @@ struct DemodParams {
     int32_t onehot;          // integer bins, one reference: every weight row is one-hot (+-1 in one row)
     int32_t acc_add;         // 1: acc_out holds the previous window's sums; this launch's sums are added to them
     DemodRun run[4];
+    void *part;              // block-partial sliding (8(f3)): [ROWS][HW] slot of the partial-sum ring; this launch's sums are
+                             // stored there, after the slot's previous content was taken off acc_out when part_sub is set
+    int32_t part_sub, reserved;
     const float *ped_in;     // FP32: pedestal to subtract (the one acc_out was seeded with); NULL: the first sample
     FinParams fin;
 };

@@ -69,7 +69,9 @@ struct StreamSmem {
     }
 };
 
-template <typename T, typename ACC, int ROWS, int V, int NWT, int NEPI>
+// PART: block-partial sliding (8(f3)): the launch's sums are also stored in p.part (after the slot's old content was
+// taken off the stored sums when p.part_sub is set)
+template <typename T, typename ACC, int ROWS, int V, int NWT, int NEPI, bool PART>
 __global__ void __launch_bounds__(32 * (NWT + 1 + NEPI), 1)
 k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ DemodParams p, const StreamShape sh, unsigned int *tile_counter)
 {
@@ -182,7 +184,12 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
             const int q = q0 + i * qstride;
             const bool ok = q < TP && tile_pix0 + q < p.HW;
 #pragma unroll
-            for (int r = 0; r < ROWS; ++r) pf[i][r] = ok ? accg[(int64_t)r * p.HW + tile_pix0 + q] : (RED)0;
+            for (int r = 0; r < ROWS; ++r) {
+                pf[i][r] = ok ? accg[(int64_t)r * p.HW + tile_pix0 + q] : (RED)0;
+                if constexpr (PART) {
+                    if (p.part_sub && ok) pf[i][r] -= static_cast<const RED *>(p.part)[(int64_t)r * p.HW + tile_pix0 + q];
+                }
+            }
         }
     };
     auto finalise_tile = [&](const RED *redb, int tile, int q0, int qstride, const RED (&pf)[PFN][ROWS], bool use_pf) {
@@ -203,7 +210,13 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
                 a.a[r] = redb[(size_t)(r * V + v) * RS + tc];
-                if (p.acc_add) a.a[r] += prev ? prev[r] : accg[(int64_t)r * p.HW + pixel];
+                RED old = 0;
+                if constexpr (PART) {                      // 8(f3): this launch's sums replace the expired batch's
+                    RED *partg = static_cast<RED *>(p.part);
+                    if (p.part_sub && !prev) old = partg[(int64_t)r * p.HW + pixel];
+                    partg[(int64_t)r * p.HW + pixel] = a.a[r];
+                }
+                if (p.acc_add) a.a[r] += prev ? prev[r] : accg[(int64_t)r * p.HW + pixel] - old;
                 if (accg) accg[(int64_t)r * p.HW + pixel] = a.a[r];
             }
             if constexpr (!IS_INT) {
@@ -299,7 +312,15 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
             if (own_prev) {
                 const RED *accg = static_cast<const RED *>(p.acc_out);
 #pragma unroll
-                for (int r = 0; r < ROWS; ++r) load_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, prev[r]);
+                for (int r = 0; r < ROWS; ++r) {
+                    load_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, prev[r]);
+                    if (PART && p.part_sub) {
+                        RED old[V];
+                        load_vec<RED, V>(static_cast<const RED *>(p.part) + (int64_t)r * p.HW + pix0, old);
+#pragma unroll
+                        for (int v = 0; v < V; ++v) prev[r][v] -= old[v];
+                    }
+                }
             }
         }
 
@@ -402,7 +423,10 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
 #pragma unroll
-                for (int v = 0; v < V; ++v) a[r][v] = (RED)acc[r][v] + (own_prev ? prev[r][v] : (RED)0);
+                for (int v = 0; v < V; ++v) a[r][v] = (RED)acc[r][v];
+                if constexpr (PART) store_vec<RED, V>(static_cast<RED *>(p.part) + (int64_t)r * p.HW + pix0, a[r]);
+#pragma unroll
+                for (int v = 0; v < V; ++v) a[r][v] += (own_prev ? prev[r][v] : (RED)0);
                 if (accg) store_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, a[r]);
             }
             float pedf[V];
@@ -465,13 +489,13 @@ int red_bytes_for(int seg, int vb, int rows, int v, bool is_int, int nw, int nep
     return ts > 1 ? (nepi > 0 ? 2 : 1) * (rows + (is_int ? 0 : 1)) * v * (cg * 32 + pad) * esz : 0;
 }
 
-template <typename T, typename ACC, int ROWS, int NWT, int NEPI>
+template <typename T, typename ACC, int ROWS, int NWT, int NEPI, bool PART>
 cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
 {
     constexpr int V = stream_v(sizeof(T), ROWS);
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
     const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT, NWT, NEPI));
-    auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI>;
+    auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI, PART>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
     if (e != cudaSuccess) return e;
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
@@ -485,7 +509,8 @@ cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const Stream
 template <typename T, typename ACC, int ROWS>
 cudaError_t launch_stream_t(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
 {
-    return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS)>(tmap, p, sh, counter, n_sms, st);
+    if (p.part) return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), true>(tmap, p, sh, counter, n_sms, st);
+    return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), false>(tmap, p, sh, counter, n_sms, st);
 }
 
 template <typename T, typename ACC>

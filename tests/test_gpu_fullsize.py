@@ -77,8 +77,9 @@ def test_whole_window_full_size_sampled(Q, oracle, name, accum_name, kernel):
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("slide_hop", [0, 32])
 @pytest.mark.parametrize("accum_name", ["AUTO", "FP32"])
-def test_sliding_full_size_sampled(Q, oracle, accum_name):
+def test_sliding_full_size_sampled(Q, oracle, accum_name, slide_hop):
     """cfg3's frame size, window, hop and batch; the first 12 hops of the stream, zero-copy ring as in bench.py."""
     import torch
     from paper_1511_03390_b200 import synth
@@ -91,7 +92,7 @@ def test_sliding_full_size_sampled(Q, oracle, accum_name):
     for a in range(0, T, 128):
         Q.synth_fill(sc, a + 1, min(128, T - a), out=ring[a:a + 128])
     ctx = Q.QLD(sc.H, sc.W, sc.dtype, N, [ref], ring_frames=T, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=sc.maxval,
-                external_store=True)
+                external_store=True, slide_hop=slide_hop)
     ctx.attach_frames_device(ring)
     ctx.commit_frames(N)
     ctx.demod(Q.QLD_SLIDE, hop)

@@ -420,6 +420,55 @@ def test_stream_kernel_sliding_update(Q, oracle, monkeypatch, tile, accum_name, 
     ctx.destroy()
 
 
+@pytest.mark.parametrize("tile", ["512,16", "2048,16", "1024,32"])
+@pytest.mark.parametrize("accum_name,ref", [("INT_BINS", {"num": 1, "den": 6}), ("FP32", {"nu": 0.0937, "phase": 0.3}), ("INT_BINS", {"num": 3, "den": 8})])
+@pytest.mark.parametrize("hop,cap", [(32, 170), (64, 200)])
+def test_block_partial_sliding(Q, oracle, monkeypatch, tile, accum_name, ref, hop, cap):
+    """8(f3): slide_hop > 0 keeps the per-batch partial sums and reads only the new frames; every window equals the
+    oracle's direct recomputation (bins bit-exact), through ring wrap-around and more hops than partial slots."""
+    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    rng = np.random.default_rng(hop + cap)
+    H, W, N, T = 12, 128, 128, 128 + 9 * hop
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095, slide_hop=hop,
+                resync_hops=5 if accum_name == "FP32" else 0)
+    ctx.push_frames(stream[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.demod(Q.QLD_SLIDE, hop // 2)                        # only the configured hop
+    assert e.value.status == Q.QLD_E_INVAL
+    for w in range(0, (T - N) // hop + 1):
+        if w > 0:
+            ctx.push_frames(stream[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+        ctx.sync()
+        a = w * hop
+        ora = oracle_maps(oracle, stream[a:a + N], ref, s_first=a + 1)
+        if accum_name == "INT_BINS":
+            den, num = ref["den"], ref["num"]
+            B = oracle.bins(stream[a:a + N], num, den, s_first=a + 1)
+            assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:den // 2] - B[den // 2:]), f"window {w}"
+            check_float_maps(_maps(ctx), ora, rel=1e-6, what=f"window {w}")
+        else:
+            check_float_maps(_maps(ctx), ora, what=f"window {w}")
+    ctx.destroy()
+
+
+def test_block_partial_sliding_rejects_what_it_cannot_do(Q):
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(12, 128, "u16", 100, [{"num": 1, "den": 6}], ring_frames=200, slide_hop=32)       # hop does not divide N
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(12, 128, "u16", 128, [{"num": 1, "den": 6}], slide_hop=32)                        # not a ring
+    assert e.value.status == Q.QLD_E_INVAL
+    ctx = Q.QLD(12, 128, "u16", 128, [{"num": 1, "den": 6}], ring_frames=200, slide_hop=32)      # a frame too small for the TMA kernel
+    ctx.push_frames(np.zeros((128, 12, 128), np.uint16))
+    with pytest.raises(Q.QLDError) as e:
+        ctx.demod(Q.QLD_SLIDE, 32)
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
+    ctx.destroy()
+
+
 # ------------------------------------------------------------------------------------------------ A2 zero-copy ingest
 @pytest.mark.parametrize("accum_name", ["INT_BINS", "FP32"])
 def test_commit_frames_into_attached_ring(Q, oracle, accum_name):
