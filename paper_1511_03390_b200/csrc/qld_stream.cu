@@ -224,7 +224,75 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
             }
             finalise_pixel_nl<ROWS, IS_INT, RED>(&p.fin, a, ped, wsum, pixel, p.HW);   // sum x w = sum (x - ped) w + ped * sum w
         };
-        if (use_pf) {
+        if (use_pf && p.fin.K == 1) {
+            // one reference, stored sums prefetched: the pixels of a thread go through the fp64 arithmetic in batches of
+            // four with no branch between them (independent dependency chains interleave), stores predicated at the end
+            constexpr int B = PFN < 4 ? PFN : 4;
+            const FinParams &f = p.fin;
+            RED *accg = static_cast<RED *>(p.acc_out);
+#pragma unroll
+            for (int i0 = 0; i0 < PFN; i0 += B) {
+                RED a[B][ROWS];
+                double S[B], C[B], pedv[B];
+                bool ok[B];
+                int64_t pix[B];
+#pragma unroll
+                for (int j = 0; j < B; ++j) {
+                    const int q = q0 + (i0 + j) * qstride;
+                    ok[j] = q < TP && tile_pix0 + q < p.HW;
+                    const int qq = ok[j] ? q : q0;
+                    pix[j] = tile_pix0 + qq;
+                    const int v = qq % V, tc = qq / V;
+                    pedv[j] = 0.0;
+                    if constexpr (!IS_INT) pedv[j] = redb[(size_t)(ROWS * V + v) * RS + tc];
+#pragma unroll
+                    for (int r = 0; r < ROWS; ++r) {
+                        a[j][r] = redb[(size_t)(r * V + v) * RS + tc];
+                        if constexpr (PART) {
+                            if (ok[j]) static_cast<RED *>(p.part)[(int64_t)r * p.HW + pix[j]] = a[j][r];
+                        }
+                        if (p.acc_add) a[j][r] += pf[i0 + j][r];
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < B; ++j) {
+                    if constexpr (IS_INT) {
+                        S[j] = 0.0; C[j] = 0.0;
+#pragma unroll
+                        for (int r = 0; r < ROWS; ++r) {
+                            const double x = (double)a[j][r];
+                            S[j] = fma(x, f.sw[r], S[j]);
+                            C[j] = fma(x, f.cw[r], C[j]);
+                        }
+                    } else {
+                        S[j] = (double)a[j][0] + pedv[j] * wsum.a[0];       // sum x w = sum (x - ped) w + ped * sum w
+                        C[j] = (double)a[j][1] + pedv[j] * wsum.a[1];
+                    }
+                    S[j] *= f.scale;
+                    C[j] *= f.scale;
+                }
+                float amp[B], ph[B];
+#pragma unroll
+                for (int j = 0; j < B; ++j) amp[j] = f.amp ? (float)sqrt(S[j] * S[j] + C[j] * C[j]) : 0.0f;
+#pragma unroll
+                for (int j = 0; j < B; ++j) ph[j] = (f.phase && !(S[j] == 0.0 && C[j] == 0.0)) ? (float)atan2(C[j], S[j]) : 0.0f;
+#pragma unroll
+                for (int j = 0; j < B; ++j) {
+                    if (!ok[j]) continue;
+                    if (accg) {
+#pragma unroll
+                        for (int r = 0; r < ROWS; ++r) accg[(int64_t)r * p.HW + pix[j]] = a[j][r];
+                    }
+                    if constexpr (!IS_INT) {
+                        if (p.ped_out) p.ped_out[pix[j]] = (float)pedv[j];
+                    }
+                    if (f.I) f.I[pix[j]] = (float)S[j];
+                    if (f.Q) f.Q[pix[j]] = (float)C[j];
+                    if (f.amp) f.amp[pix[j]] = amp[j];
+                    if (f.phase) f.phase[pix[j]] = ph[j];
+                }
+            }
+        } else if (use_pf) {
 #pragma unroll
             for (int i = 0; i < PFN; ++i) {
                 const int q = q0 + i * qstride;
@@ -242,7 +310,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
         // ===== epilogue warps: finalise tile i from red[i & 1] while the consumers run the frame loop of tile i + 1 =====
         if (!SPLIT) return;
         const int et = (warp - 1 - NWT) * 32 + lane;
-        const bool use_pf = p.acc_add && TP <= PFN * NEPI * 32;
+        const bool use_pf = TP <= PFN * NEPI * 32;          // every pixel of the tile has a register slot
         for (int it = 0;; ++it) {
             const int buf = it & 1;
             const uint32_t par = (uint32_t)(it >> 1) & 1u;
@@ -250,7 +318,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
             const int tile = tile_q[it & (TQ - 1)];
             if (tile < 0) break;
             RED pf[PFN][ROWS];
-            if (use_pf) prefetch_acc(tile, et, NEPI * 32, pf);
+            if (use_pf && p.acc_add) prefetch_acc(tile, et, NEPI * 32, pf);
             mbar_wait(&red_full[buf], par);
             finalise_tile(red + (size_t)buf * red_cells, tile, et, NEPI * 32, pf, use_pf);
             mbar_arrive(&red_empty[buf]);
@@ -300,8 +368,8 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
 
         // without epilogue warps the consumers finalise: request the stored sums now, under the frame loop
         RED pf[PFN][ROWS];
-        const bool use_pf = !SPLIT && p.acc_add && TS > 1 && TP <= PFN * NWT * 32;
-        if (use_pf) prefetch_acc(tile, cw * 32 + lane, NWT * 32, pf);
+        const bool use_pf = !SPLIT && TS > 1 && TP <= PFN * NWT * 32;
+        if (use_pf && p.acc_add) prefetch_acc(tile, cw * 32 + lane, NWT * 32, pf);
 
         // one slice per column group: the thread finalises its own V pixels; their stored sums (A5) are requested now
         // (a 2 KB segment has eight column groups only when a thread takes at most 8 bytes per frame)
