@@ -51,8 +51,9 @@ struct Pix {
     // sample j as an unsigned integer
     __device__ __forceinline__ static uint32_t geti(const uint32_t (&w)[NW], int j)
     {
-        if constexpr (sizeof(T) == 2) return (j & 1) ? (w[j >> 1] >> 16) : (w[j >> 1] & 0xffffu);
-        else return (w[j >> 2] >> (8 * (j & 3))) & 0xffu;
+        // one byte-permute (selector nibble 4 = a zero byte of the second operand)
+        if constexpr (sizeof(T) == 2) return __byte_perm(w[j >> 1], 0u, (j & 1) ? 0x4432u : 0x4410u);
+        else return __byte_perm(w[j >> 2], 0u, 0x4440u | (uint32_t)(j & 3));
     }
     // sample j as the float 2^23 + x (one byte-permute: the integer lands in the mantissa of 0x4B000000)
     __device__ __forceinline__ static float getf_biased(const uint32_t (&w)[NW], int j)
