@@ -129,11 +129,14 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
         const ACC *wtab = static_cast<const ACC *>(p.wtab);
         int stage = 0, it = 0;
         uint32_t phase = 0;
+        // the first tile of a CTA is its block index (no round trip before the first copy); later ones come from the
+        // global counter, claimed one tile ahead so that the atomic's latency hides under the current tile's copies
+        int next = (int)blockIdx.x;
         for (;; ++it) {
             int tile = 0;
             if (lane == 0) {
-                tile = (int)atomicAdd(tile_counter, 1u);
-                if (tile >= n_tiles) tile = -1;
+                tile = next < n_tiles ? next : -1;
+                if (tile >= 0) next = (int)gridDim.x + (int)atomicAdd(tile_counter, 1u);
                 tile_q[it & (TQ - 1)] = tile;            // published by the arrivals on full[stage] below
             }
             tile = __shfl_sync(0xffffffffu, tile, 0);
