@@ -200,3 +200,28 @@ def cnr(image: np.ndarray, y0: int, x0: int, m: int):
     with np.errstate(divide="ignore", invalid="ignore"):
         ratio = np.float64(mean_s - mean_surr) / np.float64(rms)
     return float(ratio), float(mean_s), float(mean_surr), float(rms)
+
+
+# ---------------------------------------------------------------------------------------------------
+# Unknown-frequency search -- SURVEY.md 8(f2), the step before the path
+# ---------------------------------------------------------------------------------------------------
+def bin_amplitudes(frames: np.ndarray, q_lo: int, q_hi: int, nthreads: int = 1) -> np.ndarray:
+    """R_q for every DFT bin q = q_lo..q_hi of the N-frame stack: one QLD per bin at nu = q/N ("a series
+    of QLDs ... at different frequencies"), each from the definition.  Returns [q_hi - q_lo + 1, ...pixels] float64."""
+    N = frames.shape[0]
+    if q_lo < 1 or q_hi < q_lo or 2 * q_hi >= N:
+        raise ValueError("bins must satisfy 1 <= q_lo <= q_hi < N/2")
+    return np.stack([qld(frames, {"num": q, "den": N}, nthreads=nthreads)[2] for q in range(q_lo, q_hi + 1)])
+
+
+def dominant_bin(frames: np.ndarray, q_lo: int, q_hi: int, nthreads: int = 1):
+    """Per pixel: the largest R_q over the bins and its bin (the lowest bin on a tie).  Also returns the runner-up
+    amplitude so that a caller can tell near-ties (where another bin is an equally valid answer)."""
+    A = bin_amplitudes(frames, q_lo, q_hi, nthreads)
+    idx = np.argmax(A, axis=0)
+    best = np.take_along_axis(A, idx[None], axis=0)[0]
+    if A.shape[0] > 1:
+        second = np.partition(A, -2, axis=0)[-2]
+    else:
+        second = np.zeros_like(best)
+    return best, (idx + q_lo).astype(np.int32), second

@@ -27,7 +27,7 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
            "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
            "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel",
-           "qld_cnr", "qld_synth_fill"]
+           "qld_cnr", "qld_dominant_bin", "qld_synth_fill"]
 
 
 class qld_ref(C.Structure):
@@ -100,6 +100,7 @@ def load_library():
     l.qld_last_kernel.argtypes = [vp]
     l.qld_last_kernel.restype = C.c_char_p
     l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
+    l.qld_dominant_bin.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
     l.qld_synth_fill.argtypes = [C.POINTER(qld_synth_scene), i64, i, vp, vp]
     _lib = l
     return l
@@ -306,6 +307,23 @@ def cnr(image, y0: int, x0: int, m: int):
     if rc != QLD_OK:
         raise QLDError(rc, "qld_cnr")
     return out
+
+
+def dominant_bin(frames, q_lo: int, q_hi: int):
+    """qld_dominant_bin on a CUDA stack [N, H, W] (uint8 / uint16 / int16 view): returns (amp_max [H, W] float32,
+    bin [H, W] int32) -- the largest amplitude over the DFT bins q_lo..q_hi and where it sits."""
+    import torch
+    lib = load_library()
+    assert frames.is_cuda and frames.is_contiguous() and frames.dim() == 3
+    N, H, W = (int(x) for x in frames.shape)
+    dtype = QLD_U8 if frames.element_size() == 1 else QLD_U16
+    amp = torch.empty((H, W), dtype=torch.float32, device=frames.device)
+    bins = torch.empty((H, W), dtype=torch.int32, device=frames.device)
+    rc = lib.qld_dominant_bin(frames.data_ptr(), dtype, H, W, N, int(q_lo), int(q_hi), amp.data_ptr(), bins.data_ptr(),
+                              torch.cuda.current_stream(frames.device).cuda_stream or 1)
+    if rc != QLD_OK:
+        raise QLDError(rc, lib.qld_last_error(None).decode())
+    return amp, bins
 
 
 def synth_fill(scene, s_first: int, n_frames: int, out=None, device="cuda"):
