@@ -238,6 +238,13 @@ int qld_cnr(const float *map_device, int32_t H, int32_t W, int32_t y0, int32_t x
 int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_t H, int32_t W, int32_t N, int32_t q_lo, int32_t q_hi,
                      float *amp_max_device, int32_t *bin_device, void *stream);
 
+/* Display mapping (the processed 32-bit image "is displayed on the computer monitor"; there is no graphics stack
+ * here, the 8-bit image is delivered to device memory; reading G22): lo / hi = smallest / largest non-NaN value
+ * of the n floats at map_device, out_device[i] = rint(255 * (x_i - lo) / (hi - lo)) clamped to 0..255 (0 for NaN and
+ * for a flat map).  range_device (2 floats, may be NULL) receives {lo, hi}; scratch_device: 8 bytes of device memory.
+ * Three small launches enqueued on `stream` (cudaStream_t or NULL). */
+int qld_display_map(const float *map_device, int64_t n, uint8_t *out_device, float *range_device, void *scratch_device, void *stream);
+
 /* ---- synthetic input filler (not part of the method; device twin of paper_1511_03390_b200/synth.py) ---- */
 typedef struct {
     int32_t H, W;

@@ -225,3 +225,22 @@ def dominant_bin(frames: np.ndarray, q_lo: int, q_hi: int, nthreads: int = 1):
     else:
         second = np.zeros_like(best)
     return best, (idx + q_lo).astype(np.int32), second
+
+
+# ---------------------------------------------------------------------------------------------------
+# Display mapping -- SURVEY.md 8(f3), the step after the path; the paper does not say how the 32-bit
+# image is mapped to the screen: linear min-max to 8 bits is this build's reading (G22): "parity unpinned"
+# against the paper, pinned against the arithmetic below by closed forms.
+# ---------------------------------------------------------------------------------------------------
+def display_map(image: np.ndarray):
+    """u8 = rint(255 (x - lo) / (hi - lo)) with lo, hi the smallest / largest non-NaN value; zeros for a flat map and
+    for NaNs.  Returns (u8 image, lo, hi)."""
+    x = np.asarray(image, dtype=np.float64)
+    ok = ~np.isnan(x)
+    lo, hi = (float(x[ok].min()), float(x[ok].max())) if ok.any() else (np.inf, -np.inf)
+    out = np.zeros(x.shape, dtype=np.uint8)
+    if hi > lo:
+        with np.errstate(invalid="ignore"):
+            t = np.rint(255.0 * (x - lo) / (hi - lo))
+        out[ok] = np.clip(t[ok], 0, 255).astype(np.uint8)
+    return out, lo, hi

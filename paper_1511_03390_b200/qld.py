@@ -27,7 +27,7 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
            "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
            "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel",
-           "qld_cnr", "qld_dominant_bin", "qld_synth_fill"]
+           "qld_cnr", "qld_dominant_bin", "qld_display_map", "qld_synth_fill"]
 
 
 class qld_ref(C.Structure):
@@ -101,6 +101,7 @@ def load_library():
     l.qld_last_kernel.restype = C.c_char_p
     l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
     l.qld_dominant_bin.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
+    l.qld_display_map.argtypes = [vp, C.c_int64, vp, vp, vp, vp]
     l.qld_synth_fill.argtypes = [C.POINTER(qld_synth_scene), i64, i, vp, vp]
     _lib = l
     return l
@@ -307,6 +308,21 @@ def cnr(image, y0: int, x0: int, m: int):
     if rc != QLD_OK:
         raise QLDError(rc, "qld_cnr")
     return out
+
+
+def display_map(image):
+    """qld_display_map on a CUDA float32 map: returns (u8 image of the same shape, range tensor {lo, hi})."""
+    import torch
+    lib = load_library()
+    assert image.is_cuda and image.dtype == torch.float32 and image.is_contiguous()
+    out = torch.empty(image.shape, dtype=torch.uint8, device=image.device)
+    rng = torch.empty(2, dtype=torch.float32, device=image.device)
+    scratch = torch.empty(2, dtype=torch.int32, device=image.device)
+    rc = lib.qld_display_map(image.data_ptr(), int(image.numel()), out.data_ptr(), rng.data_ptr(), scratch.data_ptr(),
+                             torch.cuda.current_stream(image.device).cuda_stream or 1)
+    if rc != QLD_OK:
+        raise QLDError(rc, "qld_display_map")
+    return out, rng
 
 
 def dominant_bin(frames, q_lo: int, q_hi: int):
