@@ -7,6 +7,11 @@ express a sliding window and K references as repeated calls of the single-window
 (PAPER.md:181-183 "sliding sequence"; PAPER.md:49 "a series of QLDs ... at different frequencies").
 It shares nothing with paper_1511_03390_b200/csrc and does not import the binding.
 
+Beyond the hot path it also holds the oracles of the "next" rows: cnr / cnr_regions (Eq. (1),
+PAPER.md:101-109), bin_amplitudes / dominant_bin and display_map, in plain numpy.
+Parity unpinned (inputs or rule not given by the paper): the paper's CNR values 8.8 / 6.6 and the
+display mapping (PAPER.md:169 names none; G22); everything else is pinned in tests/test_oracle_*.py.
+
 Conventions: frame index s starts at 1; I = sum x sin
 (in-phase, the reference sinusoid, PAPER.md:31), Q = sum x cos (the 90-degree shifted one);
 amplitude R = sqrt(I^2 + Q^2) with no normalisation; phase = atan2(Q, I).
