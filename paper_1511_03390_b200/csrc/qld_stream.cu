@@ -377,9 +377,11 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
         // one slice per column group: the thread finalises its own V pixels; their stored sums (A5) are requested now
         // (a 2 KB segment has eight column groups only when a thread takes at most 8 bytes per frame)
         constexpr bool CAN_OWN = VB <= 8;
-        RED prev[CAN_OWN ? ROWS : 1][CAN_OWN ? V : 1];
+        // (prefetched only where that costs at most 32 registers; the 64-accumulator variants load them in the epilogue)
+        constexpr bool OWN_PF = CAN_OWN && ROWS * V * (int)sizeof(RED) <= 128;
+        RED prev[OWN_PF ? ROWS : 1][OWN_PF ? V : 1];
         const bool own_prev = CAN_OWN && TS == 1 && p.acc_add && active;
-        if constexpr (CAN_OWN) {
+        if constexpr (OWN_PF) {
             if (own_prev) {
                 const RED *accg = static_cast<const RED *>(p.acc_out);
 #pragma unroll
@@ -495,9 +497,26 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
             for (int r = 0; r < ROWS; ++r) {
 #pragma unroll
                 for (int v = 0; v < V; ++v) a[r][v] = (RED)acc[r][v];
-                if constexpr (PART) store_vec<RED, V>(static_cast<RED *>(p.part) + (int64_t)r * p.HW + pix0, a[r]);
+                if constexpr (PART) {
+                    RED *partg = static_cast<RED *>(p.part) + (int64_t)r * p.HW + pix0;
+                    RED old[V];
 #pragma unroll
-                for (int v = 0; v < V; ++v) a[r][v] += (own_prev ? prev[r][v] : (RED)0);
+                    for (int v = 0; v < V; ++v) old[v] = 0;
+                    if (!OWN_PF && p.part_sub) load_vec<RED, V>(partg, old);
+                    store_vec<RED, V>(partg, a[r]);
+#pragma unroll
+                    for (int v = 0; v < V; ++v) a[r][v] -= old[v];
+                }
+#pragma unroll
+                if constexpr (OWN_PF) {
+#pragma unroll
+                    for (int v = 0; v < V; ++v) a[r][v] += (own_prev ? prev[r][v] : (RED)0);
+                } else if (own_prev) {
+                    RED t[V];
+                    load_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, t);
+#pragma unroll
+                    for (int v = 0; v < V; ++v) a[r][v] += t[v];
+                }
                 if (accg) store_vec<RED, V>(accg + (int64_t)r * p.HW + pix0, a[r]);
             }
             float pedf[V];
