@@ -586,8 +586,18 @@ cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const Stream
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
     const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT, NWT, NEPI));
     auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI, PART>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
-    if (e != cudaSuccess) return e;
+    // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
+    // function, and re-setting it on every launch costs a driver call)
+    static int smem_set_dev[64] = {0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int &smem_set = smem_set_dev[dev & 63];
+    cudaError_t e = cudaSuccess;
+    if (SM.total + 128 > smem_set) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
+        if (e != cudaSuccess) return e;
+        smem_set = SM.total + 128;
+    }
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
     const int n_tiles = (int)((row_bytes + sh.seg - 1) / sh.seg);
     e = cudaMemsetAsync(counter, 0, sizeof(unsigned int), st);

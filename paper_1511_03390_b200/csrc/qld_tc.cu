@@ -376,8 +376,18 @@ cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cu
     const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms);
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
     auto kern = k_demod_tc<NC, BYTES>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 1024);
-    if (e != cudaSuccess) return e;
+    // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
+    // function, and re-setting it on every launch costs a driver call)
+    static int smem_set_dev[64] = {0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int &smem_set = smem_set_dev[dev & 63];
+    cudaError_t e = cudaSuccess;
+    if (SM.total + 1024 > smem_set) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 1024);
+        if (e != cudaSuccess) return e;
+        smem_set = SM.total + 1024;
+    }
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + sh.T - 1) / sh.T;
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
