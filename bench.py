@@ -300,6 +300,11 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
         out, secs = oracle_on_rows(wl, sub, refs, nt)
         res["cpu_baseline"] = {"value": float(sub.size) / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
                                "sample": f"rows {r0}..{r0 + rows - 1} x {W} cols x {N} frames x {K} refs = {sub.size} samples, {secs:.2f} s"}
+        # the paper's other CPU figure (one thread): the same oracle on one core, on a sixteenth of the rows
+        r1 = max(1, rows // 16)
+        _, secs1 = oracle_on_rows(wl, sub[:, :r1], refs, 1)
+        res["cpu_baseline"]["single_thread"] = {"value": float(sub[:, :r1].size) / secs1, "unit": UNIT, "cores": 1,
+                                                "sample": f"{r1} rows x {W} x {N} frames x {K} refs, {secs1:.2f} s"}
         ctx.demod(qld.QLD_WHOLE)
         ctx.sync()
         worst = 0.0
