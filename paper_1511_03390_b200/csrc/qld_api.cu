@@ -16,7 +16,6 @@ namespace {
 
 constexpr int N_PUSH_EVENTS = 64;
 constexpr int N_DEMOD_EVENTS = 32;
-constexpr double PI = 3.14159265358979323846;
 
 thread_local std::string g_create_error;
 
@@ -326,12 +325,10 @@ int init_device_state(qld_ctx *c)
 int wait_for_readers(qld_ctx *c, int64_t last_overwritten)
 {
     int best = -1;
-    int64_t best_age = -1;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) {
-        const int idx = (c->demod_ev_next + i) % N_DEMOD_EVENTS;   // oldest .. newest
-        if (c->demod_ev[idx].used && c->demod_ev[idx].oldest_read <= last_overwritten) { best = idx; best_age = i; }
+        const int idx = (c->demod_ev_next + i) % N_DEMOD_EVENTS;   // oldest .. newest: keep the newest reader
+        if (c->demod_ev[idx].used && c->demod_ev[idx].oldest_read <= last_overwritten) best = idx;
     }
-    (void)best_age;
     if (best >= 0) CU(c, cudaStreamWaitEvent(c->s_copy, c->demod_ev[best].ev, 0));
     return QLD_OK;
 }

@@ -507,7 +507,6 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
 #pragma unroll
                     for (int v = 0; v < V; ++v) a[r][v] -= old[v];
                 }
-#pragma unroll
                 if constexpr (OWN_PF) {
 #pragma unroll
                     for (int v = 0; v < V; ++v) a[r][v] += (own_prev ? prev[r][v] : (RED)0);
