@@ -51,3 +51,27 @@ def test_gaussian_surround_statistics(oracle):
     img[m:2 * m, m:2 * m] = rng.normal(11.0, 2.0, size=(m, m))
     c = oracle.cnr(img, m, m, m)[0]
     assert abs(c - 3.0) < 0.06
+
+
+def test_golden_fixture(oracle):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cnr_fig6.txt")
+    n = 0
+    for line in open(path):
+        f = line.split("#")[0].split()
+        if not f:
+            continue
+        if f[0] == "geom":
+            H, W, y0, x0, m, ns, nr = (int(v) for v in f[1:8])
+            src, ring = oracle.cnr_regions(H, W, y0, x0, m)
+            assert (src.sum(), ring.sum()) == (ns, nr) == (m * m, 8 * m * m)
+        else:
+            c, b, d, exp = (float(v) for v in f[1:5])
+            H, W, y0, x0, m = 20, 22, 6, 8, 4
+            src, ring = oracle.cnr_regions(H, W, y0, x0, m)
+            img = np.full((H, W), -7.0)
+            img[src] = c
+            img[ring] = np.where(np.arange(ring.sum()) % 2 == 0, b + d, b - d)
+            assert oracle.cnr(img, y0, x0, m)[0] == exp
+        n += 1
+    assert n == 6
