@@ -197,12 +197,16 @@ class Env:
 
 def load_traffic(workload: str, kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` summaries (profiles/traffic.json, written by hand from profiles/*.md); None if absent."""
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    `ncu --set full` summaries (profiles/r01_c_traffic.csv, copied from profiles/r01_c_ncu_full.md); None if absent."""
+    tpath = os.path.join(ROOT, "profiles", "r01_c_traffic.csv")
     try:
-        return json.load(open(tpath)).get(workload, {}).get(kernel)
+        for line in open(tpath).read().splitlines()[1:]:
+            w, k, v = line.split(",")
+            if w == workload and k == kernel:
+                return float(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def roofline_hbm(algo_bytes: float, ms_per_launch: float, workload: str, kernel: str, notes=None):
