@@ -254,7 +254,8 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         }
         pl->rows = 2 * cfg->K;
     }
-    pl->rows_pad = pl->rows <= 2 ? 2 : pl->rows <= 4 ? 4 : pl->rows <= 8 ? 8 : 16;
+    // kernel instantiations exist for 2, 3, 4, 8 and 16 rows (3: one reference with den = 6, e.g. BASELINE.json configs[3])
+    pl->rows_pad = pl->rows <= 2 ? 2 : pl->rows <= 3 ? 3 : pl->rows <= 4 ? 4 : pl->rows <= 8 ? 8 : 16;
 
     // workspace layout
     size_t o = 0;

@@ -115,13 +115,16 @@ __device__ __forceinline__ void load_weights(const ACC *row, ACC (&wt)[ROWS])
             wt[4 * q + 2] = *reinterpret_cast<ACC *>(&t.z);
             wt[4 * q + 3] = *reinterpret_cast<ACC *>(&t.w);
         }
-    } else {
+    } else if constexpr (ROWS % 2 == 0) {
 #pragma unroll
         for (int q = 0; q < ROWS / 2; ++q) {
             int2 t = __ldg(reinterpret_cast<const int2 *>(row) + q);
             wt[2 * q + 0] = *reinterpret_cast<ACC *>(&t.x);
             wt[2 * q + 1] = *reinterpret_cast<ACC *>(&t.y);
         }
+    } else {
+#pragma unroll
+        for (int q = 0; q < ROWS; ++q) wt[q] = __ldg(row + q);
     }
 }
 
@@ -138,13 +141,16 @@ __device__ __forceinline__ void load_weights_shared(const ACC *row, ACC (&wt)[RO
             wt[4 * q + 2] = *reinterpret_cast<const ACC *>(&t.z);
             wt[4 * q + 3] = *reinterpret_cast<const ACC *>(&t.w);
         }
-    } else {
+    } else if constexpr (ROWS % 2 == 0) {
 #pragma unroll
         for (int q = 0; q < ROWS / 2; ++q) {
             const int2 t = reinterpret_cast<const int2 *>(row)[q];
             wt[2 * q + 0] = *reinterpret_cast<const ACC *>(&t.x);
             wt[2 * q + 1] = *reinterpret_cast<const ACC *>(&t.y);
         }
+    } else {
+#pragma unroll
+        for (int q = 0; q < ROWS; ++q) wt[q] = row[q];
     }
 }
 

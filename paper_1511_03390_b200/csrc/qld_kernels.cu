@@ -268,6 +268,7 @@ cudaError_t launch_whole_r(int rows, const DemodParams &p, bool vec, cudaStream_
 {
     switch (rows) {
     case 2: return launch_whole_t<T, ACC, 2>(p, vec, st);
+    case 3: return launch_whole_t<T, ACC, 3>(p, vec, st);
     case 4: return launch_whole_t<T, ACC, 4>(p, vec, st);
     case 8: return launch_whole_t<T, ACC, 8>(p, vec, st);
     case 16: return launch_whole_t<T, ACC, 16>(p, vec, st);
@@ -279,6 +280,7 @@ cudaError_t launch_slide_r(int rows, const SlideParams &p, bool vec, cudaStream_
 {
     switch (rows) {
     case 2: return launch_slide_t<T, ACC, 2>(p, vec, st);
+    case 3: return launch_slide_t<T, ACC, 3>(p, vec, st);
     case 4: return launch_slide_t<T, ACC, 4>(p, vec, st);
     case 8: return launch_slide_t<T, ACC, 8>(p, vec, st);
     case 16: return launch_slide_t<T, ACC, 16>(p, vec, st);

@@ -88,7 +88,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
     constexpr int RROWS = ROWS + (IS_INT ? 0 : 1);
     // pixels per thread whose stored sums are prefetched in a sliding update (about 32 registers)
     constexpr int PFN_ = (IS_INT ? 32 : 16) / ROWS;
-    constexpr int PFN = PFN_ > 8 ? 8 : (PFN_ < 1 ? 1 : PFN_);
+    constexpr int PFN = PFN_ >= 8 ? 8 : (PFN_ >= 4 ? 4 : (PFN_ >= 2 ? 2 : 1));      // a power of two (batches of four)
     const int RS = CG * 32 + PAD;
     // epilogue warps (NEPI > 0): the combine buffer is double buffered and finalised by them
     const bool SPLIT = NEPI > 0 && TS > 1;
@@ -617,6 +617,7 @@ cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, co
 {
     switch (rows) {
     case 2: return launch_stream_t<T, ACC, 2>(tmap, p, sh, counter, n_sms, st);
+    case 3: return launch_stream_t<T, ACC, 3>(tmap, p, sh, counter, n_sms, st);
     case 4: return launch_stream_t<T, ACC, 4>(tmap, p, sh, counter, n_sms, st);
     case 8: return launch_stream_t<T, ACC, 8>(tmap, p, sh, counter, n_sms, st);
     case 16: return launch_stream_t<T, ACC, 16>(tmap, p, sh, counter, n_sms, st);
