@@ -74,10 +74,21 @@ def test_golden_closed_forms(oracle):
     for kind, N, num, den, level, expect in _golden():
         s = np.arange(1, N + 1, dtype=np.float64)
         for phi in (0.0, 0.7, 2.1, -1.3):
-            if kind == "tone":
+            if kind in ("tone", "norm"):
                 x = level * np.sin(2 * np.pi * num * s / den + phi)
             else:
                 x = np.full(N, level)
+            if kind == "norm":
+                # G3: the optional normalisation multiplies I, Q and R by 2/N, once each -- a scale that is dropped,
+                # applied twice, or applied to R but not to I/Q fails here (R = A, not A*N/2 or 4A/N)
+                I, Q, R, ph = oracle.qld(x[:, None], _ref(num=num, den=den), scale=2.0 / N)
+                assert abs(R[0] - level) <= 1e-12 * level, (kind, N, R[0], level)
+                assert abs(I[0] - level * math.cos(phi)) < 1e-12 and abs(Q[0] - level * math.sin(phi)) < 1e-12
+                assert abs(math.remainder(ph[0] - phi, 2 * math.pi)) < 1e-12       # the phase does not depend on the scale
+                I1, Q1 = oracle.demod(x[:, None], *oracle.ref_tables(_ref(num=num, den=den), 1, N))
+                R2, ph2 = oracle.finalise(I1, Q1, scale=2.0 / N)                   # the same through finalise alone
+                assert abs(R2[0] - level) <= 1e-12 * level and abs(math.remainder(ph2[0] - phi, 2 * math.pi)) < 1e-12
+                continue
             I, Q, R, ph = oracle.qld(x[:, None], _ref(num=num, den=den))
             assert abs(R[0] - expect) <= 1e-11 * max(1.0, expect), (kind, N, num, den, phi, R[0], expect)
             if kind == "tone":   # G5: I = (AN/2) cos phi, Q = (AN/2) sin phi, phase map = phi
