@@ -24,7 +24,6 @@ import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
-sys.path.insert(0, os.path.join(ROOT, "tests"))
 
 METRIC = "qld_pixel_samples_per_s"
 UNIT = "pixel-samples/s"
@@ -294,7 +293,7 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     # ---- CPU baseline (the oracle, as it stands) + parity of the timed configuration on the same rows
     if with_cpu and env.rank == 0:
         import oracle
-        from _parity import check_float_maps
+        from oracle.check import check_float_maps
         nt = oracle.max_threads()
         # about 15 s of oracle work at ~1.4e8 sample-references per second per core
         rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (K * N * W))))
@@ -388,7 +387,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     # ---- CPU baseline + parity: windows recomputed directly by the oracle on a band of rows ---------
     if with_cpu and env.rank == 0:
         import oracle
-        from _parity import check_float_maps
+        from oracle.check import check_float_maps
         nt = oracle.max_threads()
         n_win = 4
         rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (n_win * K * N * W))))

@@ -100,7 +100,8 @@ typedef struct {
     int32_t maps;            /* mask of QLD_MAP_*; 0 means QLD_MAP_ALL */
     uint32_t max_value;      /* largest sample value the caller guarantees (0 = type maximum); used only for
                                 the INT_BINS overflow bound */
-    int32_t resync_hops;     /* SLIDE, FP32: recompute the window from the ring every this many hops (0 = never) */
+    int32_t resync_hops;     /* SLIDE, FP32: recompute the window from the ring every this many hops, which bounds the drift of the
+                                add/subtract update; 0 = automatic (every 16*ceil(N/hop) hops), < 0 = never */
     int32_t external_store;  /* 1: the frame store (N frames, or ring_frames frames) is the caller's device buffer, given
                                 with qld_attach_frames_device; frames arrive in place and are announced with
                                 qld_commit_frames (zero-copy ingest).  ring_frames = -1 implies it. */
@@ -112,7 +113,9 @@ typedef struct {
                                 (H*W*bytes a multiple of 16, at least one 2 KB segment per SM, slide_hop >= 16..64
                                 depending on the frame size): QLD_E_UNSUPPORTED otherwise.  Results are identical to the
                                 frame re-reading update (bit-exact for INT_BINS). */
-    int32_t reserved2;
+    int32_t ref_tables_supplied; /* 1: the caller supplies every reference table with qld_set_ref_tables before the first
+                                qld_demod (QLD_E_STATE otherwise); refs[k].nu / num / den are then not used and not validated, so
+                                nu = 0 and nu = 1/2 (reading G18) can be expressed.  FP32 / FIXED (or AUTO) on whole-window stores. */
     void *workspace;         /* device memory of qld_workspace_bytes() bytes, 256-byte aligned, owned by the
                                 caller (e.g. a torch tensor) and kept alive until qld_destroy; NULL: the
                                 library allocates and frees it */
@@ -142,8 +145,9 @@ int qld_push_frames_device(qld_ctx *ctx, const void *device_frames, int n_frames
 
 /* Use the caller's device buffer in place (no copy).  The buffer must stay valid, and frames a pending demod
  * reads unchanged, while demods are in flight.
- * Whole-window store (ring_frames 0 / -1; with 0 the library's own store is simply left unused): a buffer
- * of N frames; counts as N frames pushed.
+ * Whole-window store (ring_frames 0 / -1; with 0 the library's own store is left unused until qld_reset detaches the
+ * buffer; qld_push_frames is refused with QLD_E_STATE while a buffer is attached): a buffer of N frames; counts as N
+ * frames pushed.
  * Ring (ring_frames > 0, external_store = 1): a buffer of ring_frames frames; counts as no frames: announce
  * them with qld_commit_frames as they arrive. */
 int qld_attach_frames_device(qld_ctx *ctx, const void *device_frames);
@@ -161,7 +165,9 @@ int qld_commit_frames(qld_ctx *ctx, int n_frames, void *producer_stream);
  * QLD_E_STATE when still in flight.  block = 1: waits, then QLD_OK. */
 int qld_push_done(qld_ctx *ctx, int block);
 
-/* A3/A3'/A4/A5/A6: enqueue one demodulation on the compute stream; it waits (on the device) for every push
+/* A3/A3'/A4/A5/A6 (P:99 Methods: the two sums and R(j,k); "the intensity at every pixel is multiplied by two
+ * numbers ... accumulated", then "squared and added"; P:181-183 sliding sequence; P:49 several frequencies): enqueue one
+ * demodulation on the compute stream; it waits (on the device) for every push
  * issued before it.
  *  QLD_WHOLE: the window is the most recent N frames stored (whole store: frames 1..N).  hop is ignored.
  *  QLD_SLIDE: ring contexts only.  The first call produces window 0 (frames 1..N); each later call advances
@@ -171,7 +177,9 @@ int qld_push_done(qld_ctx *ctx, int block);
  * QLD_E_STATE if the frames the window needs are not all pushed yet. */
 int qld_demod(qld_ctx *ctx, int mode, int hop);
 
-/* Device pointers to the maps of reference k written by the last qld_demod: row-major [H][W] float32, valid
+/* The processed images ("resulting in the 32-bit n x n processed image"; I and Q are the "two different 2-D arrays
+ * that represent the two quadrature components"; amplitude per P:99; phase per reading G6).
+ * Device pointers to the maps of reference k written by the last qld_demod: row-major [H][W] float32, valid
  * until the next qld_demod / qld_reset / qld_destroy; read them on the compute stream or after qld_sync().
  * Any out-pointer may be NULL.  A map that was not requested in cfg.maps comes back as NULL. */
 int qld_get_maps(qld_ctx *ctx, int k, const float **I, const float **Q, const float **amp, const float **phase);
@@ -189,6 +197,14 @@ int qld_read_map(qld_ctx *ctx, int k, int which, float *host_dst);
  * (FP32 accumulation) -- for inspection and tests.  Blocks until done.  Host pointers. */
 int qld_read_ref_table(qld_ctx *ctx, int k, int64_t s_first, int n, float *sin_out, float *cos_out);
 
+/* Caller-supplied reference tables (the main thread "creates tables of sine and cosine functions, appropriate for
+ * the choice of lock-in and sampling frequencies"; "read from pre-calculated arrays"): replace the table of reference
+ * k by sin_tab / cos_tab (host arrays of len == N doubles, entry i belongs to frame i+1, each in [-1, 1]).  The kernels
+ * then compute I = sum_s x_s sin_tab[s-1], Q = sum_s x_s cos_tab[s-1] whatever the arrays hold.  FP32: each entry is
+ * rounded once to float32; FIXED: to rint(2^30 * entry).  Whole-window stores only (QLD_E_UNSUPPORTED on rings and on
+ * INT_BINS contexts).  Blocks until the device tables are rebuilt. */
+int qld_set_ref_tables(qld_ctx *ctx, int k, const double *sin_tab, const double *cos_tab, int64_t len);
+
 /* QLD_ACC_FIXED only.  Replace the Q1.30 reference table of reference k by caller-supplied integers (host
  * arrays of n == N entries, entry i belongs to frame i+1, each in [-2^30, 2^30]); blocks until the device
  * table is rebuilt.  qld_read_ref_table_fixed copies the table in use back to the host (blocks). */
@@ -202,9 +218,15 @@ int qld_get_sums_i64(qld_ctx *ctx, int k, const int64_t **I, const int64_t **Q);
 /* Bookkeeping (host side, never blocks): frames pushed so far, windows produced so far. */
 int qld_counters(const qld_ctx *ctx, int64_t *frames_pushed, int64_t *windows_done);
 
-int qld_sync(qld_ctx *ctx);    /* wait for both streams */
-int qld_reset(qld_ctx *ctx);   /* forget all frames and accumulators; the next push is frame 1 again */
-void qld_destroy(qld_ctx *ctx);/* waits for pending work, frees what the library allocated; NULL is a no-op */
+/* Life cycle.  The paper's threads hand frames and images over with status flags ("a flag indicates the
+ * status"); here that hand-over is stream order, and these three are the only host-side waits:
+ *  qld_sync    waits for both streams (all pushes copied, all demods finished: maps and host copies are valid);
+ *  qld_reset   forgets all frames and accumulators -- the next push is frame 1 (t_1) of a new acquisition; a buffer
+ *              attached in place of a whole-window store is detached, an attached ring stays attached;
+ *  qld_destroy waits for pending work and frees what the library allocated; NULL is a no-op. */
+int qld_sync(qld_ctx *ctx);
+int qld_reset(qld_ctx *ctx);
+void qld_destroy(qld_ctx *ctx);
 
 /* Text of the last error of this context ("" if none).  ctx may be NULL: text of the last failed qld_create
  * on this thread. */
@@ -218,6 +240,13 @@ int64_t qld_kernel_launches(const qld_ctx *ctx);
  * "k_demod_stream", "k_demod_whole", "k_demod_split", "k_demod_tc" or "k_demod_slide".  Never NULL. */
 int qld_accum_mode(const qld_ctx *ctx);
 const char *qld_last_kernel(const qld_ctx *ctx);
+
+/* Debug / test hook: force the tile shape of the next launches of this context instead of the automatic choice (an
+ * invalid shape is ignored).  which = 0: k_demod_stream, a = SEG (contiguous bytes of every frame per tile, a power of two
+ * <= 2048), b = KC (frames per pipeline stage); forcing also lifts the frame-size threshold, so small frames go through
+ * the TMA-fed kernel.  which = 1: k_demod_tc, a = T (128-byte spans per tile), b = STAGES, c = KC (32 or 64).
+ * a = 0 restores the automatic choice.  Results never depend on the shape (tests/ run every shape against the oracle). */
+int qld_debug_set_tile(qld_ctx *ctx, int which, int a, int b, int c);
 
 /* Contrast-to-noise ratio of a processed image (Eq. (1), Fig. 6; the paper's quality metric, the step
  * after the path):  CNR = (mean_s - mean_surr) / sqrt( mean over the slice of (I(j,k) - mean_surr)^2 ), mean_s

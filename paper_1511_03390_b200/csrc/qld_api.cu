@@ -1,12 +1,15 @@
 // C-ABI entry points of libqld.so (include/qld.h): context, frame ingest (A2), stream/event ordering, and the
 // host-side bookkeeping of whole-window and sliding-window demodulation.  No arithmetic of the method runs on
-// the host: tables, sums and maps are all produced by the kernels in qld_tables.cu / qld_kernels.cu.
+// the host: reference tables, bin combine weights, sums and maps are all produced by the kernels in qld_tables.cu,
+// qld_kernels.cu, qld_stream.cu and qld_tc.cu; the host only plans buffers, orders streams and keeps counters.
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
 
 #include <new>
 #include <string>
+
+#include <nvtx3/nvToolsExt.h>
 
 #include "qld_internal.h"
 #include "qld_stream.h"
@@ -18,6 +21,12 @@ constexpr int N_PUSH_EVENTS = 64;
 constexpr int N_DEMOD_EVENTS = 32;
 
 thread_local std::string g_create_error;
+
+// NVTX range around a host-side entry point (push / demod / read): shows up in Nsight timelines, costs nothing without a tool
+struct NvtxRange {
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 struct DemodEvent {
     cudaEvent_t ev;
@@ -55,6 +64,10 @@ struct qld_ctx {
     bool own_ws;
     size_t ws_bytes;
     unsigned char *frames;   // store (or attached buffer)
+    unsigned char *own_frames; // the library-owned store (NULL on external contexts)
+    int dbg_stream[2], dbg_tc[3]; // qld_debug_set_tile overrides (zeros: automatic)
+    bool tables_supplied;    // cfg.ref_tables_supplied: tables come from qld_set_ref_tables
+    unsigned tables_set;     // bit k: reference k has its table
     void *wtab;
     double *cum;
     void *acc;
@@ -109,28 +122,6 @@ size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
 int64_t gcd64(int64_t a, int64_t b) { while (b) { int64_t t = a % b; a = b; b = t; } return a; }
 
-// exact sin/cos of 2*pi*a/D for multiples of a quarter and a twelfth of a turn, libm otherwise
-void exact_sincos(int64_t a, int64_t D, double extra, double *sn, double *cs)
-{
-    a %= D;
-    if (extra == 0.0 && (4 * a) % D == 0) {
-        static const double qs[4] = {0, 1, 0, -1}, qc[4] = {1, 0, -1, 0};
-        const int j = (int)((4 * a) / D) & 3;
-        *sn = qs[j]; *cs = qc[j];
-        return;
-    }
-    const long double th = 2.0L * 3.141592653589793238462643383279502884L * ((long double)a / (long double)D) + (long double)extra;
-    long double s = sinl(th), c = cosl(th);
-    if (extra == 0.0 && (12 * a) % D == 0) {
-        const int j = (int)((12 * a) / D) % 12;
-        if (j == 1 || j == 5) s = 0.5L;
-        if (j == 7 || j == 11) s = -0.5L;
-        if (j == 2 || j == 10) c = 0.5L;
-        if (j == 4 || j == 8) c = -0.5L;
-    }
-    *sn = (double)s; *cs = (double)c;
-}
-
 struct Plan {
     int H, W, dtype, bytes, N, K, accum, norm, maps, cap, cap_w, rows, rows_pad;
     bool ring, external, is_int, is_fixed;
@@ -159,6 +150,9 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     if (cfg->slide_hop > 0 && cfg->ring_frames <= 0) return bad(QLD_E_INVAL, "slide_hop needs a ring context");
     if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
     if (cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64)) return bad(QLD_E_INVAL, "unknown bits in maps");
+    if (cfg->ref_tables_supplied != 0 && cfg->ref_tables_supplied != 1) return bad(QLD_E_INVAL, "ref_tables_supplied must be 0 or 1");
+    if (cfg->ref_tables_supplied && cfg->ring_frames > 0) return bad(QLD_E_UNSUPPORTED, "ref_tables_supplied: whole-window stores only");
+    if (cfg->ref_tables_supplied && cfg->accum == QLD_ACC_INT_BINS) return bad(QLD_E_UNSUPPORTED, "ref_tables_supplied: FP32 or FIXED accumulation");
     memset(pl, 0, sizeof *pl);
     pl->H = cfg->H; pl->W = cfg->W; pl->dtype = cfg->dtype; pl->bytes = cfg->dtype == QLD_U8 ? 1 : 2;
     pl->N = cfg->N; pl->K = cfg->K; pl->norm = cfg->norm; pl->maps = (cfg->maps & QLD_MAP_ALL) ? cfg->maps : (cfg->maps | QLD_MAP_ALL);
@@ -174,7 +168,10 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         RefPlan &rp = pl->ref[k];
         rp.phase = r.phase; rp.phase_quarter = r.phase_quarter;
         if (!isfinite(r.phase)) return bad(QLD_E_INVAL, "phase must be finite");
-        if (r.den > 0) {
+        if (cfg->ref_tables_supplied) {                    // nu is whatever the caller's tables encode (G18)
+            rp.nu = r.nu; rp.num = 0; rp.den = 0;
+            all_rational = false;
+        } else if (r.den > 0) {
             if (r.den >= (1ll << 31) || r.num <= 0 || 2 * r.num >= r.den) return bad(QLD_E_INVAL, "need 0 < num/den < 1/2 and den < 2^31");
             const int64_t g = gcd64(r.num, r.den);
             rp.num = r.num / g; rp.den = r.den / g; rp.nu = (double)rp.num / (double)rp.den;
@@ -239,12 +236,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
             rp.n_rows = (int)(rp.use_diff ? rp.den / 2 : rp.den);
             rp.row_off = off;
             f.row_off[k] = off; f.n_rows[k] = rp.n_rows;
-            const int64_t D = 4 * rp.den;
-            for (int r = 0; r < rp.n_rows; ++r) {
-                const int64_t a = (4 * (int64_t)r + (int64_t)((rp.phase_quarter % 4 + 4) % 4) * rp.den) % D;
-                exact_sincos(a, D, rp.phase, &f.sw[off + r], &f.cw[off + r]);
-            }
-            off += rp.n_rows;
+            off += rp.n_rows;                   // f.sw / f.cw are filled on the device by qld_create (k_bin_weights)
         }
         pl->rows = off;
     } else {
@@ -280,7 +272,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     pl->off_rfix = o; if (pl->is_fixed) o += align_up((size_t)2 * pl->K * pl->N * 4);
     pl->off_digits = o; if (pl->is_fixed) o += align_up(qld_tc_digit_bytes(pl->K, pl->N));
     pl->off_sums = o; if (pl->is_fixed && (pl->maps & QLD_MAP_SUMS_I64)) o += align_up((size_t)2 * pl->K * pl->HW * 8);
-    pl->off_counter = o; o += 256;            // tile counter of the persistent kernels
+    pl->off_counter = o; o += 512;            // tile counter of the persistent kernels (+256: 32 doubles of scratch)
     pl->total = o;
     return QLD_OK;
 }
@@ -304,7 +296,9 @@ int init_device_state(qld_ctx *c)
         CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
         CU(c, cudaMemsetAsync(c->cum, 0, (size_t)c->cap_w * c->rows_pad * 8, c->s_copy));
     }
-    if (c->is_fixed) {
+    if (c->tables_supplied) {
+        if (c->is_fixed) CU(c, cudaMemsetAsync(c->rfix, 0, (size_t)2 * c->K * c->N * 4, c->s_copy));
+    } else if (c->is_fixed) {
         TableFillParams tp;
         memset(&tp, 0, sizeof tp);
         tp.K = c->K;
@@ -319,6 +313,25 @@ int init_device_state(qld_ctx *c)
     }
     CU(c, cudaEventRecord(c->tables_ev, c->s_copy));
     CU(c, cudaStreamWaitEvent(c->s_comp, c->tables_ev, 0));
+    return QLD_OK;
+}
+
+// INT_BINS: the <= 16 combine weights sin / cos(2 pi r/den + phase) of the bin rows, computed on the device and kept in
+// the by-value epilogue parameters
+int fetch_bin_weights(qld_ctx *c)
+{
+    if (!c->is_int) return QLD_OK;
+    TableFillParams tp;
+    memset(&tp, 0, sizeof tp);
+    tp.K = c->K; tp.is_int = 1; tp.rows = c->rows_pad;
+    for (int k = 0; k < c->K; ++k) tp.ref[k] = c->ref[k];
+    double *scratch = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(c->tile_counter) + 256);
+    CU(c, qld_launch_bin_weights(tp, scratch, c->s_copy));
+    c->launches++;
+    double w[2 * QLD_MAX_ROWS];
+    CU(c, cudaMemcpyAsync(w, scratch, sizeof w, cudaMemcpyDeviceToHost, c->s_copy));
+    CU(c, cudaStreamSynchronize(c->s_copy));
+    for (int r = 0; r < QLD_MAX_ROWS; ++r) { c->fin.sw[r] = w[r]; c->fin.cw[r] = w[QLD_MAX_ROWS + r]; }
     return QLD_OK;
 }
 
@@ -415,13 +428,14 @@ int stream_tmap_for(qld_ctx *c, const StreamShape &sh)
 int run_whole_tc(qld_ctx *c)
 {
     if (!c->tmap_valid) {
-        CU(c, qld_tc_encode_tmap(c->tmap, c->frames, c->HW * c->bytes, c->N, c->K, c->n_sms));
+        CU(c, qld_tc_encode_tmap(c->tmap, c->frames, c->HW * c->bytes, c->N, c->K, c->n_sms, c->dbg_tc));
         c->tmap_valid = true;
     }
     TcParams p;
     memset(&p, 0, sizeof p);
     p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes;
     p.digits = c->digits; p.sums_out = c->sums; p.tile_counter = c->tile_counter;
+    p.force_T = c->dbg_tc[0]; p.force_stages = c->dbg_tc[1]; p.force_kc = c->dbg_tc[2];
     p.fin = fin_with_maps(c);
     CU(c, qld_launch_demod_tc(c->tmap, p, c->n_sms, c->s_comp));
     c->launches++;
@@ -445,7 +459,7 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
     p.onehot = c->is_int && c->K == 1;
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0) {
         int rc = stream_tmap_for(c, sh);
         if (rc) return rc;
@@ -464,7 +478,7 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
 // expired batch: taken off the accumulators, then overwritten).
 int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool add, bool sub, bool first_of_seed)
 {
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
     DemodParams p;
     memset(&p, 0, sizeof p);
@@ -511,7 +525,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         return record_demod(c, a_old + 1);                    // conservative: the whole window stays protected from overwriting
     }
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
-    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms);
+    const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0 && hop >= sh.kc) {
         DemodParams p;
         memset(&p, 0, sizeof p);
@@ -582,12 +596,13 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     qld_ctx *c = new (std::nothrow) qld_ctx();
     if (!c) return fail(nullptr, QLD_E_NOMEM, "host allocation failed");
     c->H = pl.H; c->W = pl.W; c->dtype = pl.dtype; c->bytes = pl.bytes; c->N = pl.N; c->K = pl.K;
-    c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops > 0 ? cfg->resync_hops : 0;
+    c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops;
     c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
     c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
     for (int k = 0; k < pl.K; ++k) c->ref[k] = pl.ref[k];
     c->fin = pl.fin;
     c->ws_bytes = pl.total;
+    c->tables_supplied = cfg->ref_tables_supplied == 1;
     auto cleanup = [&](int code) { qld_destroy(c); return code; };
     if (cfg->workspace) {
         if (cfg->workspace_bytes < pl.total || (reinterpret_cast<uintptr_t>(cfg->workspace) & 255)) {
@@ -602,6 +617,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     }
     unsigned char *b = static_cast<unsigned char *>(c->ws);
     c->frames = pl.external ? nullptr : b + pl.off_frames;
+    c->own_frames = c->frames;
     c->wtab = b + pl.off_wtab; c->cum = reinterpret_cast<double *>(b + pl.off_cum);
     c->acc = b + pl.off_acc; c->ped = reinterpret_cast<float *>(b + pl.off_ped);
     c->part = b + pl.off_part; c->slide_hop = pl.slide_hop; c->n_part = pl.slide_hop > 0 ? pl.N / pl.slide_hop : 0;
@@ -634,6 +650,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     }
     if (cudaEventCreateWithFlags(&c->tables_ev, cudaEventDisableTiming) != cudaSuccess) return cleanup(fail(nullptr, QLD_E_CUDA, "event creation failed"));
     rc = init_device_state(c);
+    if (rc == QLD_OK) rc = fetch_bin_weights(c);
     if (rc) { g_create_error = c->err; return cleanup(rc); }
     ce = cudaStreamSynchronize(c->s_copy);
     if (ce != cudaSuccess) { g_create_error = cudaGetErrorString(ce); return cleanup(QLD_E_CUDA); }
@@ -643,10 +660,12 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
 
 static int push_checked(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
 {
+    NvtxRange nvtx("qld_push_frames");
     if (!c) return QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
     if (!src || n < 1) return fail(c, QLD_E_INVAL, "push: null buffer or n_frames < 1");
     if (c->external) return fail(c, QLD_E_STATE, "push: this context takes frames in place (external_store): attach + qld_commit_frames");
+    if (c->frames != c->own_frames) return fail(c, QLD_E_STATE, "push: a caller buffer is attached in place of the store (qld_reset detaches it)");
     if (n > c->cap) return fail(c, QLD_E_INVAL, "push: more frames than the store holds");
     return push_common(c, src, n, kind);
 }
@@ -657,6 +676,7 @@ int qld_push_frames_device(qld_ctx *c, const void *device_frames, int n_frames) 
 
 int qld_commit_frames(qld_ctx *c, int n_frames, void *producer_stream)
 {
+    NvtxRange nvtx("qld_commit_frames");
     if (!c) return QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
     if (!c->external) return fail(c, QLD_E_STATE, "commit: context owns its frame store (use qld_push_frames)");
@@ -698,10 +718,12 @@ int qld_push_done(qld_ctx *c, int block)
 
 int qld_demod(qld_ctx *c, int mode, int hop)
 {
+    NvtxRange nvtx(mode == QLD_SLIDE ? "qld_demod(SLIDE)" : "qld_demod(WHOLE)");
     if (!c) return QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
     if (mode != QLD_WHOLE && mode != QLD_SLIDE) return fail(c, QLD_E_INVAL, "demod: unknown mode");
     if (!c->frames) return fail(c, QLD_E_STATE, "demod: no frames attached");
+    if (c->tables_supplied && c->tables_set != (1u << c->K) - 1u) return fail(c, QLD_E_STATE, "demod: qld_set_ref_tables has not been called for every reference");
     if (c->push_pending || c->pushed > 0) CU(c, cudaStreamWaitEvent(c->s_comp, last_push_event(c), 0));
     if (mode == QLD_WHOLE) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames stored");
@@ -724,7 +746,10 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (c->slide_hop > 0 && hop != c->slide_hop) return fail(c, QLD_E_INVAL, "demod: this context slides by cfg.slide_hop only");
     if (c->pushed < c->win_start + hop + c->N) return fail(c, QLD_E_STATE, "demod: fewer than hop new frames pushed");
     int rc;
-    if (!c->is_int && c->resync_hops > 0 && c->hops_since_seed + 1 >= c->resync_hops) {
+    // FP32 ring sums random-walk away from a recompute (each hop adds rounding of its own): resynchronise from the ring
+    // every resync_hops hops; 0 = automatic (16 windows' worth of hops: 1/16 more traffic), negative = never
+    const int64_t resync = c->resync_hops > 0 ? c->resync_hops : (c->resync_hops == 0 ? 16 * (int64_t)((c->N + hop - 1) / hop) : 0);
+    if (!c->is_int && resync > 0 && c->hops_since_seed + 1 >= resync) {
         rc = seed_window(c, c->win_start + hop);
         c->hops_since_seed = 0;
     } else {
@@ -759,6 +784,7 @@ int qld_get_bins(qld_ctx *c, int k, const int32_t **rows, int *n_rows)
 
 int qld_read_map(qld_ctx *c, int k, int which, float *host_dst)
 {
+    NvtxRange nvtx("qld_read_map");
     if (!c || !host_dst || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "read_map: bad argument") : QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
     const float *src = which == QLD_MAP_I ? c->mapI : which == QLD_MAP_Q ? c->mapQ : which == QLD_MAP_AMP ? c->mapA : which == QLD_MAP_PHASE ? c->mapP : nullptr;
@@ -784,6 +810,37 @@ int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out
     return QLD_OK;
 }
 
+int qld_set_ref_tables(qld_ctx *c, int k, const double *sin_tab, const double *cos_tab, int64_t len)
+{
+    if (!c || k < 0 || k >= c->K || !sin_tab || !cos_tab) return c ? fail(c, QLD_E_INVAL, "set_ref_tables: bad argument") : QLD_E_INVAL;
+    if (c->sticky) return QLD_E_CUDA;
+    if (c->ring || c->is_int) return fail(c, QLD_E_UNSUPPORTED, "set_ref_tables: whole-window FP32 / FIXED contexts only");
+    if (len != c->N) return fail(c, QLD_E_INVAL, "set_ref_tables: len must equal N");
+    for (int64_t i = 0; i < len; ++i)
+        if (!(sin_tab[i] >= -1.0 && sin_tab[i] <= 1.0 && cos_tab[i] >= -1.0 && cos_tab[i] <= 1.0))
+            return fail(c, QLD_E_INVAL, "set_ref_tables: entries must lie in [-1, 1]");
+    int rc = qld_sync(c);
+    if (rc) return rc;
+    double *tab = nullptr;
+    if (cudaMalloc(&tab, (size_t)2 * len * sizeof(double)) != cudaSuccess) { (void)cudaGetLastError(); return fail(c, QLD_E_NOMEM, "set_ref_tables: device scratch"); }
+    cudaError_t e = cudaMemcpy(tab, sin_tab, (size_t)len * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(tab + len, cos_tab, (size_t)len * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        if (c->is_fixed) {
+            e = qld_launch_fixed_from_doubles(tab, (int)len, k, c->rfix, c->N, c->s_comp);
+            if (e == cudaSuccess) e = qld_launch_digit_pack(c->rfix, c->N, c->N, c->K, c->digits, c->s_comp);
+        } else {
+            e = qld_launch_table_from_doubles(tab, (int)len, 2 * k, c->rows_pad, c->cap_w, c->wtab, c->cum, c->s_comp);
+        }
+        c->launches += c->is_fixed ? 2 : 1;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->s_comp);
+    cudaFree(tab);
+    if (e != cudaSuccess) return cuda_fail(c, e, "set_ref_tables");
+    c->tables_set |= 1u << k;
+    return QLD_OK;
+}
+
 int qld_set_ref_table_fixed(qld_ctx *c, int k, const int32_t *sin_q30, const int32_t *cos_q30, int n)
 {
     if (!c || k < 0 || k >= c->K || !sin_q30 || !cos_q30) return c ? fail(c, QLD_E_INVAL, "set_ref_table_fixed: bad argument") : QLD_E_INVAL;
@@ -799,6 +856,7 @@ int qld_set_ref_table_fixed(qld_ctx *c, int k, const int32_t *sin_q30, const int
     CU(c, cudaMemcpy(c->rfix + (size_t)(2 * k + 1) * c->N, cos_q30, (size_t)n * 4, cudaMemcpyHostToDevice));
     CU(c, qld_launch_digit_pack(c->rfix, c->N, c->N, c->K, c->digits, c->s_comp));
     c->launches++;
+    c->tables_set |= 1u << k;
     return QLD_OK;
 }
 
@@ -847,7 +905,9 @@ int qld_reset(qld_ctx *c)
     if (rc) return rc;
     c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
-    if (c->external && !c->ring) { c->frames = nullptr; c->tmap_valid = false; }   // an attached ring stays attached
+    if (!c->ring && c->frames != c->own_frames) {          // an attached stack is detached (an attached ring stays attached)
+        c->frames = c->own_frames; c->tmap_valid = false; c->stream_tmap_frames = nullptr;
+    }
     if (c->ring) {
         rc = init_device_state(c);
         if (rc) return rc;
@@ -873,6 +933,16 @@ void qld_destroy(qld_ctx *c)
 const char *qld_last_error(const qld_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 int64_t qld_kernel_launches(const qld_ctx *c) { return c ? c->launches : 0; }
+
+int qld_debug_set_tile(qld_ctx *c, int which, int a, int b, int d)
+{
+    if (!c) return QLD_E_INVAL;
+    if (a < 0 || b < 0 || d < 0) return fail(c, QLD_E_INVAL, "debug_set_tile: negative value");
+    if (which == 0) { c->dbg_stream[0] = a; c->dbg_stream[1] = b; }
+    else if (which == 1) { c->dbg_tc[0] = a; c->dbg_tc[1] = b; c->dbg_tc[2] = d; c->tmap_valid = false; }
+    else return fail(c, QLD_E_INVAL, "debug_set_tile: which must be 0 (k_demod_stream) or 1 (k_demod_tc)");
+    return QLD_OK;
+}
 
 int qld_accum_mode(const qld_ctx *c) { return c ? c->accum : QLD_E_INVAL; }
 

@@ -6,7 +6,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "qld.h"
+#include "qld_internal.h"
 
 namespace {
 
@@ -70,7 +70,8 @@ extern "C" int qld_display_map(const float *map_device, int64_t n, uint8_t *out_
     if (!map_device || !out_device || !scratch_device || n < 1) return QLD_E_INVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     uint32_t *mm = static_cast<uint32_t *>(scratch_device);
-    const int blocks = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+    const int cap = qld_sm_count() * 8;
+    const int blocks = (int)((n + 255) / 256 < cap ? (n + 255) / 256 : cap);
     k_range_init<<<1, 1, 0, st>>>(mm);
     k_range<<<blocks, 256, 0, st>>>(map_device, n, mm);
     k_to_u8<<<blocks, 256, 0, st>>>(map_device, n, mm, range_device, out_device);

@@ -98,4 +98,18 @@ struct TableFillParams {
 cudaError_t qld_launch_demod_whole(int dtype, int is_int, int rows, const DemodParams &p, cudaStream_t st);
 cudaError_t qld_launch_demod_slide(int dtype, int is_int, int rows, const SlideParams &p, cudaStream_t st);
 cudaError_t qld_launch_table_fill(const TableFillParams &p, cudaStream_t st);
+// rows (row0, row0 + 1) of the float table from caller-supplied doubles tab[2][n] (sin, cos), frames 1..n; recomputes cum
+cudaError_t qld_launch_table_from_doubles(const double *tab, int n, int row0, int rows, int cap_w, void *wtab, double *cum, cudaStream_t st);
+cudaError_t qld_launch_bin_weights(const TableFillParams &p, double *out32 /* device: sw[16], cw[16] */, cudaStream_t st);
 int qld_pixels_per_thread(int dtype, int rows, int64_t HW, const void *frames, int64_t frame_stride);
+
+// multiprocessor count of the current device (cached per device)
+inline int qld_sm_count()
+{
+    static int cached[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 1;
+    int &n = cached[dev & 63];
+    if (n == 0 && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 1;
+    return n > 0 ? n : 1;
+}

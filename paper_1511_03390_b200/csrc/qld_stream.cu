@@ -20,9 +20,6 @@
 // The frames of a launch are a list of runs (DemodRun): a whole window is one or two runs of weight +w, and the
 // sliding update of PAPER.md:181-183 (A5) is the same kernel over {expired frames, -w} + {new frames, +w} with the
 // sums added to the accumulators the previous window left in global memory.
-#include <stdio.h>
-#include <stdlib.h>
-
 #include "qld_device.cuh"
 #include "qld_ptx.cuh"
 #include "qld_stream.h"
@@ -629,7 +626,7 @@ cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, co
 
 // Tile shape for this (dtype, rows, frame size), or seg = 0 when the streaming kernel does not apply (row pitch or
 // base not 16-byte aligned, or a frame too small to give every SM a tile: k_demod_whole handles those).
-StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms)
+StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int force_seg, int force_kc)
 {
     StreamShape sh = {0, 0, 0};
     const int bytes = dtype == QLD_U8 ? 1 : 2;
@@ -644,9 +641,9 @@ StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const 
     while (seg > 32 * vb && (row_bytes + seg - 1) / seg < 2 * (int64_t)n_sms) seg /= 2;
     int kc = 32768 / seg > 16 ? 32768 / seg : 16, stages = 0;      // stages of at least 32 KB
     bool forced = false;
-    if (const char *e = getenv("QLD_STREAM_TILE")) {      // tuning / test override: "SEG,KC" (also lifts the size threshold)
-        int s2 = 0, k2 = 0;
-        if (sscanf(e, "%d,%d", &s2, &k2) == 2 && s2 >= 32 * vb && s2 <= nw * 32 * vb && s2 <= 2048 && (s2 & (s2 - 1)) == 0 && k2 >= 4 && k2 <= 256) { seg = s2; kc = k2; forced = true; }
+    if (force_seg > 0) {                                   // debug / test override (qld_debug_set_tile)
+        const int s2 = force_seg, k2 = force_kc;
+        if (s2 >= 32 * vb && s2 <= nw * 32 * vb && s2 <= 2048 && (s2 & (s2 - 1)) == 0 && k2 >= 4 && k2 <= 256) { seg = s2; kc = k2; forced = true; }
     }
     if (!forced && (row_bytes + seg - 1) / seg < n_sms) return sh;
     const int ts = nw / (seg / (32 * vb));

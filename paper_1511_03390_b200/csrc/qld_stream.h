@@ -11,7 +11,8 @@ struct StreamShape {
     int32_t stages;   // shared-memory stages
 };
 
-StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms);
+// force_seg / force_kc > 0: debug override of the tile shape (qld_debug_set_tile); it also lifts the frame-size threshold
+StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int force_seg = 0, int force_kc = 0);
 cudaError_t qld_stream_encode_tmap(void *tmap_out /*128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int cap, const StreamShape &sh);
 cudaError_t qld_launch_demod_stream(int dtype, int is_int, int rows, const void *tmap, const DemodParams &p, const StreamShape &sh,
                                     unsigned int *counter, int n_sms, cudaStream_t st);

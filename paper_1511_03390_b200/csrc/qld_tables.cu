@@ -7,31 +7,12 @@
 // used when a frame enters a sliding window and when it leaves it.
 // For INT_BINS the rows are integer indicators of the phase bin r = num*s mod den (see include/qld.h).
 // A running fp64 sum of every float row (cum) provides sum_s w(s) over any window for the pedestal term.
+#include "qld_angle.cuh"
 #include "qld_internal.h"
 
+using namespace qld_angle;
+
 namespace {
-
-__device__ __forceinline__ int64_t bin_of(const RefPlan &rf, int64_t s)
-{
-    const uint64_t a = (uint64_t)(rf.num % rf.den), b = (uint64_t)(s % rf.den);
-    return (int64_t)((a * b) % (uint64_t)rf.den);      // den < 2^31: the product fits 64 bits
-}
-
-__device__ __forceinline__ double half_turns_of(const RefPlan &rf, int64_t s)
-{
-    double a;
-    if (rf.den > 0) {
-        a = 2.0 * (double)bin_of(rf, s) / (double)rf.den;
-    } else {
-        const double sd = (double)s;
-        const double hi = rf.nu * sd;
-        const double lo = fma(rf.nu, sd, -hi);          // exact low part of nu*s
-        a = 2.0 * ((hi - floor(hi)) + lo);
-    }
-    a += 0.5 * (double)(rf.phase_quarter & 3);
-    if (rf.phase != 0.0) a += rf.phase * 0.31830988618379067154;   // phase / pi
-    return a;
-}
 
 __global__ void k_table_fill(const TableFillParams p)
 {
@@ -68,7 +49,74 @@ __global__ void k_table_fill(const TableFillParams p)
     }
 }
 
+// INT_BINS combine weights: row r of reference k holds the (difference of) phase-bin sums whose frames all carry the
+// reference value sin / cos(2*pi*r/den + phase), so I = sum_r row_r * sw[r], Q = sum_r row_r * cw[r] (include/qld.h).
+// With no free phase the angle is the rational a/D of a turn, D = 4*den, a = 4*r + phase_quarter*den; whenever that is a
+// whole number j of twelfths of a turn the value is taken from the twelve-entry table of 2*sin(j*30 deg) =
+// 0, 1, sqrt3, 2, sqrt3, 1, 0, -1, ... halved (exact 0, +-1/2, +-1; sqrt3/2 correctly rounded) -- this is what makes
+// nu = 1/4 integer valued and nu = 1/6 exact in its halves; every other angle goes through fp64 sincospi of the reduced
+// half-turn count.  out[0..15] = sw, out[16..31] = cw (zeros for padding rows).
+__global__ void k_bin_weights(const TableFillParams p, double *out)
+{
+    const int t = threadIdx.x;
+    if (t >= 2 * QLD_MAX_ROWS) return;
+    out[t] = 0.0;
+    if (t >= QLD_MAX_ROWS) return;
+    for (int k = 0; k < p.K; ++k) {
+        const RefPlan &rf = p.ref[k];
+        const int r = t - rf.row_off;
+        if (r < 0 || r >= rf.n_rows) continue;
+        const int64_t D = 4 * rf.den;
+        const int64_t a = (4 * (int64_t)r + (int64_t)(rf.phase_quarter & 3) * rf.den) % D;
+        double sn, cs;
+        if (rf.phase == 0.0 && (12 * a) % D == 0) {
+            const double r3 = sqrt(3.0);
+            const double twice_sin[12] = {0.0, 1.0, r3, 2.0, r3, 1.0, 0.0, -1.0, -r3, -2.0, -r3, -1.0};
+            const int j = (int)((12 * a) / D);
+            sn = 0.5 * twice_sin[j];
+            cs = 0.5 * twice_sin[(j + 3) % 12];           // cos x = sin(x + 90 deg)
+        } else {
+            sincospi(2.0 * (double)a / (double)D + rf.phase * 0.31830988618379067154, &sn, &cs);
+        }
+        out[t] = sn;
+        out[QLD_MAX_ROWS + t] = cs;
+    }
+}
+
+// caller-supplied tables (qld_set_ref_tables): rounded once to fp32, running sums redone for the two rows
+__global__ void k_table_from_doubles(const double *tab, int n, int row0, int rows, int cap_w, float *wtab, double *cum)
+{
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int64_t e = (int64_t)(i + 1) % cap_w;
+        wtab[e * rows + row0] = (float)tab[i];
+        wtab[e * rows + row0 + 1] = (float)tab[n + i];
+    }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        const int r = row0 + threadIdx.x;
+        double c = 0.0;                                   // entry of frame 0
+        cum[r] = 0.0;
+        for (int i = 0; i < n; ++i) {
+            const int64_t e = (int64_t)(i + 1) % cap_w;
+            c += (double)wtab[e * rows + r];
+            cum[e * rows + r] = c;
+        }
+    }
+}
+
 }  // namespace
+
+cudaError_t qld_launch_table_from_doubles(const double *tab, int n, int row0, int rows, int cap_w, void *wtab, double *cum, cudaStream_t st)
+{
+    k_table_from_doubles<<<1, 256, 0, st>>>(tab, n, row0, rows, cap_w, static_cast<float *>(wtab), cum);
+    return cudaGetLastError();
+}
+
+cudaError_t qld_launch_bin_weights(const TableFillParams &p, double *out32, cudaStream_t st)
+{
+    k_bin_weights<<<1, 2 * QLD_MAX_ROWS, 0, st>>>(p, out32);
+    return cudaGetLastError();
+}
 
 cudaError_t qld_launch_table_fill(const TableFillParams &p, cudaStream_t st)
 {

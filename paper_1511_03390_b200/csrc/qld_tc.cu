@@ -21,14 +21,14 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
-#include <stdio.h>
-#include <stdlib.h>
 
+#include "qld_angle.cuh"
 #include "qld_internal.h"
 #include "qld_ptx.cuh"
 #include "qld_tc.h"
 
 using namespace qld_ptx;
+using qld_angle::half_turns_of;
 
 namespace {
 
@@ -36,6 +36,9 @@ constexpr int KC_PAD = 64;        // the digit tiles are padded to a multiple of
 constexpr int SUB_BYTES = 128;    // pixel bytes per MMA M tile
 constexpr int MMA_K = 32;         // frames per tcgen05.mma (8-bit operands)
 constexpr int GRP = 8;            // frames per 128-byte-swizzle atom (8 rows of 128 bytes = 1 KB)
+constexpr int TC_TQ = 16;         // tile-id queue entries: the producer runs at most `stages` <= 12 tiles ahead of the MMA warp
+constexpr int TC_MAX_STAGES = 12;
+static_assert(TC_MAX_STAGES < TC_TQ, "the tile queue must outlast the producer's run-ahead");
 
 // ---------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -75,21 +78,6 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes,
 // ---------------------------------------------------------------------------------------------------
 // fixed-point reference table and its digit tiles
 // ---------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double half_turns_of(const RefPlan &rf, int64_t s)
-{
-    double a;
-    if (rf.den > 0) {
-        const uint64_t r = ((uint64_t)(rf.num % rf.den) * (uint64_t)(s % rf.den)) % (uint64_t)rf.den;
-        a = 2.0 * (double)r / (double)rf.den;
-    } else {
-        const double sd = (double)s, hi = rf.nu * sd, lo = fma(rf.nu, sd, -hi);
-        a = 2.0 * ((hi - floor(hi)) + lo);
-    }
-    a += 0.5 * (double)(rf.phase_quarter & 3);
-    if (rf.phase != 0.0) a += rf.phase * 0.31830988618379067154;
-    return a;
-}
-
 // rfix[r][s-1] = rint(2^30 * sin or cos(theta_{k,s})), r = 2k (sin) / 2k+1 (cos), s = 1..n
 __global__ void k_fixed_table_fill(TableFillParams p, int32_t *rfix, int n_stride)
 {
@@ -99,6 +87,14 @@ __global__ void k_fixed_table_fill(TableFillParams p, int32_t *rfix, int n_strid
         sincospi(half_turns_of(p.ref[k], p.s_first + i), &sn, &cs);
         rfix[(int64_t)(2 * k) * n_stride + i] = (int32_t)rint(sn * 1073741824.0);
         rfix[(int64_t)(2 * k + 1) * n_stride + i] = (int32_t)rint(cs * 1073741824.0);
+    }
+}
+
+__global__ void k_fixed_from_doubles(const double *tab, int n, int k, int32_t *rfix, int n_stride)
+{
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        rfix[(int64_t)(2 * k) * n_stride + i] = (int32_t)rint(tab[i] * 1073741824.0);
+        rfix[(int64_t)(2 * k + 1) * n_stride + i] = (int32_t)rint(tab[n + i] * 1073741824.0);
     }
 }
 
@@ -138,7 +134,7 @@ struct TcSmem {
         b_stage = (kc / MMA_K) * nc * MMA_K;
         off_b = stages * a_stage;
         off_bar = off_b + stages * b_stage;
-        total = off_bar + (2 * stages + 4) * 8 + 16 + 48;
+        total = off_bar + (2 * stages + 4) * 8 + 16 + 8 + TC_TQ * 4 + 8;   // barriers, TMEM slot, tile queue, tbuf_tile
     }
 };
 
@@ -157,8 +153,8 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     uint64_t *tfull = empty + STAGES;
     uint64_t *tempty = tfull + 2;
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
-    volatile int *tile_q = reinterpret_cast<volatile int *>(tmem_slot + 2);      // [8] tile ids, producer -> MMA warp
-    volatile int *tbuf_tile = tile_q + 8;                                        // [2] tile id per accumulator buffer
+    volatile int *tile_q = reinterpret_cast<volatile int *>(tmem_slot + 2);      // [TC_TQ] tile ids, producer -> MMA warp
+    volatile int *tbuf_tile = tile_q + TC_TQ;                                        // [2] tile id per accumulator buffer
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n_chunks = (p.N + KC - 1) / KC;
@@ -196,7 +192,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
             for (;; ++it) {
                 int tile = (int)atomicAdd(p.tile_counter, 1u);
                 if (tile >= n_tiles) tile = -1;
-                tile_q[it & 7] = tile;                       // published by the next arrive on full[stage]
+                tile_q[it & (TC_TQ - 1)] = tile;                       // published by the next arrive on full[stage]
                 if (tile < 0) {                              // end of work: an empty stage carries the sentinel
                     mbar_wait(&empty[stage], phase ^ 1);
                     mbar_arrive(&full[stage]);
@@ -240,7 +236,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
             mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);     // epilogue has drained this accumulator buffer
             tc_fence_after();
             mbar_wait(&full[stage], phase);                   // first chunk of the tile (or the sentinel) has landed
-            const int tile = tile_q[it & 7];
+            const int tile = tile_q[it & (TC_TQ - 1)];
             if (lane == 0) tbuf_tile[buf] = tile;
             if (tile < 0) {
                 if (lane == 0) { mbar_arrive(&tfull[buf]); mbar_arrive(&tfull[buf]); }
@@ -345,7 +341,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
 // stages as fit in shared memory.
 struct TcShape { int T, kc, stages, use4d; };
 
-TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms)
+TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms, const int *force)
 {
     TcShape sh;
     const int n_sub = (int)((row_bytes + SUB_BYTES - 1) / SUB_BYTES);
@@ -360,12 +356,11 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms)
     sh.T = T;
     sh.kc = 64;
     sh.stages = (200 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
-    if (const char *e = getenv("QLD_TC_TILE")) {          // tuning override: "T,STAGES,KC"
-        int t = 0, s2 = 0, kc = 0;
-        if (sscanf(e, "%d,%d,%d", &t, &s2, &kc) == 3 && t >= 1 && 2 * t * nc <= 512 && s2 >= 2 && (kc == 32 || kc == 64) &&
-            TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
+    if (force && force[0] > 0) {                          // debug / test override (qld_debug_set_tile): T, STAGES, KC
+        const int t = force[0], s2 = force[1], kc = force[2];
+        if (2 * t * nc <= 512 && s2 >= 2 && (kc == 32 || kc == 64) && TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
     }
-    if (sh.stages > 12) sh.stages = 12;
+    if (sh.stages > TC_MAX_STAGES) sh.stages = TC_MAX_STAGES;
     sh.use4d = (row_bytes % SUB_BYTES == 0 && N >= GRP) ? 1 : 0;
     return sh;
 }
@@ -373,7 +368,8 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms)
 template <int NC, int BYTES>
 cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
-    const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms);
+    const int force[3] = {p.force_T, p.force_stages, p.force_kc};
+    const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
     auto kern = k_demod_tc<NC, BYTES>;
     // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
@@ -415,7 +411,7 @@ size_t qld_tc_digit_bytes(int K, int N)
 //  [0] 2-D {row bytes, frames}, box {128 B, 8 frames}: one swizzle atom, any shape (zero fill beyond the edges);
 //  [1] 4-D {128 B, 8 frames, spans, frame groups}, box {128, 8, T, KC/8}: a whole pipeline stage in one copy,
 //      spans innermost in the walk.  Only valid (and only used) when row_bytes % 128 == 0 and N >= 8.
-cudaError_t qld_tc_encode_tmap(void *tmaps_out, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms)
+cudaError_t qld_tc_encode_tmap(void *tmaps_out, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms, const int *force)
 {
     static EncodeTiledFn fn = nullptr;
     if (!fn) {
@@ -437,7 +433,7 @@ cudaError_t qld_tc_encode_tmap(void *tmaps_out, const void *frames, int64_t row_
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
     }
-    const TcShape sh = tc_shape(qld_tc_columns(K), row_bytes, n_frames, n_sms);
+    const TcShape sh = tc_shape(qld_tc_columns(K), row_bytes, n_frames, n_sms, force);
     if (sh.use4d) {
         const cuuint64_t dims[4] = {SUB_BYTES, GRP, (cuuint64_t)(row_bytes / SUB_BYTES), (cuuint64_t)(n_frames / GRP)};
         const cuuint64_t strides[3] = {(cuuint64_t)row_bytes, SUB_BYTES, (cuuint64_t)row_bytes * GRP};
@@ -456,6 +452,12 @@ cudaError_t qld_tc_encode_tmap(void *tmaps_out, const void *frames, int64_t row_
 cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st)
 {
     k_fixed_table_fill<<<(p.n * p.K + 255) / 256, 256, 0, st>>>(p, rfix, n_stride);
+    return cudaGetLastError();
+}
+
+cudaError_t qld_launch_fixed_from_doubles(const double *tab, int n, int k, int32_t *rfix, int n_stride, cudaStream_t st)
+{
+    k_fixed_from_doubles<<<(n + 255) / 256, 256, 0, st>>>(tab, n, k, rfix, n_stride);
     return cudaGetLastError();
 }
 

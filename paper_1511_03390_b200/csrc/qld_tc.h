@@ -13,12 +13,17 @@ struct TcParams {
     const int8_t *digits;     // digit tiles, see k_digit_pack
     int64_t *sums_out;        // optional [2K][HW] exact fixed-point sums (Q30 references)
     unsigned int *tile_counter; // device counter for the dynamic tile scheduler, zeroed by the launcher
+    int32_t force_T, force_stages, force_kc;   // debug override of the tile shape (qld_debug_set_tile), 0 = automatic
+    int32_t reserved;
     FinParams fin;
 };
 
 int qld_tc_columns(int K);                       // N columns of the MMA: 8 per reference, padded to 16
 size_t qld_tc_digit_bytes(int K, int N);
-cudaError_t qld_tc_encode_tmap(void *tmaps_out /*2 x 128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms);
+cudaError_t qld_tc_encode_tmap(void *tmaps_out /*2 x 128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms,
+                               const int *force /* {T, stages, kc} or zeros */);
 cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st);
+// rfix rows (2k, 2k+1) = rint(2^30 * tab[2][n]) from caller-supplied doubles
+cudaError_t qld_launch_fixed_from_doubles(const double *tab, int n, int k, int32_t *rfix, int n_stride, cudaStream_t st);
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);

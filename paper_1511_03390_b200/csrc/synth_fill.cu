@@ -56,7 +56,8 @@ extern "C" int qld_synth_fill(const qld_synth_scene *scene, int64_t s_first, int
     if (!scene || !out_device || n_frames < 1 || scene->H < 1 || scene->W < 1 || scene->n_terms < 0 || scene->n_terms > 8) return QLD_E_INVAL;
     const int64_t total = (int64_t)scene->H * scene->W * n_frames;
     const int64_t blocks = (total + 255) / 256;
-    const unsigned grid = (unsigned)(blocks < 148 * 32 ? blocks : 148 * 32);
+    const int64_t cap = (int64_t)qld_sm_count() * 32;
+    const unsigned grid = (unsigned)(blocks < cap ? blocks : cap);
     k_synth_fill<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(*scene, s_first, n_frames, out_device);
     return cudaGetLastError() == cudaSuccess ? QLD_OK : QLD_E_CUDA;
 }

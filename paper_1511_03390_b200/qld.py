@@ -25,8 +25,8 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 
 # every symbol include/qld.h declares (tests check that the library exports each of them)
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
-           "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table",
-           "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel",
+           "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table", "qld_set_ref_tables",
+           "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel", "qld_debug_set_tile",
            "qld_cnr", "qld_dominant_bin", "qld_display_map", "qld_synth_fill"]
 
 
@@ -39,7 +39,7 @@ class qld_config(C.Structure):
     _fields_ = [("H", C.c_int32), ("W", C.c_int32), ("dtype", C.c_int32), ("N", C.c_int32), ("K", C.c_int32),
                 ("refs", C.POINTER(qld_ref)), ("ring_frames", C.c_int32), ("accum", C.c_int32), ("norm", C.c_int32),
                 ("maps", C.c_int32), ("max_value", C.c_uint32), ("resync_hops", C.c_int32), ("external_store", C.c_int32),
-                ("slide_hop", C.c_int32), ("reserved2", C.c_int32),
+                ("slide_hop", C.c_int32), ("ref_tables_supplied", C.c_int32),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("compute_stream", C.c_void_p), ("copy_stream", C.c_void_p)]
 
@@ -84,6 +84,7 @@ def load_library():
     l.qld_get_bins.argtypes = [vp, i, pf, C.POINTER(C.c_int)]
     l.qld_read_map.argtypes = [vp, i, i, vp]
     l.qld_read_ref_table.argtypes = [vp, i, i64, i, vp, vp]
+    l.qld_set_ref_tables.argtypes = [vp, i, vp, vp, i64]
     l.qld_set_ref_table_fixed.argtypes = [vp, i, vp, vp, i]
     l.qld_read_ref_table_fixed.argtypes = [vp, i, vp, vp]
     l.qld_get_sums_i64.argtypes = [vp, i, pf, pf]
@@ -99,6 +100,7 @@ def load_library():
     l.qld_accum_mode.argtypes = [vp]
     l.qld_last_kernel.argtypes = [vp]
     l.qld_last_kernel.restype = C.c_char_p
+    l.qld_debug_set_tile.argtypes = [vp, i, i, i, i]
     l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
     l.qld_dominant_bin.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
     l.qld_display_map.argtypes = [vp, C.c_int64, vp, vp, vp, vp]
@@ -124,7 +126,8 @@ class QLD:
     def __init__(self, H: int, W: int, dtype, N: int, refs: Sequence[dict], ring_frames: int = 0,
                  accum: int = QLD_ACC_AUTO, norm: int = QLD_NORM_PAPER, maps: int = QLD_MAP_ALL, max_value: int = 0,
                  resync_hops: int = 0, device=None, copy_stream=None, torch_workspace: bool = True,
-                 external_store: bool = False, slide_hop: int = 0):
+                 external_store: bool = False, slide_hop: int = 0, debug_tile=None,
+                 ref_tables_supplied: bool = False):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -137,6 +140,7 @@ class QLD:
         cfg.ring_frames, cfg.accum, cfg.norm, cfg.maps = int(ring_frames), int(accum), int(norm), int(maps)
         cfg.max_value, cfg.resync_hops, cfg.external_store = int(max_value), int(resync_hops), int(bool(external_store))
         cfg.slide_hop = int(slide_hop)
+        cfg.ref_tables_supplied = int(bool(ref_tables_supplied))
         self._ctx = C.c_void_p()
         nbytes = C.c_size_t()
         rc = self.lib.qld_workspace_bytes(C.byref(cfg), C.byref(nbytes))
@@ -164,6 +168,8 @@ class QLD:
             rc = self.lib.qld_create(C.byref(cfg), C.byref(self._ctx))   # fails loudly: QLD_E_CUDA
         if rc != QLD_OK:
             raise QLDError(rc, self.lib.qld_last_error(None).decode())
+        if debug_tile:
+            self.debug_set_tile(*debug_tile)
 
     # -- helpers -------------------------------------------------------------------------------
     def _check(self, rc: int):
@@ -243,6 +249,13 @@ class QLD:
         self._check(self.lib.qld_read_ref_table(self._ctx, int(k), int(s_first), int(n), sn.ctypes.data, cs.ctypes.data))
         return sn, cs
 
+    def set_ref_tables(self, k: int, sin_tab, cos_tab) -> None:
+        import numpy as np
+        a = np.ascontiguousarray(sin_tab, dtype=np.float64)
+        b = np.ascontiguousarray(cos_tab, dtype=np.float64)
+        assert a.size == b.size
+        self._check(self.lib.qld_set_ref_tables(self._ctx, int(k), a.ctypes.data, b.ctypes.data, int(a.size)))
+
     def set_ref_table_fixed(self, k: int, sin_q30, cos_q30) -> None:
         import numpy as np
         a = np.ascontiguousarray(sin_q30, dtype=np.int32)
@@ -280,6 +293,11 @@ class QLD:
 
     def accum_name(self) -> str:
         return {QLD_ACC_FP32: "FP32", QLD_ACC_INT_BINS: "INT_BINS", QLD_ACC_FIXED: "FIXED"}[self.accum_mode()]
+
+    def debug_set_tile(self, which, a: int = 0, b: int = 0, c: int = 0) -> None:
+        """qld_debug_set_tile: which = "stream" (SEG, KC) or "tc" (T, STAGES, KC)."""
+        w = {"stream": 0, "tc": 1}.get(which, which)
+        self._check(self.lib.qld_debug_set_tile(self._ctx, int(w), int(a), int(b), int(c)))
 
     def last_kernel(self) -> str:
         return self.lib.qld_last_kernel(self._ctx).decode()

@@ -50,6 +50,13 @@ def test_argument_validation_without_gpu(lib):
     assert lib.qld_workspace_bytes(C.byref(_cfg(qld, accum=qld.QLD_ACC_INT_BINS)), C.byref(n)) == qld.QLD_E_UNSUPPORTED
     big = _cfg(qld, refs=[{"num": 1, "den": 4}], N=200000, accum=qld.QLD_ACC_INT_BINS)
     assert lib.qld_workspace_bytes(C.byref(big), C.byref(n)) == qld.QLD_E_UNSUPPORTED
+    # caller-supplied tables lift the nu check (reading G18) but not on rings / integer bins
+    assert lib.qld_workspace_bytes(C.byref(_cfg(qld, refs=[{"nu": 0.5}], ref_tables_supplied=1)), C.byref(n)) == qld.QLD_OK
+    assert lib.qld_workspace_bytes(C.byref(_cfg(qld, refs=[{"nu": 0.0}], ref_tables_supplied=1)), C.byref(n)) == qld.QLD_OK
+    assert lib.qld_workspace_bytes(C.byref(_cfg(qld, ref_tables_supplied=1, ring_frames=40)), C.byref(n)) == qld.QLD_E_UNSUPPORTED
+    assert lib.qld_workspace_bytes(C.byref(_cfg(qld, ref_tables_supplied=1, accum=qld.QLD_ACC_INT_BINS)), C.byref(n)) == qld.QLD_E_UNSUPPORTED
+    assert lib.qld_workspace_bytes(C.byref(_cfg(qld, ref_tables_supplied=2)), C.byref(n)) == qld.QLD_E_INVAL
+    assert lib.qld_set_ref_tables(None, 0, None, None, 0) == qld.QLD_E_INVAL and lib.qld_debug_set_tile(None, 0, 0, 0, 0) == qld.QLD_E_INVAL
     ok = _cfg(qld, refs=[{"num": 1, "den": 4}], N=200000, accum=qld.QLD_ACC_INT_BINS, max_value=4095)
     assert lib.qld_workspace_bytes(C.byref(ok), C.byref(n)) == qld.QLD_OK
 

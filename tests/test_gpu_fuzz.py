@@ -6,7 +6,7 @@ import os
 import numpy as np
 import pytest
 
-from _parity import check_float_maps, oracle_maps
+from _parity import check_float_maps, forced, oracle_maps
 
 pytestmark = pytest.mark.gpu
 
@@ -43,16 +43,15 @@ def _case(seed):
 
 
 @pytest.mark.parametrize("seed", range(120))
-def test_random_configuration(Q, oracle, monkeypatch, seed):
+def test_random_configuration(Q, oracle, seed):
     rng, dtype, H, W, N, K, kind, refs, tile = _case(seed)
-    if tile:
-        monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     hi = 256 if dtype == np.uint8 else int(rng.choice([4096, 65536]))
     x = rng.integers(0, hi, size=(N, H, W)).astype(dtype) if rng.random() < 0.5 else \
         np.clip(rng.normal(hi / 3, hi / 40, size=(N, H, W)), 0, hi - 1).astype(dtype)
     accum = {"fp32": Q.QLD_ACC_FP32, "bins": Q.QLD_ACC_INT_BINS, "fixed": Q.QLD_ACC_FIXED, "auto": Q.QLD_ACC_AUTO}[kind]
     try:
-        ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=accum, max_value=hi - 1)
+        ctx = mk(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=accum, max_value=hi - 1)
     except Q.QLDError as e:
         # the only legitimate refusals: bins with too many rows / an int32 bound, fixed point on a frame that is not
         # a multiple of 16 bytes
@@ -73,11 +72,10 @@ def test_random_configuration(Q, oracle, monkeypatch, seed):
 
 
 @pytest.mark.parametrize("seed", range(40))
-def test_random_sliding(Q, oracle, monkeypatch, seed):
+def test_random_sliding(Q, oracle, seed):
     rng = np.random.default_rng(5000 + seed)
     tile = rng.choice(["512,16", "1024,16", "2048,16", "1024,32", ""])
-    if tile:
-        monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     H, W = int(rng.choice([4, 9, 16])), int(rng.choice([16, 64, 128, 136]))
     hop = int(rng.choice([1, 3, 8, 16, 24, 32, 64]))
     N = hop * int(rng.integers(1, 5)) if rng.random() < 0.6 else int(rng.integers(max(hop, 2), 160))
@@ -90,7 +88,7 @@ def test_random_sliding(Q, oracle, monkeypatch, seed):
     ref = {"num": 1, "den": int(rng.choice([4, 6, 8]))} if kind == "bins" else {"nu": float(rng.uniform(0.02, 0.48)), "phase": 0.3}
     stream = np.clip(rng.normal(1500, 60, size=(T, H, W)), 0, 4095).astype(np.uint16)
     try:
-        ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_INT_BINS if kind == "bins" else Q.QLD_ACC_FP32, max_value=4095,
+        ctx = mk(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_INT_BINS if kind == "bins" else Q.QLD_ACC_FP32, max_value=4095,
                     slide_hop=hop if partial else 0)
         ctx.push_frames(stream[:N])
         ctx.demod(Q.QLD_SLIDE, hop)

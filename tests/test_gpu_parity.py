@@ -6,7 +6,7 @@ map median).  Every call goes through paper_1511_03390_b2
 import numpy as np
 import pytest
 
-from _parity import check_float_maps, oracle_maps
+from _parity import check_float_maps, forced, oracle_maps
 
 pytestmark = pytest.mark.gpu
 
@@ -110,6 +110,47 @@ def test_normalisation_and_map_selection(Q, oracle):
     assert I is None and Qm is None and P is None
     check_float_maps((None, None, A, None), oracle_maps(oracle, x, ref, scale=2.0 / N))
     ctx.destroy()
+
+
+@pytest.mark.parametrize("accum_name", ["FP32", "FIXED"])
+@pytest.mark.parametrize("H,W,N,dtype", [(16, 64, 64, np.uint16), (7, 24, 33, np.uint8), (128, 320, 48, np.uint16)])
+def test_supplied_reference_tables(Q, oracle, accum_name, H, W, N, dtype):
+    """qld_set_ref_tables ("creates tables of sine and cosine functions"): nu = 1/2, nu = 0 (reading G18) and an
+    arbitrary table; the sums are the definition on whatever the arrays hold."""
+    rng = np.random.default_rng(N)
+    x = _rand_stack(rng, N, H, W, dtype, hi=256 if dtype == np.uint8 else 65536)
+    s = np.arange(1, N + 1)
+    tabs = [(np.zeros(N), np.where(s % 2 == 0, 1.0, -1.0)),                 # nu = 1/2
+            (np.zeros(N), np.ones(N)),                                       # nu = 0: Q = sum x
+            (np.sin(0.61 * s + 0.2) * np.hanning(N + 2)[1:-1], np.cos(0.61 * s + 0.2) * np.hanning(N + 2)[1:-1])]   # a windowed reference
+    refs = [{"nu": 0.5}, {"nu": 0.0}, {"nu": 0.3}]
+    try:
+        ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=getattr(Q, "QLD_ACC_" + accum_name), ref_tables_supplied=True)
+    except Q.QLDError as e:
+        assert accum_name == "FIXED" and e.status == Q.QLD_E_UNSUPPORTED and (H * W * x.itemsize) % 16 != 0
+        return
+    ctx.push_frames(x)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.demod()                                            # tables missing
+    assert e.value.status == Q.QLD_E_STATE
+    for k, (sn, cs) in enumerate(tabs):
+        ctx.set_ref_tables(k, sn, cs)
+    with pytest.raises(Q.QLDError) as e:
+        ctx.set_ref_tables(0, np.full(N, 1.5), np.zeros(N))
+    assert e.value.status == Q.QLD_E_INVAL
+    ctx.demod()
+    ctx.sync()
+    for k, (sn, cs) in enumerate(tabs):
+        I, Qo = oracle.demod(x, sn, cs, nthreads=oracle.max_threads())
+        R, ph = oracle.finalise(I, Qo)
+        check_float_maps(_maps(ctx, k), (I, Qo, R, ph), rel=1e-5 if accum_name == "FP32" else 1e-6, what=f"supplied tables k={k}")
+    if accum_name == "FP32":
+        Qsum = _maps(ctx, 1)[1]
+        assert np.array_equal(Qsum, x.astype(np.float64).sum(axis=0).astype(np.float32))      # nu = 0: the plain sum, exact below 2^24... rounded once
+    ctx.destroy()
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(H, W, "u16", N, [{"nu": 0.5}])                   # without tables nu = 1/2 stays rejected
+    assert e.value.status == Q.QLD_E_INVAL
 
 
 def test_closed_form_tone_on_gpu(Q):
@@ -302,20 +343,20 @@ def test_device_generator_is_bit_identical_to_numpy(Q):
 
 
 # ------------------------------------------------------------------------------------------------ TMA-fed kernel
-# k_demod_stream takes over for large frames; QLD_STREAM_TILE = "SEG,KC" forces it (and its tile shape) on small ones.
+# k_demod_stream takes over for large frames; qld_debug_set_tile(SEG, KC) forces it (and its tile shape) on small ones.
 STREAM_TILES = ["512,16", "1024,16", "2048,16", "2048,32", "256,32", "1024,64"]
 
 
 @pytest.mark.parametrize("tile", STREAM_TILES)
 @pytest.mark.parametrize("H,W,N,dtype", [(16, 200, 70, np.uint16), (9, 136, 16, np.uint16), (50, 128, 9, np.uint8), (37, 48, 129, np.uint16),
                                          (25, 64, 3, np.uint16), (33, 256, 100, np.uint8), (128, 320, 40, np.uint16)])
-def test_stream_kernel_fp32_tiles(Q, oracle, monkeypatch, tile, H, W, N, dtype):
+def test_stream_kernel_fp32_tiles(Q, oracle, tile, H, W, N, dtype):
     """Every tile shape (column groups x time slices), ragged last tile, ragged last stage, fewer frames than a stage."""
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(H + W + N)
     x = _rand_stack(rng, N, H, W, dtype)
     ref = {"nu": 0.0937, "phase": 0.3}
-    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+    ctx = mk(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FP32)
     ctx.push_frames(x)
     ctx.demod(Q.QLD_WHOLE)
     ctx.demod(Q.QLD_WHOLE)             # second launch: cached tensor map, tile counter reset
@@ -327,13 +368,13 @@ def test_stream_kernel_fp32_tiles(Q, oracle, monkeypatch, tile, H, W, N, dtype):
 @pytest.mark.parametrize("tile", ["512,16", "2048,16"])
 @pytest.mark.parametrize("K", [2, 3, 8])
 @pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
-def test_stream_kernel_multi_reference(Q, oracle, monkeypatch, tile, K, dtype):
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+def test_stream_kernel_multi_reference(Q, oracle, tile, K, dtype):
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(K)
     H, W, N = 24, 256, 130
     x = _rand_stack(rng, N, H, W, dtype)
     refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
-    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FP32)
+    ctx = mk(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FP32)
     ctx.push_frames(x)
     ctx.demod(Q.QLD_WHOLE)
     ctx.sync()
@@ -344,15 +385,15 @@ def test_stream_kernel_multi_reference(Q, oracle, monkeypatch, tile, K, dtype):
 
 @pytest.mark.parametrize("tile", ["512,16", "2048,16", "1024,32"])
 @pytest.mark.parametrize("den,dtype", [(4, np.uint8), (6, np.uint16), (8, np.uint8), (5, np.uint16), (16, np.uint16)])
-def test_stream_kernel_integer_bins_bit_exact(Q, oracle, monkeypatch, tile, den, dtype):
+def test_stream_kernel_integer_bins_bit_exact(Q, oracle, tile, den, dtype):
     """A3' through the TMA-fed kernel: int32 phase bins bit-exact against the int64 oracle."""
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(den)
     H, W, N = 20, 192, 150
     hi = 256 if dtype == np.uint8 else 65536
     x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
     ref = {"num": 1, "den": den}
-    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_INT_BINS)
+    ctx = mk(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_INT_BINS)
     ctx.push_frames(x)
     ctx.demod(Q.QLD_WHOLE)
     ctx.sync()
@@ -368,15 +409,15 @@ def test_stream_kernel_integer_bins_bit_exact(Q, oracle, monkeypatch, tile, den,
 
 
 @pytest.mark.parametrize("tile", ["512,16", "2048,16"])
-def test_stream_kernel_ring_wraparound(Q, oracle, monkeypatch, tile):
+def test_stream_kernel_ring_wraparound(Q, oracle, tile):
     """QLD_WHOLE on a ring whose window straddles the wrap: two runs of slots, weights by absolute frame index."""
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(7)
     H, W, N, cap = 16, 128, 40, 56
     total = 152
     x = _rand_stack(rng, total, H, W, np.uint16)
     ref = {"nu": 0.0937, "phase": 0.3}
-    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_FP32)
+    ctx = mk(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_FP32)
     pushed = 0
     for b in (40, 8, 16, 8, 16, 16, 16, 16, 16):
         ctx.push_frames(x[pushed:pushed + b])
@@ -392,14 +433,14 @@ def test_stream_kernel_ring_wraparound(Q, oracle, monkeypatch, tile):
 @pytest.mark.parametrize("accum_name,ref", [("INT_BINS", {"num": 1, "den": 6}), ("FP32", {"num": 1, "den": 6}), ("FP32", {"nu": 0.0937, "phase": 0.3}),
                                             ("INT_BINS", {"num": 1, "den": 4})])
 @pytest.mark.parametrize("hop,cap", [(32, 170), (40, 173), (64, 192)])
-def test_stream_kernel_sliding_update(Q, oracle, monkeypatch, tile, accum_name, ref, hop, cap):
+def test_stream_kernel_sliding_update(Q, oracle, tile, accum_name, ref, hop, cap):
     """A5 through the TMA-fed kernel: runs {expired, -w} + {new, +w} added to the stored accumulators; hops that are
     and are not multiples of a stage, expired and new runs that wrap around the ring; bins bit-exact at every hop."""
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(hop + cap)
     H, W, N, T = 12, 128, 96, 96 + 9 * hop
     stream = _rand_stack(rng, T, H, W, np.uint16)
-    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095)
+    ctx = mk(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095)
     ctx.push_frames(stream[:N])
     ctx.demod(Q.QLD_SLIDE, hop)
     for w in range(0, (T - N) // hop + 1):
@@ -423,14 +464,14 @@ def test_stream_kernel_sliding_update(Q, oracle, monkeypatch, tile, accum_name, 
 @pytest.mark.parametrize("tile", ["512,16", "2048,16", "1024,32"])
 @pytest.mark.parametrize("accum_name,ref", [("INT_BINS", {"num": 1, "den": 6}), ("FP32", {"nu": 0.0937, "phase": 0.3}), ("INT_BINS", {"num": 3, "den": 8})])
 @pytest.mark.parametrize("hop,cap", [(32, 170), (64, 200)])
-def test_block_partial_sliding(Q, oracle, monkeypatch, tile, accum_name, ref, hop, cap):
+def test_block_partial_sliding(Q, oracle, tile, accum_name, ref, hop, cap):
     """8(f3): slide_hop > 0 keeps the per-batch partial sums and reads only the new frames; every window equals the
     oracle's direct recomputation (bins bit-exact), through ring wrap-around and more hops than partial slots."""
-    monkeypatch.setenv("QLD_STREAM_TILE", tile)
+    mk = forced(Q, "stream", tile)
     rng = np.random.default_rng(hop + cap)
     H, W, N, T = 12, 128, 128, 128 + 9 * hop
     stream = _rand_stack(rng, T, H, W, np.uint16)
-    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095, slide_hop=hop,
+    ctx = mk(H, W, "u16", N, [ref], ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095, slide_hop=hop,
                 resync_hops=5 if accum_name == "FP32" else 0)
     ctx.push_frames(stream[:N])
     ctx.demod(Q.QLD_SLIDE, hop)

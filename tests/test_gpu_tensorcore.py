@@ -3,7 +3,7 @@ Q1.30 reference table (bit-exact), and the float maps against the fp64 definitio
 import numpy as np
 import pytest
 
-from _parity import check_float_maps, oracle_maps
+from _parity import check_float_maps, forced, oracle_maps
 
 pytestmark = pytest.mark.gpu
 
@@ -87,17 +87,17 @@ def test_fixed_multi_reference(Q, oracle, K, dtype):
 @pytest.mark.parametrize("tile", ["16,3,32", "8,6,32", "4,6,64", "2,8,64", "1,8,32"])
 @pytest.mark.parametrize("H,W,N,dtype", [(16, 200, 70, np.uint16), (16, 200, 64, np.uint16), (50, 128, 9, np.uint8), (37, 48, 129, np.uint16),
                                          (25, 64, 7, np.uint16), (33, 256, 100, np.uint8)])
-def test_fixed_tile_shapes_bit_exact(Q, oracle, monkeypatch, tile, H, W, N, dtype):
+def test_fixed_tile_shapes_bit_exact(Q, oracle, tile, H, W, N, dtype):
     """Every tile shape the launcher can pick (T spans x KC frames per stage), forced through the tuning override, on
     stacks with a ragged last tile, a ragged last 8-frame group, fewer than 8 frames, and a row pitch that is not a
     multiple of 128 bytes (the 1 KB-box path): bit-exact int64 sums."""
-    monkeypatch.setenv("QLD_TC_TILE", tile)
+    mk = forced(Q, "tc", tile)
     rng = np.random.default_rng(H + W + N)
     hi = 256 if dtype == np.uint8 else 65536
     x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
     refs = [{"nu": 0.0937, "phase": 0.3}, {"num": 1, "den": 6}]
     tabs = [_q30(oracle, r, N) for r in refs]
-    ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
+    ctx = mk(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
     for k in range(2):
         ctx.set_ref_table_fixed(k, *tabs[k])
     ctx.push_frames(x)

@@ -244,6 +244,24 @@ def test_degenerate_cases(oracle):
     assert not I.any() and not Q.any()
 
 
+def test_supplied_tables_half_rate_and_dc(oracle):
+    """Reading G18: with caller-supplied tables the definition is computed whatever the arrays hold.  nu = 1/2: sin(pi s) = 0,
+    cos(pi s) = (-1)^s, so a source A sin(pi s + phi) = A (-1)^s sin phi gives I = 0, Q = A N sin phi, R = A N |sin phi| --
+    phase immunity is lost (why qld_create rejects nu = 1/2 without tables).  nu = 0: sin = 0, cos = 1: Q = sum x."""
+    N, A = 64, 3.0
+    s = np.arange(1, N + 1)
+    alt = np.where(s % 2 == 0, 1.0, -1.0)
+    for phi in (0.0, 0.4, 1.3, -2.0):
+        x = (A * alt * math.sin(phi))[:, None]
+        I, Q = oracle.demod(x, np.zeros(N), alt)
+        R, _ = oracle.finalise(I, Q)
+        assert I[0] == 0.0 and abs(Q[0] - A * N * math.sin(phi)) < 1e-12 and abs(R[0] - A * N * abs(math.sin(phi))) < 1e-12
+    rng = np.random.default_rng(0)
+    xi = rng.integers(0, 4096, size=(N, 5)).astype(np.uint16)
+    I, Q = oracle.demod(xi, np.zeros(N), np.ones(N))
+    assert np.array_equal(Q, xi.astype(np.int64).sum(axis=0)) and not I.any()
+
+
 def test_sliding_is_window_by_window_definition(oracle):
     """Window w = absolute frames w*hop+1..w*hop+N, references by absolute index (G10): equals the
     window-relative result rotated by 2 pi nu w hop; amplitude equals the window-relative amplitude."""
