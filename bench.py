@@ -10,8 +10,12 @@ demodulation + A4 finalise (reference tables, A1, were built by qld_create).  St
 batch of `hop` new frames -> qld_commit_frames (A1 table extension + A2 without a copy: frames are resident)
 -> qld_demod(QLD_SLIDE) = A5 update + A4.  `value` has the frames resident in HBM; `e2e` runs the same step
 from pinned host buffers: qld_push_frames (A2), qld_demod, qld_read_map of the amplitude map(s) to the host.
-Prints ONE JSON line (rank 0).  With the default flags at N = 1 the line also carries, under "also", a short
-run of the other large configs (cfg4 on the tensor cores, cfg3 sliding) so one run covers every row of 8(a).
+The headline workload is cfg4 (BASELINE.json configs[4], 17.2 GB, K = 8: the largest single-GPU config).  With the default
+flags at N = 1 the other configs (cfg2, cfg3 sliding, cfg1) are run briefly first and each prints its own compact JSON line
+(marked "also": "<cfg>"); the LAST line is the contract's line for the headline workload, carrying a short summary of the
+others under "also".  `--gpus N` without a torchrun environment re-executes itself under torch.distributed.run with N ranks;
+`--shard rows` makes the ranks split ONE frame into row bands (strong scaling) instead of running one
+independent stack each (weak scaling, the default).
 """
 from __future__ import annotations
 
@@ -78,9 +82,10 @@ class ClockSampler(threading.Thread):
                 "samples": len(s)}
 
 
-def build_workload(name: str, rank: int):
+def build_workload(name: str, rank: int, shard_rows: bool = False):
     from paper_1511_03390_b200 import shard, synth
-    return synth.BUILDERS[name](seed=shard.stream_seed(int(name[3]), rank))   # BASELINE.json seeds: cfgN -> seed N on rank 0
+    # BASELINE.json seeds: cfgN -> seed N on rank 0; row sharding: every rank sees the same frame (same seed)
+    return synth.BUILDERS[name](seed=shard.stream_seed(int(name[3]), 0 if shard_rows else rank))
 
 
 def oracle_on_rows(wl, frames_rows_host, refs, nthreads):
@@ -163,6 +168,13 @@ class Env:
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
         return float(t.item())
 
+    def sum_over_ranks(self, x: float) -> float:
+        if self.dist is None:
+            return x
+        t = self.torch.tensor([x], device=self.dev, dtype=self.torch.float64)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+        return float(t.item())
+
     def timed(self, step, steps: int, warmup: int, keep_busy=None, counter=None):
         """warmup untimed steps, then exactly `steps` steps between CUDA events on the launching stream (torch's
         current stream is the context's compute stream), barrier + synchronize on both sides, max over ranks.
@@ -223,14 +235,26 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     """Whole-window workloads (8(a) rows A1, A3/A3'/A6, A4; A2 in the e2e leg)."""
     torch = env.torch
     from paper_1511_03390_b200 import qld
-    wl = build_workload(workload, env.rank)
+    from paper_1511_03390_b200 import shard
+    shard_rows = args.shard == "rows" and env.world > 1
+    wl = build_workload(workload, env.rank, shard_rows)
     sc = wl.scene
-    N, H, W, K = wl.N, sc.H, sc.W, len(wl.refs)
+    N, H_full, W, K = wl.N, sc.H, sc.W, len(wl.refs)
     b = 1 if sc.dtype == "u8" else 2
     refs = [dict(r) for r in wl.refs]
     accum = ACCUM_NAMES[accum_name]
     # inputs: the synthetic stack, filled on the device, resident before the timed region
-    frames = qld.synth_fill(sc, 1, N, device=env.dev)
+    if shard_rows:
+        # SURVEY.md 8(e): one frame, contiguous row bands, one per rank; this rank keeps only its band of every frame
+        r_lo, r_hi = shard.row_bands(H_full, env.world)[env.rank]
+        H = r_hi - r_lo
+        frames = torch.empty((N, H, W), dtype=torch.uint8 if b == 1 else torch.uint16, device=env.dev)
+        for a in range(0, N, 64):
+            n = min(64, N - a)
+            frames[a:a + n].copy_(qld.synth_fill(sc, a + 1, n, device=env.dev)[:, r_lo:r_hi, :])
+    else:
+        r_lo, H = 0, H_full
+        frames = qld.synth_fill(sc, 1, N, device=env.dev)
     torch.cuda.synchronize()
     # BASELINE.json configs[4] asks for the K amplitude maps only; the other configs produce all four maps
     maps, map_names = (qld.QLD_MAP_AMP, "amplitude") if workload == "cfg4" else (qld.QLD_MAP_ALL, "I,Q,amplitude,phase")
@@ -244,9 +268,11 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     ms, clocks, launches = env.timed(step, steps, warmup, keep_busy=step, counter=ctx.kernel_launches)
     kernel = ctx.last_kernel()
     mode = ctx.accum_name()
-    samples = float(N) * H * W
-    res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
-           "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel}
+    samples = float(N) * H * W                               # this rank's units per step
+    job_samples = env.sum_over_ranks(samples)                # row bands may differ by one row
+    res = {"workload": workload, "value": job_samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
+           "maps_per_s": (1 if shard_rows else env.world) * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel,
+           "scaling": "strong" if shard_rows else "weak"}
     res["gpu_launches"] = int(launches)
     algo = samples * b + n_maps * K * H * W * 4.0            # every sample once + the fp32 maps of every reference
     in_l2 = samples * b <= 126e6
@@ -256,13 +282,14 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": map_names, "step": "qld_demod(QLD_WHOLE) over the resident stack",
                      "cache": f"input {samples * b / 1e6:.0f} MB per step " + ("<= 126 MB L2: L2-resident" if in_l2 else "> 126 MB L2: no flush needed"),
-                     "parallelism": f"{env.world} x independent stacks (pixels are independent; no collective)"}
+                     "parallelism": (f"one {H_full}x{W} frame split into {env.world} row bands, one per rank (pixels are independent; no collective)"
+                                     if shard_rows else f"{env.world} x independent stacks (pixels are independent; no collective)")}
 
     # ---- end to end through host buffers (pinned): push + demod + read amplitude maps back ---------
     if e2e_steps > 0:
-        host = torch.empty((N, H, W), dtype=frames.dtype).pin_memory()
+        host = torch.empty((N, H, W), dtype=frames.dtype, pin_memory=True)
         host.copy_(frames)
-        amp_host = torch.empty((K, H, W), dtype=torch.float32).pin_memory()
+        amp_host = torch.empty((K, H, W), dtype=torch.float32, pin_memory=True)
         torch.cuda.synchronize()
         ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=0, accum=accum, maps=maps, max_value=sc.maxval)
         chunk = max(1, min(N, (256 << 20) // (H * W * b)))       # pushes of about 256 MiB
@@ -283,7 +310,7 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
             e2e_step()
         env.barrier()
         dt = env.max_over_ranks(time.perf_counter() - t0)
-        res["e2e"] = {"value": env.world * samples * e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(samples * b),
+        res["e2e"] = {"value": job_samples * e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(samples * b),
                       "d2h_bytes_per_step": int(K * H * W * 4), "ms_per_step": 1e3 * dt / e2e_steps,
                       "h2d_GBps": samples * b * e2e_steps / dt / 1e9, "steps": e2e_steps,
                       "note": "pinned host stack -> qld_push_frames -> qld_demod -> qld_read_map(amp) -> host"}
@@ -364,16 +391,25 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
            "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel, "gpu_launches": int(launches),
            "window_samples_per_s": env.world * float(N) * H * W * steps / (ms * 1e-3)}
-    # per pixel: hop new + hop expired samples, accumulators read-modify-write, one amplitude map
-    algo = H * W * (2.0 * hop * b + 2.0 * n_rows * acc_bytes + 4.0 * K)
-    moved = H * W * (1.0 * hop * b + 4.0 * n_rows * acc_bytes + 4.0 * K) if slide_hop else algo
-    res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
-                                   f"algorithmic bytes = SURVEY.md 8(a) A5: per pixel 2*hop*{b} B of frames (new + expired) + {n_rows} x {acc_bytes} B "
-                                   f"accumulators read and written + 4 B map; a recompute would read {N * b} B."
-                                   + (f" This run keeps per-batch partial sums (8(f3)) and reads only the new frames: it moves {moved / 1e6:.1f} MB "
-                                      f"per launch ({hop * b} B of frames + 2 x {n_rows} x {acc_bytes} B accumulators and partials read and written + 4 B), "
-                                      f"i.e. {moved / (ms / steps * 1e-3) / 1e9:.0f} GB/s of real traffic" if slide_hop else ""))
+    # Two byte counts per launch (both in the line, both recomputable from it):
+    #  survey_A5: SURVEY.md 8(a)/(d) row A5, the frame re-reading update with two accumulators per pixel:
+    #             2*hop*b (new + expired frames) + 2 x (4 B read + 4 B written) + 4 B map = 148 B per pixel on cfg3;
+    #  moved:     what this run's update really moves.  Block-partial form (8(f3)): hop*b of NEW frames only + n_rows
+    #             accumulators and n_rows expired partials read, both written back + the map.  Re-reading form: 2*hop*b +
+    #             n_rows accumulators read and written + the map.
+    # `achieved` / `frac` use `moved` (never bytes the kernel does not touch); `frac_survey_A5` is the equivalent figure.
+    survey = H * W * (2.0 * hop * b + 16.0 + 4.0 * K)
+    moved = H * W * ((1.0 if slide_hop else 2.0) * hop * b + (4.0 if slide_hop else 2.0) * n_rows * acc_bytes + 4.0 * K)
+    res["roofline"] = roofline_hbm(moved, ms / steps, workload, kernel,
+                                   (f"moved = per pixel {hop * b} B of new frames + {n_rows} x {acc_bytes} B accumulators and as many expired partial sums read, "
+                                    f"both written back + 4 B map (block-partial update, 8(f3)); " if slide_hop else
+                                    f"moved = per pixel 2 x {hop * b} B of frames (new + expired) + {n_rows} x {acc_bytes} B accumulators read and written + 4 B map; ")
+                                   + f"survey_A5 = 2*hop*b + 16 + 4 = {survey / (H * W):.0f} B per pixel (SURVEY.md 8(d)); a recompute would read {N * b} B per pixel")
+    peak = res["roofline"]["peak"]
     res["roofline"]["bytes_moved_per_launch"] = moved
+    res["roofline"]["frac_moved"] = res["roofline"]["frac"]
+    res["roofline"]["survey_A5_bytes_per_launch"] = survey
+    res["roofline"]["frac_survey_A5"] = survey / (ms / steps * 1e-3) / 1e9 / peak
     res["dtype"] = {"INT_BINS": "int32", "FP32": "f32"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "hop": hop, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": "amplitude", "step": "qld_commit_frames(hop) + qld_demod(QLD_SLIDE, hop) over the resident ring",
@@ -389,7 +425,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
         import oracle
         from oracle.check import check_float_maps
         nt = oracle.max_threads()
-        n_win = 4
+        n_win = 6
         rows = max(1, min(H, args.ref_rows or -(-int(15 * 1.4e8 * nt) // (n_win * K * N * W))))
         r0 = H // 2 - rows // 2                               # the moving disk crosses these rows
         pctx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=T, accum=accum, maps=qld.QLD_MAP_ALL, max_value=sc.maxval, external_store=True,
@@ -398,7 +434,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
         pctx.commit_frames(N)
         pctx.demod(qld.QLD_SLIDE, hop)
         last_w = min((T - N) // hop, warmup + steps)
-        check_at = sorted(set([0, 1, last_w // 2, last_w]))[:n_win]
+        check_at = sorted(set(w for w in (0, 1, 15, 16, 17, last_w) if w <= last_w))
         secs, worst, done = 0.0, 0.0, 0
         for w in range(0, last_w + 1):
             if w > 0:
@@ -425,102 +461,168 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     del ring
     torch.cuda.empty_cache()
 
-    # ---- end to end: pinned host batches -> qld_push_frames (ring owned by the library) -> slide -> amp to host
+    # ---- end to end, the stream as BASELINE.json configs[3] states it: every batch of the 16384-frame stream pushed from
+    # pinned host memory (qld_push_frames, copy stream) into a WRAPPING library-owned ring, one slide + one amplitude map
+    # read back per hop.  The timed region covers the whole stream, seeding window included.
     if e2e_steps > 0:
+        import numpy as np
         batch = wl.batch
-        n_rot = 4                                             # rotate over a few pinned batches (the stream is 34 GB)
-        host = torch.empty((n_rot, batch, H, W), dtype=tdt).pin_memory()
+        assert batch == hop, "the e2e leg slides once per pushed batch"
+        n_batches = sc.n_frames // batch
+        full_stream = True
+        try:
+            host = torch.empty((n_batches, batch, H, W), dtype=tdt, pin_memory=True)
+        except Exception:
+            full_stream = False                               # not enough pinnable memory: rotate over a few batches
+            host = torch.empty((4, batch, H, W), dtype=tdt, pin_memory=True)
+        n_rot = host.shape[0]
         for i in range(n_rot):
             host[i].copy_(qld.synth_fill(sc, 1 + i * batch, batch, device=env.dev))
-        amp_host = torch.empty((2, K, H, W), dtype=torch.float32).pin_memory()
-        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=N + hop + 2 * batch, accum=accum, maps=maps, max_value=sc.maxval, slide_hop=slide_hop)
-        for i in range(N // batch):
-            ectx.push_frames(host[i % n_rot])
-        ectx.demod(qld.QLD_SLIDE, hop)
-        ectx.sync()
-        it = [0]
+        torch.cuda.synchronize()
+        ring_frames = N + hop + 2 * batch
+        n_win = (sc.n_frames - N) // hop + 1
+        check_at = [w for w in (0, 1, 15, 16, 17, 255, 495, 496) if w < n_win] if (full_stream and with_cpu and env.rank == 0) else []
+        kept = {w: torch.empty((K, H, W), dtype=torch.float32, pin_memory=True) for w in check_at}
+        amp_host = torch.empty((2, K, H, W), dtype=torch.float32, pin_memory=True)
+        ectx = qld.QLD(H, W, sc.dtype, N, refs, ring_frames=ring_frames, accum=accum, maps=maps, max_value=sc.maxval, slide_hop=slide_hop)
 
-        def e2e_step():
-            i = it[0]
-            it[0] += 1
-            ectx.push_frames(host[i % n_rot])
-            ectx.demod(qld.QLD_SLIDE, hop)
-            for k in range(K):
-                ectx.read_map(k, qld.QLD_MAP_AMP, amp_host[i & 1, k])
-            if i & 1:
-                ectx.sync()                                   # a consumer looks at the maps every other hop
+        def run_stream():
+            ectx.reset()
+            w = 0
+            for i in range(n_batches):
+                ectx.push_frames(host[i % n_rot])
+                if (i + 1) * batch >= N:
+                    ectx.demod(qld.QLD_SLIDE, hop)
+                    dst = kept[w] if w in kept else amp_host[w & 1]
+                    for k in range(K):
+                        ectx.read_map(k, qld.QLD_MAP_AMP, dst[k])
+                    if w & 1:
+                        ectx.sync()                           # a consumer looks at the maps every other hop
+                    w += 1
+            ectx.sync()
+            return w
 
-        for _ in range(4):
-            e2e_step()
-        ectx.sync()
         env.barrier()
-        n = max(e2e_steps, 64)
         t0 = time.perf_counter()
-        for _ in range(n):
-            e2e_step()
-        ectx.sync()
+        n_maps_out = run_stream()
         env.barrier()
         dt = env.max_over_ranks(time.perf_counter() - t0)
-        res["e2e"] = {"value": env.world * samples * n / dt, "unit": UNIT, "h2d_bytes_per_step": int(batch * H * W * b),
-                      "d2h_bytes_per_step": int(K * H * W * 4), "ms_per_step": 1e3 * dt / n, "h2d_GBps": batch * H * W * b * n / dt / 1e9,
-                      "maps_per_s": env.world * K * n / dt, "input_frames_per_s": env.world * hop * n / dt, "steps": n,
-                      "note": "pinned host batch -> qld_push_frames (copy stream) -> qld_demod(QLD_SLIDE) -> qld_read_map(amp) -> host; copies overlap the update"}
+        total = float(sc.n_frames) * H * W
+        res["e2e"] = {"value": env.world * total / dt, "unit": UNIT, "h2d_bytes_per_step": int(batch * H * W * b),
+                      "d2h_bytes_per_step": int(K * H * W * 4), "ms_per_step": 1e3 * dt / n_batches, "h2d_GBps": total * b / dt / 1e9,
+                      "maps_per_s": env.world * K * n_maps_out / dt, "input_frames_per_s": env.world * sc.n_frames / dt, "steps": n_batches,
+                      "maps": n_maps_out, "ring_frames": ring_frames, "stream_frames": sc.n_frames, "seconds": dt,
+                      "host_stream": "the whole stream in pinned memory" if full_stream else f"{n_rot} pinned batches, rotated (same bytes per step)",
+                      "note": "whole stream: pinned host batch -> qld_push_frames (copy stream, wrapping ring) -> qld_demod(QLD_SLIDE) -> "
+                              "qld_read_map(amp) -> host; copies overlap the update; timed region includes the seeding window"}
+        if check_at:
+            import oracle
+            from oracle.check import check_float_maps
+            nt = oracle.max_threads()
+            rows = 8
+            r0 = H // 2 - rows // 2
+            worst = 0.0
+            hs = host.view(n_batches * batch, H, W)
+            for w in check_at:
+                sub = hs[w * hop:w * hop + N, r0:r0 + rows, :].numpy()
+                out = oracle.qld(sub, refs[0], s_first=w * hop + 1, nthreads=nt)
+                got = (None, None, kept[w][0, r0:r0 + rows].numpy(), None)
+                worst = max(worst, check_float_maps(got, out, rel=1e-6 if mode == "INT_BINS" else 1e-5, what=f"e2e stream window {w}"))
+            res["e2e"]["parity"] = {"windows_checked": check_at, "rows_checked": rows, "strict_max_rel_err_amp": worst, "ok": True,
+                                    "note": "amplitude maps of the streamed run (ring wrapped " + str((sc.n_frames - 1) // ring_frames) + " times) vs the oracle's direct recomputation"}
         ectx.destroy()
+        del host
     return res
 
 
 RUNNERS = {"cfg0": bench_whole, "cfg1": bench_whole, "cfg2": bench_whole, "cfg3": bench_slide, "cfg4": bench_whole}
 
 
+def spawn_ranks(n: int):
+    """`python bench.py --gpus N` outside a torchrun environment: re-execute under torch.distributed.run, one rank per GPU."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def compact(r: dict) -> dict:
+    """The short form of a config's result: enough to recompute every fraction from the record alone."""
+    rf = r["roofline"]
+    out = {"value": r["value"], "ms_per_step": r["ms_per_step"], "kernel": r["kernel"], "frac": rf["frac"], "achieved_GBps": rf["achieved"],
+           "peak_GBps": rf["peak"], "bytes_per_launch": rf["algorithmic_bytes_per_launch"]}
+    for k in ("frac_survey_A5", "survey_A5_bytes_per_launch"):
+        if k in rf:
+            out[k] = rf[k]
+    if r.get("parity"):
+        out["parity_ok"] = r["parity"]["ok"]
+    if r.get("e2e"):
+        out["e2e_value"] = r["e2e"]["value"]
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=sorted(RUNNERS))
+    ap.add_argument("--workload", default="cfg4", choices=sorted(RUNNERS))
     ap.add_argument("--accum", default="auto", choices=sorted(ACCUM_NAMES))
-    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--shard", default="stacks", choices=["stacks", "rows"], help="N > 1: 'stacks' = one independent stack / stream per rank "
+                    "(weak scaling); 'rows' = the ranks split ONE frame into contiguous row bands (SURVEY.md 8(e); strong scaling; "
+                    "whole-window workloads)")
     ap.add_argument("--ref-rows", type=int, default=0, help="rows of the frame the CPU oracle is timed / checked on "
                     "(0: sized for about 15 s of oracle work on the host cores; 32 for --impl reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--reread-expired", action="store_true", help="cfg3: update the window by re-reading the expired frames "
                     "(SURVEY.md 8(a) A5 as literally stated) instead of keeping per-batch partial sums (8(f3), cfg.slide_hop: "
                     "identical results, fewer bytes, and the faster of the two on B200: the default)")
-    ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly and report under "
-                    "\"also\" (default: cfg4,cfg3,cfg1 when --workload is cfg2 on one GPU; 'none' to skip)")
+    ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly first, one compact JSON line each "
+                    "(default: cfg2,cfg3,cfg1 when --workload is cfg4 on one GPU; 'none' to skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     if args.impl == "reference":
         run_reference(args, int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")))
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args.gpus)                                  # does not return
 
     env = Env(args)
-    main_res = RUNNERS[args.workload](env, args, args.workload, args.accum, args.steps, args.warmup, args.e2e_steps,
-                                      not args.no_cpu_baseline)
-    also = {}
     names = args.also
     if names == "default":
-        names = "cfg4,cfg3,cfg1" if (args.workload == "cfg2" and env.world == 1 and args.accum == "auto") else "none"
+        names = "cfg2,cfg3,cfg1" if (args.workload == "cfg4" and env.world == 1 and args.accum == "auto") else "none"
+    also = {}
     if names != "none":
         for w in [x for x in names.split(",") if x and x != args.workload]:
-            r = RUNNERS[w](env, args, w, "auto", min(args.steps, 50), 3, 0, not args.no_cpu_baseline)
-            also[w] = {k: r[k] for k in ("value", "ms_per_step", "maps_per_s", "kernel", "gpu_launches", "dtype", "roofline", "parity", "cpu_baseline", "clocks") if k in r}
-            also[w]["unit"] = UNIT
-            also[w]["config"] = {k: r["config"][k] for k in ("accum", "step", "cache", "N", "K") if k in r["config"]}
+            r = RUNNERS[w](env, args, w, "auto", min(args.steps, 200) if w != "cfg2" else max(args.steps, 100), 5,
+                           args.e2e_steps if w == "cfg3" else 0, not args.no_cpu_baseline)
+            also[w] = compact(r)
+            if env.rank == 0:
+                line = {"also": w, "metric": METRIC, "unit": UNIT}
+                line.update({k: r[k] for k in ("value", "ms_per_step", "maps_per_s", "window_samples_per_s", "kernel", "gpu_launches", "dtype",
+                                               "config", "roofline", "parity", "cpu_baseline", "e2e", "clocks") if k in r})
+                print(json.dumps(line), flush=True)
 
+    main_res = RUNNERS[args.workload](env, args, args.workload, args.accum, args.steps, args.warmup, args.e2e_steps,
+                                      not args.no_cpu_baseline)
     if env.rank == 0:
         r = main_res
-        line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": env.world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": r["dtype"], "data": "synthetic", "config": r["config"], "maps_per_s": r["maps_per_s"],
-                "roofline": r["roofline"], "cpu_baseline": r.get("cpu_baseline"), "e2e": r.get("e2e"),
-                "gpu_launches": r["gpu_launches"], "clocks": r["clocks"], "parity": r.get("parity")}
+        line = {}
+        if also:
+            line["also"] = also                                  # summaries first: the headline keys close the line
+        line.update({"maps_per_s": r["maps_per_s"], "parity": r.get("parity"), "clocks": r["clocks"], "cpu_baseline": r.get("cpu_baseline"),
+                     "e2e": r.get("e2e"), "roofline": r["roofline"], "gpu_launches": r["gpu_launches"], "config": r["config"],
+                     "data": "synthetic", "dtype": r["dtype"], "vs_baseline": None, "scaling": r.get("scaling", "weak"),
+                     "higher_is_better": True, "ms_per_step": r["ms_per_step"], "warmup": args.warmup, "steps": args.steps,
+                     "n_gpus": env.world, "unit": UNIT, "value": r["value"], "metric": METRIC})
         if "window_samples_per_s" in r:
             line["window_samples_per_s"] = r["window_samples_per_s"]
-        if also:
-            line["also"] = also
         print(json.dumps(line), flush=True)
     if env.dist is not None:
         env.dist.destroy_process_group()

@@ -141,8 +141,11 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
 
 // ---------------------------------------------------------------------------------------------------
 // A5: sliding-window update.  acc += sum over the hop new frames - sum over the hop expired frames, each
-// partial computed from zero in frame order (so the partial a batch adds is bit-identical to the partial
-// it later removes), accumulators fp64 (FP32 mode) or int32 (bins, exact).  One thread = V pixels.
+// partial computed from zero in frame order, accumulators fp64 (FP32 mode) or int32 (bins, exact).  With a
+// constant hop the fp32 partial a batch adds here is the one this kernel later removes, but the seed comes from
+// another kernel with another time slicing, and k_demod_stream folds -expired and +new into one fp32 sum: FP32
+// ring sums therefore drift (a random walk of rounding errors) and qld_demod resynchronises them from the ring
+// every cfg.resync_hops hops (default: every 16 windows' worth).  One thread = V pixels.
 // ---------------------------------------------------------------------------------------------------
 template <typename T, typename ACC, int ROWS, int V>
 __device__ __forceinline__ void hop_partial(const unsigned char *base, int64_t stride, int cap, int slot, const ACC *wtab, int cap_w,

@@ -115,3 +115,132 @@ def test_sliding_full_size_sampled(Q, oracle, accum_name, slide_hop):
                 rows = ctx.get_bins(0).reshape(3, -1)[:, torch.from_numpy(pix).cuda()].cpu().numpy()
                 assert np.array_equal(rows.reshape(3, 1, -1), B[:3] - B[3:]), f"window {w}"
     ctx.destroy()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Full maps (not samples) at BASELINE.json's sizes, in the configuration bench.py times
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name,rows", [("cfg1", 0), ("cfg2", 0), ("cfg4", 1024)])
+def test_whole_window_full_maps(Q, oracle, name, rows):
+    """cfg1 / cfg2: every pixel of every map against the oracle; cfg4 (8 references, 17 GB): the first `rows` rows of all
+    8 x 4 maps.  Accumulation = AUTO, as bench.py runs them (bins / fp32 / tcgen05 fixed point)."""
+    import torch
+    from paper_1511_03390_b200 import synth
+    wl = synth.BUILDERS[name]()
+    sc, N, K = wl.scene, wl.N, len(wl.refs)
+    refs = [dict(r) for r in wl.refs]
+    frames = Q.synth_fill(sc, 1, N)
+    ctx = Q.QLD(sc.H, sc.W, sc.dtype, N, refs, ring_frames=-1, accum=Q.QLD_ACC_AUTO, max_value=sc.maxval)
+    ctx.attach_frames_device(frames)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    mode = ctx.accum_name()
+    rows = rows or sc.H
+    x = frames[:, :rows, :].contiguous().cpu().numpy()
+    nt = oracle.max_threads()
+    for k in range(K):
+        ora = oracle.qld(x, refs[k], nthreads=nt)
+        got = tuple(m[:rows].cpu().numpy() for m in ctx.get_maps(k))
+        check_float_maps(got, ora, rel=1e-5 if mode == "FP32" else 1e-6, what=f"{name} {mode} full maps k={k}")
+    if mode == "INT_BINS":
+        den = refs[0]["den"]
+        B = oracle.bins(x, refs[0]["num"], den)
+        assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:den // 2] - B[den // 2:])
+    ctx.destroy()
+    del frames
+    torch.cuda.empty_cache()
+
+
+CFG3_FULL_WINDOWS = (0, 1, 15, 16, 17, 255, 495, 496)      # SURVEY.md 8(d): straddle the ring's wrap-arounds
+
+
+def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, tile_every, curve_path=None):
+    """BASELINE.json configs[3] as stated: all 16384 frames, 32-frame batches from pinned host buffers (qld_push_frames)
+    into a wrapping library-owned ring, one slide per batch, 497 maps.  Full maps at `full_windows` and a 128 x 128 tile on
+    the path of the moving disk at every `tile_every`-th window are compared with the oracle's direct recomputation."""
+    import torch
+    from paper_1511_03390_b200 import synth
+    wl = synth.cfg3()
+    sc, N, hop, batch = wl.scene, wl.N, wl.hop, wl.batch
+    H, W = sc.H, sc.W
+    ring_frames = N + hop + 2 * batch
+    ctx = Q.QLD(H, W, sc.dtype, N, [ref], ring_frames=ring_frames, accum=accum, max_value=sc.maxval, slide_hop=slide_hop,
+                resync_hops=resync_hops)
+    n_batches = sc.n_frames // batch
+    n_win = (sc.n_frames - N) // hop + 1
+    assert n_win == 497 and ring_frames < sc.n_frames // 8        # the ring wraps many times
+    pinned = [torch.empty((batch, H, W), dtype=torch.uint16, pin_memory=True) for _ in range(4)]
+    y0, x0 = H // 2 - 64, 300
+    tile = np.empty((sc.n_frames, 128, 128), dtype=np.uint16)
+    keep = {}                                                     # window -> (I, Q, amp, phase[, bins]) on the host
+    is_int = None
+    nt = oracle.max_threads()
+    w = 0
+    for i in range(n_batches):
+        dev = Q.synth_fill(sc, 1 + i * batch, batch)
+        buf = pinned[i % 4]
+        if i >= 4:
+            ctx.push_done(block=True)                             # the copy that read this buffer four pushes ago is done
+        buf.copy_(dev)
+        tile[i * batch:(i + 1) * batch] = buf[:, y0:y0 + 128, x0:x0 + 128].numpy()
+        ctx.push_frames(buf)
+        if (i + 1) * batch >= N:
+            ctx.demod(Q.QLD_SLIDE, hop)
+            if is_int is None:
+                is_int = ctx.accum_name() == "INT_BINS"
+            if w in full_windows or w % tile_every == 0:
+                ctx.sync()
+                maps = ctx.get_maps(0)
+                if w in full_windows:
+                    keep[w] = [m.cpu().numpy() for m in maps] + ([ctx.get_bins(0).cpu().numpy()] if is_int else [])
+                else:
+                    keep[w] = [m[y0:y0 + 128, x0:x0 + 128].cpu().numpy() for m in maps] + \
+                              ([ctx.get_bins(0)[:, y0:y0 + 128, x0:x0 + 128].cpu().numpy()] if is_int else [])
+            w += 1
+    ctx.sync()
+    assert w == n_win and ctx.counters() == (sc.n_frames, n_win)
+    ctx.destroy()
+    rel = 1e-6 if is_int else 1e-5
+    curve = []
+    for ww in sorted(keep):
+        a = ww * hop
+        if ww in full_windows:
+            x = np.concatenate([Q.synth_fill(sc, a + 1 + j, min(128, N - j)).cpu().numpy() for j in range(0, N, 128)])
+            assert np.array_equal(x[:, y0:y0 + 128, x0:x0 + 128], tile[a:a + N])      # the pushed bytes are the generator's
+        else:
+            x = tile[a:a + N]
+        ora = oracle.qld(x, ref, s_first=a + 1, nthreads=nt)
+        strict = check_float_maps(tuple(keep[ww][:4]), ora, rel=rel, what=f"cfg3 stream window {ww}")
+        med = float(np.median(ora[2]))
+        curve.append((ww, float(np.abs(keep[ww][2] - ora[2]).max() / med), strict))
+        if is_int:
+            B = oracle.bins(x, ref["num"], ref["den"], s_first=a + 1)
+            h = ref["den"] // 2
+            assert np.array_equal(keep[ww][4], B[:h] - B[h:]), f"bins of window {ww}"
+    if curve_path:
+        import os
+        os.makedirs(os.path.dirname(curve_path), exist_ok=True)
+        with open(curve_path, "w") as f:
+            f.write("# window  max|amp_gpu - amp_oracle| / median(amp_oracle)  strict_max_rel\n")
+            for c in curve:
+                f.write("%d %.3e %.3e\n" % c)
+    return curve
+
+
+@pytest.mark.parametrize("slide_hop", [32, 0])
+def test_cfg3_full_stream_integer_bins(Q, oracle, slide_hop):
+    """nu = 1/6: exact integer bins; block-partial update (the bench default) and the frame re-reading update."""
+    curve = _stream_cfg3(Q, oracle, {"num": 1, "den": 6}, Q.QLD_ACC_AUTO, slide_hop, 0, CFG3_FULL_WINDOWS, tile_every=1)
+    assert len(curve) == 497
+
+
+@pytest.mark.parametrize("resync_hops", [-1, 64, 0])
+def test_cfg3_full_stream_fp32_drift(Q, oracle, resync_hops):
+    """Float references (nu = 0.0937) over the whole stream: add/subtract drift of the fp32 update stays inside the 1e-5
+    bar for 496 hops without any resynchronisation (-1), with one every 64 hops, and with the default (0 = every 16
+    windows' worth of hops).  The error curve goes to gpurun_out/ (DESIGN.md quotes it)."""
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    curve = _stream_cfg3(Q, oracle, {"nu": 0.0937, "phase": 0.3}, Q.QLD_ACC_FP32, 0, resync_hops, (0, 255, 496), tile_every=8,
+                         curve_path=os.path.join(root, "gpurun_out", f"cfg3_fp32_drift_resync{resync_hops}.txt"))
+    assert max(c[1] for c in curve) <= 1e-5

@@ -67,10 +67,15 @@ def test_reference_tables_deep_in_a_stream(Q, oracle):
 # ------------------------------------------------------------------------------------------------ A3 / A4 / A6
 @pytest.mark.parametrize("H,W", [(1, 1), (3, 17), (17, 3), (64, 64), (5, 48)])
 @pytest.mark.parametrize("N", [1, 2, 5, 63, 64, 65, 200])
-@pytest.mark.parametrize("dtype", [np.uint8, np.uint16])
-def test_whole_window_fp32_shapes(Q, oracle, H, W, N, dtype):
+@pytest.mark.parametrize("dtype,full_range", [(np.uint8, False), (np.uint16, False), (np.uint16, True), (np.uint8, True)])
+def test_whole_window_fp32_shapes(Q, oracle, H, W, N, dtype, full_range):
+    """full_range: samples uniform over 0..65535 (0..255), far from the pedestal (the pixel's first sample): the worst
+    case for the pedestal-subtracted fp32 sums."""
     rng = np.random.default_rng(H * 1000 + W * 10 + N)
-    x = _rand_stack(rng, N, H, W, dtype)
+    if full_range:
+        x = rng.integers(0, 65536 if dtype == np.uint16 else 256, size=(N, H, W)).astype(dtype)
+    else:
+        x = _rand_stack(rng, N, H, W, dtype)
     ref = {"nu": 0.0937, "phase": 0.3}
     ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, [ref], accum=Q.QLD_ACC_FP32)
     ctx.push_frames(x)

@@ -72,3 +72,49 @@ def test_row_bands_properties():
     assert shard.stream_seed(2, 0) == 2 and shard.stream_seed(2, 3) == 3002
     # single-process fall-through: no process group needed
     assert shard.whole_job_rate(10.0, 2.0) == (5.0, 10.0, 2.0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,shape,accum_name", [("cfg2", dict(H=301, W=256, N=96), "FP32"), ("cfg4", dict(H=256, W=512, N=128), "AUTO"),
+                                                   ("cfg1", dict(H=203, W=320, N=64), "AUTO")])
+def test_row_bands_through_libqld_on_one_gpu(name, shape, accum_name):
+    """SURVEY.md 8(e) with the product, not the oracle: world = 2 row bands of one frame, each through its own libqld
+    context on its own stream (what two ranks would run), concatenate to exactly the maps of one whole-frame context --
+    bit for bit, because a pixel's sums depend on that pixel only.  Integer bins and the fixed-point
+    contraction are exact in any order; the fp32 kernel's summation order depends on its tile shape (time slices), which
+    the launcher picks from the frame size, so the FP32 case pins one shape for the three contexts."""
+    import torch
+    assert torch.cuda.is_available(), "needs the B200"
+    from paper_1511_03390_b200 import qld, shard, synth
+    wl = synth.BUILDERS[name](**shape)
+    sc, N, K = wl.scene, wl.N, len(wl.refs)
+    refs = [dict(r) for r in wl.refs]
+    frames = qld.synth_fill(sc, 1, N)
+    accum = getattr(qld, "QLD_ACC_" + accum_name)
+    tile = ("stream", 1024, 16) if accum_name == "FP32" else None
+    whole = qld.QLD(sc.H, sc.W, sc.dtype, N, refs, ring_frames=-1, accum=accum, max_value=sc.maxval, debug_tile=tile)
+    whole.attach_frames_device(frames)
+    whole.demod(qld.QLD_WHOLE)
+    whole.sync()
+    bands = shard.row_bands(sc.H, 2)
+    shard.check_partition(bands, sc.H)
+    parts, keep = [], []
+    for band in bands:
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            sub = shard.band_of(frames, band)
+            ctx = qld.QLD(band[1] - band[0], sc.W, sc.dtype, N, refs, ring_frames=-1, accum=accum, max_value=sc.maxval, debug_tile=tile)
+            ctx.attach_frames_device(sub)
+            ctx.demod(qld.QLD_WHOLE)
+        keep.append((ctx, sub, st))
+    for ctx, _, _ in keep:
+        ctx.sync()
+        assert ctx.accum_mode() == whole.accum_mode()
+        parts.append([torch.stack([m for m in ctx.get_maps(k)]) for k in range(K)])
+    for k in range(K):
+        cat = torch.cat([p[k] for p in parts], dim=-2)
+        ref = torch.stack([m for m in whole.get_maps(k)])
+        assert torch.equal(cat.view(torch.int32), ref.view(torch.int32)), f"{name} k={k}: bands differ from the whole-frame maps"
+    for ctx, _, _ in keep:
+        ctx.destroy()
+    whole.destroy()
