@@ -14,10 +14,12 @@
 // The kernel is HBM-bound for any K <= 8 (N columns = 8K <= 64): per 32-frame MMA step the tensor pipe needs
 // 128*N/256 <= 32 cycles for 4 KB of samples, about five times faster than HBM delivers them to one SM.
 //
-// Structure (one persistent CTA per SM, 192 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warps 2-5 =
-// epilogue (TMEM -> registers -> maps).  A CTA tile is T adjacent 128-byte pixel spans over all frames; the
-// accumulators of a tile (T * NC columns) are double buffered in TMEM so the epilogue of tile i overlaps the
-// main loop of tile i+1.
+// Structure (one persistent CTA per SM, 320 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warps 2-9 =
+// epilogue (TMEM -> registers -> maps; two quartets, each warp reads its own TMEM lane quarter).  A CTA tile is T adjacent 128-byte pixel spans over all frames.  When two
+// tiles' accumulators fit the 512 TMEM columns (2 * T * NC <= 512) they are double buffered; otherwise (K = 8: NC = 64,
+// T = 8 -- 1 KB of contiguous bytes per frame, which DRAM serves measurably better than 512 B) there is one set and the
+// epilogue hands the columns back span by span: the MMA warp restarts span t of the next tile as soon as span t is
+// drained, and the TMA producer keeps filling the stage ring meanwhile, so HBM never idles.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -38,6 +40,9 @@ constexpr int MMA_K = 32;         // frames per tcgen05.mma (8-bit operands)
 constexpr int GRP = 8;            // frames per 128-byte-swizzle atom (8 rows of 128 bytes = 1 KB)
 constexpr int TC_TQ = 16;         // tile-id queue entries: the producer runs at most `stages` <= 12 tiles ahead of the MMA warp
 constexpr int TC_MAX_STAGES = 12;
+constexpr int EPI_SETS = 2;        // epilogue warp quartets: set e drains the spans t with t % EPI_SETS == e
+constexpr int TC_THREADS = 64 + 128 * EPI_SETS;
+constexpr int TC_MAX_SPANS = 32;  // accumulator sets: T spans, times two when double buffered
 static_assert(TC_MAX_STAGES < TC_TQ, "the tile queue must outlast the producer's run-ahead");
 
 // ---------------------------------------------------------------------------------------------------
@@ -64,6 +69,14 @@ __device__ __forceinline__ void tc_ld16(uint32_t taddr, uint32_t (&r)[16])
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
                    "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
                  : "r"(taddr));
+}
+// one lane of the (fully active) warp; the compiler keeps values that do not depend on the lane in uniform registers, which
+// is what tcgen05.mma's descriptor operands want
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.b32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
@@ -125,6 +138,38 @@ __global__ void k_digit_pack(const int32_t *rfix, int n_stride, int n, int rows,
 // ---------------------------------------------------------------------------------------------------
 // the contraction kernel
 // ---------------------------------------------------------------------------------------------------
+#ifdef QLD_TC_TRACE   // development builds only: per-chunk time stamps of CTA 0 (producer issue, data landed, MMAs issued)
+__device__ unsigned long long g_tc_trace[3 * 1024];
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TC_TRACE(kind, n) do { if (blockIdx.x == 0 && (n) < 1024) g_tc_trace[(kind) * 1024 + (n)] = gtime(); } while (0)
+#else
+#define TC_TRACE(kind, n) do { } while (0)
+#endif
+// sqrt of a non-negative double to a few units in 1e-14: fp32 reciprocal square root of the rounded argument, one Newton
+// step in fp64 (the library routine is correctly rounded but several times longer; the result is stored as fp32)
+__device__ __forceinline__ double sqrt_newton(double x)
+{
+    if (x == 0.0) return 0.0;
+    const double y = (double)rsqrtf((float)x);
+    const double r = x * y;
+    return fma(0.5 * y, fma(-r, r, x), r);
+}
+
+// A4 for one pixel of one reference from its exact sums (I * 2^30, Q * 2^30)
+__device__ __forceinline__ void emit_fixed(const TcParams &p, int k, int64_t pixel, long long Si, long long Ci, double sc30)
+{
+    const int64_t o = (int64_t)k * p.HW + pixel;
+    if (p.sums_out) {
+        p.sums_out[(int64_t)(2 * k) * p.HW + pixel] = Si;
+        p.sums_out[(int64_t)(2 * k + 1) * p.HW + pixel] = Ci;
+    }
+    const double S = (double)Si * sc30, C = (double)Ci * sc30;
+    if (p.fin.I) p.fin.I[o] = (float)S;
+    if (p.fin.Q) p.fin.Q[o] = (float)C;
+    if (p.fin.amp) p.fin.amp[o] = (float)sqrt_newton(fma(S, S, C * C));
+    if (p.fin.phase) p.fin.phase[o] = (Si == 0 && Ci == 0) ? 0.0f : (float)atan2(C, S);
+}
+
 // shared-memory carve-up for (NC columns, T spans per tile, STAGES pipeline stages)
 struct TcSmem {
     int a_stage, b_stage, off_b, off_bar, total;
@@ -134,14 +179,17 @@ struct TcSmem {
         b_stage = (kc / MMA_K) * nc * MMA_K;
         off_b = stages * a_stage;
         off_bar = off_b + stages * b_stage;
-        total = off_bar + (2 * stages + 4) * 8 + 16 + 8 + TC_TQ * 4 + 8;   // barriers, TMEM slot, tile queue, tbuf_tile
+        total = off_bar + (2 * stages + 2 + TC_MAX_SPANS) * 8 + 16 + 8 + TC_TQ * 4 + 8;   // barriers, TMEM slot, tile queue, tbuf_tile
     }
 };
 
-template <int NC, int BYTES>
-__global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap2, const __grid_constant__ CUtensorMap tmap4,
-                                                     const TcParams p, const int T, const int STAGES, const int KC, const int use4d)
+// TT, KCC > 0: the tile shape as compile-time constants (the shape the launcher picks for large frames): the MMA warp's
+// loops over spans and K steps unroll and every descriptor is "stage base + immediate"; 0: run-time shape (T_rt, KC_rt).
+template <int NC, int BYTES, int TT, int KCC>
+__global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap2, const __grid_constant__ CUtensorMap tmap4,
+                                                     const TcParams p, const int T_rt, const int STAGES, const int KC_rt, const int use4d)
 {
+    const int T = TT > 0 ? TT : T_rt, KC = KCC > 0 ? KCC : KC_rt;
     const TcSmem SM(NC, T, STAGES, KC);
     extern __shared__ unsigned char smem_raw[];
     // 128-byte-swizzled TMA/UMMA tiles need 1024-byte alignment in the shared window
@@ -151,26 +199,27 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     uint64_t *full = reinterpret_cast<uint64_t *>(smem + SM.off_bar);
     uint64_t *empty = full + STAGES;
     uint64_t *tfull = empty + STAGES;
-    uint64_t *tempty = tfull + 2;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+    uint64_t *tempty = tfull + 2;                       // [NBUF * T] one per span accumulator: drained by the epilogue
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + TC_MAX_SPANS);
     volatile int *tile_q = reinterpret_cast<volatile int *>(tmem_slot + 2);      // [TC_TQ] tile ids, producer -> MMA warp
     volatile int *tbuf_tile = tile_q + TC_TQ;                                        // [2] tile id per accumulator buffer
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // the warp index as a broadcast: the compiler then knows that the role branches below are warp-uniform and keeps the MMA
+    // warp's loop state in uniform registers
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const int n_chunks = (p.N + KC - 1) / KC;
     const int n_full = p.N / GRP * GRP;               // frames covered by whole 8-frame groups (the 4-D map's extent)
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + T - 1) / T;
+    const int NBUF = 2 * T * NC <= 512 ? 2 : 1;       // accumulator sets in TMEM
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < STAGES; ++i) {
             mbar_init(&full[i], 1);
             mbar_init(&empty[i], 1);
         }
-        for (int i = 0; i < 2; ++i) {
-            mbar_init(&tfull[i], 2);
-            mbar_init(&tempty[i], 128);
-        }
+        for (int i = 0; i < 2; ++i) mbar_init(&tfull[i], 2);
+        for (int i = 0; i < TC_MAX_SPANS; ++i) mbar_init(&tempty[i], 128);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -180,15 +229,16 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);      // broadcast: provably warp-uniform
 
     if (warp == 0) {
         // ===== TMA producer + tile scheduler =====
         // Tiles are claimed from a global counter: under HBM contention SMs progress at very different rates
         // (ncu: fastest SM done in 56 % of the time with a static split), so the split must be dynamic.
         if (lane == 0) {
-            int stage = 0, it = 0;
+            int stage = 0, it = 0, n_issued = 0;
             uint32_t phase = 0;
+            (void)n_issued;
             for (;; ++it) {
                 int tile = (int)atomicAdd(p.tile_counter, 1u);
                 if (tile >= n_tiles) tile = -1;
@@ -203,6 +253,7 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
                 const uint64_t hint = 0x12F0000000000000ull;     // evict first: every sample is read once
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&empty[stage], phase ^ 1);
+                    TC_TRACE(0, n_issued); ++n_issued;
                     unsigned char *dst = sA + stage * SM.a_stage;
                     if (use4d && (c + 1) * KC <= n_full) {
                         // one 4-D box {128 B, 8 frames, T spans, KC/8 groups}: the TMA walks the T adjacent spans of a
@@ -227,42 +278,81 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
         }
     } else if (warp == 1) {
         // ===== MMA issuer =====
+        // The whole warp runs this loop and one elected lane issues: every operand of tcgen05.mma (descriptors, TMEM address)
+        // is then warp-uniform and lives in uniform registers.  Under `if (lane == 0)` the compiler cannot prove that and
+        // wraps every MMA in an ELECT / 5 x R2UR / branch sequence of about 200 cycles -- which, not the operand fetch, was
+        // what held the round-1 kernel at 20 bytes per clock per SM (an MMA of this shape retires in about 80 cycles).
         // instruction descriptor (cute::UMMA::InstrDescriptor): D = s32, A = u8 MN-major, B = s8 K-major, M = 128, N = NC
         constexpr uint32_t idesc = (2u << 4) | (0u << 7) | (1u << 10) | (1u << 15) | (0u << 16) | ((uint32_t)(NC >> 3) << 17) | ((128u >> 4) << 24);
-        int stage = 0;
+        const bool leader = elect_one();
+        const uint32_t sA0 = smem_u32(sA), sB0 = smem_u32(sB);
+        const uint32_t a_sbo = (uint32_t)(T * GRP * SUB_BYTES);
+        int stage = 0, n_done = 0;
         uint32_t phase = 0;
+        (void)n_done;
         for (int it = 0;; ++it) {
-            const int buf = it & 1;
-            mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);     // epilogue has drained this accumulator buffer
-            tc_fence_after();
+            const int buf = it & 1;                           // hand-off slot (tfull / tbuf_tile), always alternating
+            const int abuf = NBUF == 2 ? buf : 0;             // accumulator set
+            const uint32_t epar = (NBUF == 2 ? (uint32_t)(it >> 1) : (uint32_t)it) & 1u;   // a set's barriers flip once per use
             mbar_wait(&full[stage], phase);                   // first chunk of the tile (or the sentinel) has landed
-            const int tile = tile_q[it & (TC_TQ - 1)];
-            if (lane == 0) tbuf_tile[buf] = tile;
+            const int tile = __shfl_sync(0xffffffffu, tile_q[it & (TC_TQ - 1)], 0);
+            // The first span of every epilogue quartet (spans 0 .. EPI_SETS-1 of this accumulator set) is drained: each
+            // quartet is then past the hand-off that used tfull[buf] / tbuf_tile[buf] two tiles ago, so both may be reused.
+            for (int e = 0; e < EPI_SETS && e < T; ++e) mbar_wait(&tempty[abuf * T + e], epar ^ 1u);
+            if (leader) tbuf_tile[buf] = tile;
             if (tile < 0) {
-                if (lane == 0) { mbar_arrive(&tfull[buf]); mbar_arrive(&tfull[buf]); }
+                if (leader) { mbar_arrive(&tfull[buf]); mbar_arrive(&tfull[buf]); }
                 break;
             }
             const int nv = min(T, n_sub - tile * T);
+            const uint32_t d0 = tmem_base + (uint32_t)(abuf * T * NC);
             for (int c = 0; c < n_chunks; ++c) {
                 if (c > 0) mbar_wait(&full[stage], phase);
                 tc_fence_after();
-                if (lane == 0) {
-                    const uint32_t a0 = smem_u32(sA + stage * SM.a_stage), b0 = smem_u32(sB + stage * SM.b_stage);
-                    for (int t = 0; t < nv; ++t) {
-                        for (int ks = 0; ks < KC / MMA_K; ++ks) {
-                            // A: MN-major, 128-byte swizzle: rows of 128 pixel bytes, 8-frame atoms T KB apart (SBO)
-                            const uint64_t ad = smem_desc(a0 + (ks * (MMA_K / GRP) * T + t) * (GRP * SUB_BYTES), T * GRP * SUB_BYTES, T * GRP * SUB_BYTES, 2);
-                            // B: K-major, no swizzle: K halves 128 B apart (LBO), 8-column groups 256 B apart (SBO)
-                            const uint64_t bd = smem_desc(b0 + ks * NC * MMA_K, 128, 256, 0);
-                            tc_mma_i8(tmem_base + (uint32_t)(buf * T * NC + t * NC), ad, bd, idesc, (c | ks) ? 1u : 0u);
+                if (leader) TC_TRACE(1, n_done);
+                // descriptors of this stage: A MN-major with 128-byte swizzle (rows of 128 pixel bytes, 8-frame atoms T KB
+                // apart = SBO); B K-major without swizzle (K halves 128 B apart = LBO, 8-column groups 256 B apart = SBO).
+                // The start address sits in the low 14 bits (units of 16 bytes): span t / K step ks are plain additions.
+                const uint64_t ad0 = smem_desc(sA0 + (uint32_t)(stage * SM.a_stage), a_sbo, a_sbo, 2);
+                const uint64_t bd0 = smem_desc(sB0 + (uint32_t)(stage * SM.b_stage), 128, 256, 0);
+                if (TT > 0) {
+#pragma unroll
+                    for (int t = 0; t < (TT > 0 ? TT : 1); ++t) {
+                        if (t < nv) {
+                            if (c == 0) {                     // the epilogue has drained this span's previous accumulator
+                                mbar_wait(&tempty[abuf * T + t], epar ^ 1u);
+                                tc_fence_after();
+                            }
+#pragma unroll
+                            for (int ks = 0; ks < (KCC > 0 ? KCC : MMA_K) / MMA_K; ++ks) {
+                                const uint64_t ad = ad0 + (uint64_t)(((ks * (MMA_K / GRP) * TT + t) * (GRP * SUB_BYTES)) >> 4);
+                                const uint64_t bd = bd0 + (uint64_t)((ks * NC * MMA_K) >> 4);
+                                if (leader) tc_mma_i8(d0 + (uint32_t)(t * NC), ad, bd, idesc, (c | ks) ? 1u : 0u);
+                            }
                         }
                     }
+                } else {
+                    for (int t = 0; t < nv; ++t) {
+                        if (c == 0) {
+                            mbar_wait(&tempty[abuf * T + t], epar ^ 1u);
+                            tc_fence_after();
+                        }
+                        for (int ks = 0; ks < KC / MMA_K; ++ks) {
+                            const uint64_t ad = ad0 + (uint64_t)(((ks * (MMA_K / GRP) * T + t) * (GRP * SUB_BYTES)) >> 4);
+                            const uint64_t bd = bd0 + (uint64_t)((ks * NC * MMA_K) >> 4);
+                            if (leader) tc_mma_i8(d0 + (uint32_t)(t * NC), ad, bd, idesc, (c | ks) ? 1u : 0u);
+                        }
+                    }
+                }
+                if (leader) {
                     tc_commit(&empty[stage]);                 // frees the stage when these MMAs have read it
                     if (c == n_chunks - 1) {
                         tc_commit(&tfull[buf]);               // arrival 1 of 2: the accumulators are complete
                         mbar_arrive(&tfull[buf]);             // arrival 2 of 2: releases tbuf_tile[buf]
                     }
+                    TC_TRACE(2, n_done);
                 }
+                ++n_done;
                 __syncwarp();
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
             }
@@ -270,29 +360,41 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
     } else {
         // ===== epilogue: TMEM -> registers -> exact int64 sums -> A4 finalise =====
         const int q = warp & 3;                         // TMEM lane quarter this warp may read
+        const int eset = (warp - 2) >> 2;               // which quartet of epilogue warps: it drains spans t % EPI_SETS == eset
         const int m = q * 32 + lane;                    // accumulator row = byte index inside the 128-byte span
-        for (int it = 0;; ++it) {
+        for (int it = 0; eset < T; ++it) {              // a quartet without spans (T < EPI_SETS) has nothing to do
             const int buf = it & 1;
+            const int abuf = NBUF == 2 ? buf : 0;
             mbar_wait(&tfull[buf], (it >> 1) & 1);
             const int tile = tbuf_tile[buf];
             if (tile < 0) break;
             const int nv = min(T, n_sub - tile * T);
             tc_fence_after();
-            for (int t = 0; t < nv; ++t) {
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * T * NC + t * NC);
+            for (int t = eset; t < T; t += EPI_SETS) {
+                if (t >= nv) {                                // span beyond the frame: nothing was accumulated, hand it back
+                    mbar_arrive(&tempty[abuf * T + t]);
+                    continue;
+                }
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(abuf * T * NC + t * NC);
                 const int64_t byte0 = (int64_t)(tile * T + t) * SUB_BYTES + m;
                 const int64_t pixel = BYTES == 2 ? (byte0 >> 1) : byte0;
                 const bool valid = byte0 < p.row_bytes;
+                // all NC columns of the span into registers with one wait, then the span goes straight back to the MMA warp:
+                // the arithmetic below runs out of registers while the next tile's MMAs already overwrite the columns
+                uint32_t r[NC / 16][16];
+#pragma unroll
+                for (int g = 0; g < NC / 16; ++g) tc_ld16(taddr + g * 16, r[g]);
+                tc_wait_ld();
+                tc_fence_before();
+                mbar_arrive(&tempty[abuf * T + t]);
+                const double sc30 = p.fin.scale * 9.31322574615478515625e-10;                   // scale * 2^-30
 #pragma unroll
                 for (int g = 0; g < NC / 16; ++g) {       // 16 columns = 4 reference rows = 2 references per group
-                    uint32_t r[16];
-                    tc_ld16(taddr + g * 16, r);
-                    tc_wait_ld();
                     long long v[4];
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr)
-                        v[rr] = (long long)(int)r[4 * rr] + ((long long)(int)r[4 * rr + 1] << 8) + ((long long)(int)r[4 * rr + 2] << 16) +
-                                ((long long)(int)r[4 * rr + 3] << 24);
+                        v[rr] = (long long)(int)r[g][4 * rr] + ((long long)(int)r[g][4 * rr + 1] << 8) + ((long long)(int)r[g][4 * rr + 2] << 16) +
+                                ((long long)(int)r[g][4 * rr + 3] << 24);
                     if (BYTES == 2) {
                         // even row = low byte, odd row = high byte of the same pixel: x = lo + 256 * hi
 #pragma unroll
@@ -302,29 +404,17 @@ __global__ void __launch_bounds__(192, 1) k_demod_tc(const __grid_constant__ CUt
                         }
                     }
                     // this group holds references 2g and 2g+1; with 16-bit samples the lane pair splits them
+                    if (BYTES == 2) {
+                        const int k = 2 * g + (lane & 1);
+                        const long long Si = (lane & 1) ? v[2] : v[0], Ci = (lane & 1) ? v[3] : v[1];
+                        if (valid && k < p.fin.K) emit_fixed(p, k, pixel, Si, Ci, sc30);
+                    } else {
 #pragma unroll
-                    for (int kk = 0; kk < 2; ++kk) {
-                        const int k = 2 * g + kk;
-                        const bool mine = BYTES == 1 || (lane & 1) == kk;
-                        if (valid && mine && k < p.fin.K) {
-                            const long long Si = v[2 * kk], Ci = v[2 * kk + 1];
-                            const int64_t o = (int64_t)k * p.HW + pixel;
-                            if (p.sums_out) {
-                                p.sums_out[(int64_t)(2 * k) * p.HW + pixel] = Si;
-                                p.sums_out[(int64_t)(2 * k + 1) * p.HW + pixel] = Ci;
-                            }
-                            const double S = (double)Si * (p.fin.scale * 9.31322574615478515625e-10);   // 2^-30
-                            const double C = (double)Ci * (p.fin.scale * 9.31322574615478515625e-10);
-                            if (p.fin.I) p.fin.I[o] = (float)S;
-                            if (p.fin.Q) p.fin.Q[o] = (float)C;
-                            if (p.fin.amp) p.fin.amp[o] = (float)sqrt(S * S + C * C);
-                            if (p.fin.phase) p.fin.phase[o] = (Si == 0 && Ci == 0) ? 0.0f : (float)atan2(C, S);
-                        }
+                        for (int kk = 0; kk < 2; ++kk)
+                            if (valid && 2 * g + kk < p.fin.K) emit_fixed(p, 2 * g + kk, pixel, v[2 * kk], v[2 * kk + 1], sc30);
                     }
                 }
             }
-            tc_fence_before();
-            mbar_arrive(&tempty[buf]);
         }
     }
 
@@ -349,29 +439,27 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms, const int *force)
     // 32 frames) from shared memory whatever N is, i.e. about 21 B/clk/SM = 6.1 TB/s over 148 SMs -- that, not HBM,
     // bounds this kernel.  64-frame stages (two MMAs per span per barrier round trip) and 1 KB of contiguous
     // bytes per frame were the best point of the sweep (T,stages,KC = 8,3,64: 6.17 TB/s; 16,3,32: 5.05; 4,6,64: 5.78).
-    int T = 512 / (2 * nc);
+    int T = 512 / nc;                                               // one accumulator set may fill the TMEM (K = 8: T = 8)
     if (T > 8) T = 8;
     while (T & (T - 1)) --T;                                        // power of two
     while (T > 1 && (n_sub + T - 1) / T < 2 * n_sms) T /= 2;      // small frames: keep every SM busy
     sh.T = T;
     sh.kc = 64;
-    sh.stages = (200 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
+    sh.stages = (225 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
     if (force && force[0] > 0) {                          // debug / test override (qld_debug_set_tile): T, STAGES, KC
         const int t = force[0], s2 = force[1], kc = force[2];
-        if (2 * t * nc <= 512 && s2 >= 2 && (kc == 32 || kc == 64) && TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
+        if (t * nc <= 512 && t <= TC_MAX_SPANS / 2 && s2 >= 2 && (kc == 32 || kc == 64) && TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
     }
     if (sh.stages > TC_MAX_STAGES) sh.stages = TC_MAX_STAGES;
     sh.use4d = (row_bytes % SUB_BYTES == 0 && N >= GRP) ? 1 : 0;
     return sh;
 }
 
-template <int NC, int BYTES>
-cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
+template <int NC, int BYTES, int TT, int KCC>
+cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const TcShape &sh, int n_sms, cudaStream_t st)
 {
-    const int force[3] = {p.force_T, p.force_stages, p.force_kc};
-    const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
-    auto kern = k_demod_tc<NC, BYTES>;
+    auto kern = k_demod_tc<NC, BYTES, TT, KCC>;
     // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
     // function, and re-setting it on every launch costs a driver call)
     static int smem_set_dev[64] = {0};
@@ -389,8 +477,18 @@ cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cu
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
     e = cudaMemsetAsync(p.tile_counter, 0, sizeof(unsigned int), st);
     if (e != cudaSuccess) return e;
-    kern<<<grid, 192, SM.total + 1024, st>>>(tmaps[0], tmaps[1], p, sh.T, sh.stages, sh.kc, sh.use4d);
+    kern<<<grid, TC_THREADS, SM.total + 1024, st>>>(tmaps[0], tmaps[1], p, sh.T, sh.stages, sh.kc, sh.use4d);
     return cudaGetLastError();
+}
+
+template <int NC, int BYTES>
+cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
+{
+    const int force[3] = {p.force_T, p.force_stages, p.force_kc};
+    const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
+    // the shape of large frames (T = 8 spans = 1 KB of every frame, 64-frame stages) has its own instantiation
+    if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64>(tmaps, p, sh, n_sms, st);
+    return launch_tc_shape<NC, BYTES, 0, 0>(tmaps, p, sh, n_sms, st);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -491,3 +589,10 @@ cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms,
     }
     return cudaErrorInvalidValue;
 }
+
+#ifdef QLD_TC_TRACE
+extern "C" int qld_tc_trace_read(unsigned long long *out, int n)
+{
+    return (int)cudaMemcpyFromSymbol(out, g_tc_trace, sizeof(unsigned long long) * (size_t)n);
+}
+#endif

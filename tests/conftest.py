@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "timeout: pytest-timeout limit for tests that would hang on a dead-locked kernel")
 
 
 @pytest.fixture(scope="session")

@@ -177,3 +177,32 @@ def test_auto_moves_k_ge_4_to_the_tensor_cores(Q, oracle):
     c3 = Q.QLD(3, 7, "u8", N, refs)              # 21-byte frames: not a TMA row pitch -> FP32
     assert c3.accum_name() == "FP32"
     c3.destroy()
+
+
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("tile", ["", "4,5,64", "2,8,64", "8,3,64", "1,8,32"])
+@pytest.mark.parametrize("H,W,N,K", [(256, 512, 128, 8), (128, 512, 64, 8), (96, 256, 32, 3)])
+def test_slow_epilogue_against_a_fast_main_loop(Q, oracle, tile, H, W, N, K):
+    """Few frames, many references and every output requested: the epilogue (two warp quartets that advance
+    independently) is then much slower than the MMA warp, which runs several tiles' worth of hand-offs ahead of it.  The
+    tile-id slots and accumulator sets must not be reused before BOTH quartets are past them (a regression: the second
+    quartet once read a later tile's id -- wrong pixels, then a dead-locked barrier).  Exact int64 sums at every pixel."""
+    rng = np.random.default_rng(H + N + K)
+    x = rng.integers(0, 65536, size=(N, H, W)).astype(np.uint16)
+    refs = [{"nu": 0.05 + 0.05 * k, "phase": 0.1 * k} for k in range(K)]
+    tabs = [_q30(oracle, r, N) for r in refs]
+    mk = forced(Q, "tc", tile)
+    ctx = mk(H, W, "u16", N, refs, accum=Q.QLD_ACC_FIXED, maps=Q.QLD_MAP_ALL | Q.QLD_MAP_SUMS_I64)
+    for k in range(K):
+        ctx.set_ref_table_fixed(k, *tabs[k])
+    ctx.push_frames(x)
+    for _ in range(3):
+        ctx.demod()
+    ctx.sync()
+    nt = oracle.max_threads()
+    for k in range(K):
+        oI, oQ = oracle.demod_int(x, *tabs[k], nthreads=nt)
+        gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
+        assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"k={k}"
+    check_float_maps(_maps(ctx, K - 1), oracle_maps(oracle, x, refs[K - 1]), rel=1e-6, what="slow epilogue")
+    ctx.destroy()
