@@ -237,7 +237,7 @@ int64_t qld_kernel_launches(const qld_ctx *ctx);
 
 /* Introspection for benchmarks and tests: the accumulation mode in use (a qld_accum other than AUTO; negative
  * status if ctx is NULL), and the name of the kernel the last qld_demod launched ("" before the first):
- * "k_demod_stream", "k_demod_whole", "k_demod_split", "k_demod_tc" or "k_demod_slide".  Never NULL. */
+ * "k_demod_stream", "k_demod_whole", "k_demod_tc", "k_slide_bulk" or "k_demod_slide".  Never NULL. */
 int qld_accum_mode(const qld_ctx *ctx);
 const char *qld_last_kernel(const qld_ctx *ctx);
 
@@ -245,7 +245,8 @@ const char *qld_last_kernel(const qld_ctx *ctx);
  * invalid shape is ignored).  which = 0: k_demod_stream, a = SEG (contiguous bytes of every frame per tile, a power of two
  * <= 2048), b = KC (frames per pipeline stage); forcing also lifts the frame-size threshold, so small frames go through
  * the TMA-fed kernel.  which = 1: k_demod_tc, a = T (128-byte spans per tile), b = STAGES, c = KC (32 or 64).
- * a = 0 restores the automatic choice.  Results never depend on the shape (tests/ run every shape against the oracle). */
+ * which = 2: the sliding update: a = 1 always runs k_slide_bulk (also on frames too small to give every SM a tile), a = 2
+ * never, a = 0 automatic.  For which = 0 / 1, a = 0 restores the automatic choice.  Results never depend on the shape (tests/ run every shape against the oracle). */
 int qld_debug_set_tile(qld_ctx *ctx, int which, int a, int b, int c);
 
 /* Contrast-to-noise ratio of a processed image (Eq. (1), Fig. 6; the paper's quality metric, the step

@@ -12,6 +12,7 @@
 #include <nvtx3/nvToolsExt.h>
 
 #include "qld_internal.h"
+#include "qld_slide.h"
 #include "qld_stream.h"
 #include "qld_tc.h"
 
@@ -51,7 +52,8 @@ struct qld_ctx {
     int32_t *rfix;           // [2K][N] Q30 references
     int8_t *digits;          // digit tiles for the MMA B operand
     int64_t *sums;           // optional [2K][HW] exact sums
-    unsigned int *tile_counter;
+    unsigned int *tile_counter;   // two counters that alternate between launches: each launch zeroes the other one
+    unsigned int counter_flip;
     alignas(64) unsigned char tmap[256];   // two CUtensorMap (qld_tc_encode_tmap)
     bool tmap_valid;
     int n_sms;
@@ -59,6 +61,11 @@ struct qld_ctx {
     alignas(64) unsigned char stream_tmap[128];
     const void *stream_tmap_frames;   // frame store the map was encoded for (NULL: none yet)
     StreamShape stream_shape;
+    // bulk-copy sliding update (qld_slide.cu)
+    alignas(64) unsigned char slide_tmap[128];
+    const void *slide_tmap_frames;
+    SlideShape slide_shape;
+    int dbg_slide;           // qld_debug_set_tile(which = 2): 0 automatic, 1 always k_slide_bulk, 2 never
     // device memory
     void *ws;
     bool own_ws;
@@ -291,6 +298,7 @@ int fill_tables(qld_ctx *c, int64_t s_first, int n, cudaStream_t st)
 
 int init_device_state(qld_ctx *c)
 {
+    CU(c, cudaMemsetAsync(c->tile_counter, 0, 2 * sizeof(unsigned int), c->s_copy));
     // tables zeroed (padding rows stay zero; cum entry of frame 0 is zero), then filled for the whole store
     if (!c->is_fixed) {
         CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
@@ -333,6 +341,14 @@ int fetch_bin_weights(qld_ctx *c)
     CU(c, cudaStreamSynchronize(c->s_copy));
     for (int r = 0; r < QLD_MAX_ROWS; ++r) { c->fin.sw[r] = w[r]; c->fin.cw[r] = w[QLD_MAX_ROWS + r]; }
     return QLD_OK;
+}
+
+// the tile counter of the next persistent-kernel launch (zero) and the one that launch has to zero
+void next_counters(qld_ctx *c, unsigned int **cur, unsigned int **nxt)
+{
+    *cur = c->tile_counter + (c->counter_flip & 1u);
+    *nxt = c->tile_counter + ((c->counter_flip + 1u) & 1u);
+    c->counter_flip++;
 }
 
 // make the copy stream wait for demods that still read frames <= last_overwritten
@@ -434,7 +450,8 @@ int run_whole_tc(qld_ctx *c)
     TcParams p;
     memset(&p, 0, sizeof p);
     p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes;
-    p.digits = c->digits; p.sums_out = c->sums; p.tile_counter = c->tile_counter;
+    p.digits = c->digits; p.sums_out = c->sums;
+    next_counters(c, &p.tile_counter, &p.tile_counter_next);
     p.force_T = c->dbg_tc[0]; p.force_stages = c->dbg_tc[1]; p.force_kc = c->dbg_tc[2];
     p.fin = fin_with_maps(c);
     CU(c, qld_launch_demod_tc(c->tmap, p, c->n_sms, c->s_comp));
@@ -463,7 +480,11 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     if (sh.seg > 0) {
         int rc = stream_tmap_for(c, sh);
         if (rc) return rc;
-        CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+        {
+            unsigned int *cur, *nxt;
+            next_counters(c, &cur, &nxt);
+            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
+        }
         c->last_kernel = "k_demod_stream";
     } else {
         CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
@@ -473,11 +494,50 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     return record_demod(c, a + 1);
 }
 
+// The sliding update through k_slide_bulk when the frames are large enough (or forced): returns 1 if it was launched,
+// 0 if the kernel does not apply, < 0 on error.
+int try_slide_bulk(qld_ctx *c, const DemodParams &p)
+{
+    const int n_map_rows = c->K * ((c->mapI != nullptr) + (c->mapQ != nullptr) + (c->mapA != nullptr) + (c->mapP != nullptr));
+    const SlideShape sh = qld_slide_shape(c->dtype, c->is_int, c->rows_pad, p.part != nullptr, n_map_rows, c->HW, c->frames, c->n_sms, c->dbg_slide);
+    if (sh.seg == 0) return 0;
+    if (c->slide_tmap_frames != c->frames || sh.seg != c->slide_shape.seg || sh.kc != c->slide_shape.kc) {
+        cudaError_t e = qld_slide_encode_tmap(c->slide_tmap, c->frames, c->HW * c->bytes, c->cap, sh);
+        if (e != cudaSuccess) return cuda_fail(c, e, "qld_slide_encode_tmap");
+        c->slide_tmap_frames = c->frames;
+        c->slide_shape = sh;
+    }
+    unsigned int *cur, *nxt;
+    next_counters(c, &cur, &nxt);
+    cudaError_t e = qld_launch_slide_bulk(c->dtype, c->is_int, c->rows_pad, c->slide_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp);
+    if (e != cudaSuccess) return cuda_fail(c, e, "qld_launch_slide_bulk");
+    c->launches++;
+    c->last_kernel = "k_slide_bulk";
+    return 1;
+}
+
 // Block-partial mode (8(f3)): one launch over the frames of batch b of the window that starts at offset a.
 // sub = false: seeding (the slot is only written); sub = true: a sliding update (the slot's old content is the
 // expired batch: taken off the accumulators, then overwritten).
 int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool add, bool sub, bool first_of_seed)
 {
+    if (add && sub) {                                       // steady state: every byte through the copy engines
+        DemodParams q;
+        memset(&q, 0, sizeof q);
+        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
+        q.cap = c->cap; q.cap_w = c->cap_w;
+        q.cum_lo = (int)(a_win % c->cap_w); q.cum_hi = (int)((a_win + c->N) % c->cap_w);
+        q.wtab = c->wtab; q.cum = c->cum;
+        q.acc_out = c->acc; q.acc_add = 1;
+        q.onehot = c->is_int && c->K == 1;
+        q.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
+        q.part_sub = 1;
+        q.ped_in = c->is_int ? nullptr : c->ped;
+        q.fin = fin_with_maps(c);
+        q.n_runs = add_runs(c, q.run, 0, first, c->slide_hop, +1);
+        const int rc = try_slide_bulk(c, q);
+        if (rc != 0) return rc < 0 ? rc : QLD_OK;
+    }
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
     DemodParams p;
@@ -497,7 +557,11 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
     p.n_runs = add_runs(c, p.run, 0, first, c->slide_hop, +1);
     int rc = stream_tmap_for(c, sh);
     if (rc) return rc;
-    CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+    {
+            unsigned int *cur, *nxt;
+            next_counters(c, &cur, &nxt);
+            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
+        }
     c->launches++;
     c->last_kernel = "k_demod_stream";
     return QLD_OK;
@@ -524,6 +588,23 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         if (rc) return rc;
         return record_demod(c, a_old + 1);                    // conservative: the whole window stays protected from overwriting
     }
+    {
+        // {expired, -w} + {new, +w} added to the stored sums: k_slide_bulk when the frames are large enough
+        DemodParams q;
+        memset(&q, 0, sizeof q);
+        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
+        q.cap = c->cap; q.cap_w = c->cap_w;
+        q.cum_lo = (int)(a_new % c->cap_w); q.cum_hi = (int)((a_new + c->N) % c->cap_w);
+        q.wtab = c->wtab; q.cum = c->cum;
+        q.acc_out = c->acc; q.acc_add = 1;
+        q.onehot = c->is_int && c->K == 1;
+        q.ped_in = c->is_int ? nullptr : c->ped;
+        q.fin = fin_with_maps(c);
+        int n = add_runs(c, q.run, 0, a_old, hop, -1);
+        q.n_runs = add_runs(c, q.run, n, a_old + c->N, hop, +1);
+        const int rc = try_slide_bulk(c, q);
+        if (rc != 0) return rc < 0 ? rc : record_demod(c, a_old + 1);
+    }
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0 && hop >= sh.kc) {
@@ -542,7 +623,11 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         p.n_runs = n;
         int rc = stream_tmap_for(c, sh);
         if (rc) return rc;
-        CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, c->tile_counter, c->n_sms, c->s_comp));
+        {
+            unsigned int *cur, *nxt;
+            next_counters(c, &cur, &nxt);
+            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
+        }
         c->launches++;
         c->last_kernel = "k_demod_stream";
         return record_demod(c, a_old + 1);
@@ -906,7 +991,7 @@ int qld_reset(qld_ctx *c)
     c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
     if (!c->ring && c->frames != c->own_frames) {          // an attached stack is detached (an attached ring stays attached)
-        c->frames = c->own_frames; c->tmap_valid = false; c->stream_tmap_frames = nullptr;
+        c->frames = c->own_frames; c->tmap_valid = false; c->stream_tmap_frames = nullptr; c->slide_tmap_frames = nullptr;
     }
     if (c->ring) {
         rc = init_device_state(c);
@@ -940,7 +1025,8 @@ int qld_debug_set_tile(qld_ctx *c, int which, int a, int b, int d)
     if (a < 0 || b < 0 || d < 0) return fail(c, QLD_E_INVAL, "debug_set_tile: negative value");
     if (which == 0) { c->dbg_stream[0] = a; c->dbg_stream[1] = b; }
     else if (which == 1) { c->dbg_tc[0] = a; c->dbg_tc[1] = b; c->dbg_tc[2] = d; c->tmap_valid = false; }
-    else return fail(c, QLD_E_INVAL, "debug_set_tile: which must be 0 (k_demod_stream) or 1 (k_demod_tc)");
+    else if (which == 2 && a <= 2) c->dbg_slide = a;
+    else return fail(c, QLD_E_INVAL, "debug_set_tile: which must be 0 (k_demod_stream), 1 (k_demod_tc) or 2 (k_slide_bulk: a = 0 / 1 / 2)");
     return QLD_OK;
 }
 

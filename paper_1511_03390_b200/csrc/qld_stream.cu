@@ -70,7 +70,8 @@ struct StreamSmem {
 // taken off the stored sums when p.part_sub is set)
 template <typename T, typename ACC, int ROWS, int V, int NWT, int NEPI, bool PART>
 __global__ void __launch_bounds__(32 * (NWT + 1 + NEPI), 1)
-k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ DemodParams p, const StreamShape sh, unsigned int *tile_counter)
+k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ DemodParams p, const StreamShape sh, unsigned int *tile_counter,
+               unsigned int *counter_next)
 {
     using PX = Pix<T, V>;
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
@@ -108,6 +109,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
     const int n_tiles = (int)((row_bytes + SEG - 1) / SEG);
 
     if (threadIdx.x == 0) {
+        if (blockIdx.x == 0) *counter_next = 0;   // the next launch's tile counter (the two alternate: no memset between launches)
         for (int i = 0; i < STAGES; ++i) {
             mbar_init(&full[i], 2);          // the producer's expect_tx arrival + its "weights written" arrival
             mbar_init(&empty[i], NWT);
@@ -576,7 +578,7 @@ int red_bytes_for(int seg, int vb, int rows, int v, bool is_int, int nw, int nep
 }
 
 template <typename T, typename ACC, int ROWS, int NWT, int NEPI, bool PART>
-cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
+cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
     constexpr int V = stream_v(sizeof(T), ROWS);
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
@@ -596,28 +598,26 @@ cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const Stream
     }
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
     const int n_tiles = (int)((row_bytes + sh.seg - 1) / sh.seg);
-    e = cudaMemsetAsync(counter, 0, sizeof(unsigned int), st);
-    if (e != cudaSuccess) return e;
-    kern<<<n_tiles < n_sms ? n_tiles : n_sms, 32 * (NWT + 1 + NEPI), SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, counter);
+    kern<<<n_tiles < n_sms ? n_tiles : n_sms, 32 * (NWT + 1 + NEPI), SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, counter, counter_next);
     return cudaGetLastError();
 }
 
 template <typename T, typename ACC, int ROWS>
-cudaError_t launch_stream_t(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
+cudaError_t launch_stream_t(const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
-    if (p.part) return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), true>(tmap, p, sh, counter, n_sms, st);
-    return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), false>(tmap, p, sh, counter, n_sms, st);
+    if (p.part) return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), true>(tmap, p, sh, counter, counter_next, n_sms, st);
+    return launch_stream_n<T, ACC, ROWS, NW, stream_nepi(sizeof(T), ROWS), false>(tmap, p, sh, counter, counter_next, n_sms, st);
 }
 
 template <typename T, typename ACC>
-cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, int n_sms, cudaStream_t st)
+cudaError_t launch_stream_r(int rows, const void *tmap, const DemodParams &p, const StreamShape &sh, unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
     switch (rows) {
-    case 2: return launch_stream_t<T, ACC, 2>(tmap, p, sh, counter, n_sms, st);
-    case 3: return launch_stream_t<T, ACC, 3>(tmap, p, sh, counter, n_sms, st);
-    case 4: return launch_stream_t<T, ACC, 4>(tmap, p, sh, counter, n_sms, st);
-    case 8: return launch_stream_t<T, ACC, 8>(tmap, p, sh, counter, n_sms, st);
-    case 16: return launch_stream_t<T, ACC, 16>(tmap, p, sh, counter, n_sms, st);
+    case 2: return launch_stream_t<T, ACC, 2>(tmap, p, sh, counter, counter_next, n_sms, st);
+    case 3: return launch_stream_t<T, ACC, 3>(tmap, p, sh, counter, counter_next, n_sms, st);
+    case 4: return launch_stream_t<T, ACC, 4>(tmap, p, sh, counter, counter_next, n_sms, st);
+    case 8: return launch_stream_t<T, ACC, 8>(tmap, p, sh, counter, counter_next, n_sms, st);
+    case 16: return launch_stream_t<T, ACC, 16>(tmap, p, sh, counter, counter_next, n_sms, st);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -680,9 +680,9 @@ cudaError_t qld_stream_encode_tmap(void *tmap_out, const void *frames, int64_t r
 }
 
 cudaError_t qld_launch_demod_stream(int dtype, int is_int, int rows, const void *tmap, const DemodParams &p, const StreamShape &sh,
-                                    unsigned int *counter, int n_sms, cudaStream_t st)
+                                    unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
     if (dtype == QLD_U8)
-        return is_int ? launch_stream_r<uint8_t, int>(rows, tmap, p, sh, counter, n_sms, st) : launch_stream_r<uint8_t, float>(rows, tmap, p, sh, counter, n_sms, st);
-    return is_int ? launch_stream_r<uint16_t, int>(rows, tmap, p, sh, counter, n_sms, st) : launch_stream_r<uint16_t, float>(rows, tmap, p, sh, counter, n_sms, st);
+        return is_int ? launch_stream_r<uint8_t, int>(rows, tmap, p, sh, counter, counter_next, n_sms, st) : launch_stream_r<uint8_t, float>(rows, tmap, p, sh, counter, counter_next, n_sms, st);
+    return is_int ? launch_stream_r<uint16_t, int>(rows, tmap, p, sh, counter, counter_next, n_sms, st) : launch_stream_r<uint16_t, float>(rows, tmap, p, sh, counter, counter_next, n_sms, st);
 }

@@ -15,4 +15,4 @@ struct StreamShape {
 StreamShape qld_stream_shape(int dtype, int is_int, int rows, int64_t HW, const void *frames, int n_sms, int force_seg = 0, int force_kc = 0);
 cudaError_t qld_stream_encode_tmap(void *tmap_out /*128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int cap, const StreamShape &sh);
 cudaError_t qld_launch_demod_stream(int dtype, int is_int, int rows, const void *tmap, const DemodParams &p, const StreamShape &sh,
-                                    unsigned int *counter, int n_sms, cudaStream_t st);
+                                    unsigned int *counter /* zero on entry */, unsigned int *counter_next /* zeroed by the launch */, int n_sms, cudaStream_t st);

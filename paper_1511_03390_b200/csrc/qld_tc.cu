@@ -214,6 +214,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
     const int NBUF = 2 * T * NC <= 512 ? 2 : 1;       // accumulator sets in TMEM
 
     if (threadIdx.x == 0) {
+        if (blockIdx.x == 0) *p.tile_counter_next = 0;
         for (int i = 0; i < STAGES; ++i) {
             mbar_init(&full[i], 1);
             mbar_init(&empty[i], 1);
@@ -475,8 +476,6 @@ cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const T
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + sh.T - 1) / sh.T;
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
-    e = cudaMemsetAsync(p.tile_counter, 0, sizeof(unsigned int), st);
-    if (e != cudaSuccess) return e;
     kern<<<grid, TC_THREADS, SM.total + 1024, st>>>(tmaps[0], tmaps[1], p, sh.T, sh.stages, sh.kc, sh.use4d);
     return cudaGetLastError();
 }

@@ -12,7 +12,8 @@ struct TcParams {
     int32_t bytes;            // 1 (u8) or 2 (u16)
     const int8_t *digits;     // digit tiles, see k_digit_pack
     int64_t *sums_out;        // optional [2K][HW] exact fixed-point sums (Q30 references)
-    unsigned int *tile_counter; // device counter for the dynamic tile scheduler, zeroed by the launcher
+    unsigned int *tile_counter; // device counter for the dynamic tile scheduler: zero on entry
+    unsigned int *tile_counter_next; // the next launch's counter, zeroed by this launch (the two alternate)
     int32_t force_T, force_stages, force_kc;   // debug override of the tile shape (qld_debug_set_tile), 0 = automatic
     int32_t reserved;
     FinParams fin;

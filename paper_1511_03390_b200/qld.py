@@ -295,8 +295,8 @@ class QLD:
         return {QLD_ACC_FP32: "FP32", QLD_ACC_INT_BINS: "INT_BINS", QLD_ACC_FIXED: "FIXED"}[self.accum_mode()]
 
     def debug_set_tile(self, which, a: int = 0, b: int = 0, c: int = 0) -> None:
-        """qld_debug_set_tile: which = "stream" (SEG, KC) or "tc" (T, STAGES, KC)."""
-        w = {"stream": 0, "tc": 1}.get(which, which)
+        """qld_debug_set_tile: which = "stream" (SEG, KC), "tc" (T, STAGES, KC) or "slide" (1 = always k_slide_bulk, 2 = never)."""
+        w = {"stream": 0, "tc": 1, "slide": 2}.get(which, which)
         self._check(self.lib.qld_debug_set_tile(self._ctx, int(w), int(a), int(b), int(c)))
 
     def last_kernel(self) -> str:

@@ -104,7 +104,7 @@ def test_sliding_full_size_sampled(Q, oracle, accum_name, slide_hop):
         if w > 0:
             ctx.commit_frames(hop)
             ctx.demod(Q.QLD_SLIDE, hop)
-            assert ctx.last_kernel() == "k_demod_stream"
+            assert ctx.last_kernel() == "k_slide_bulk"
         if w in (0, 1, 5, n_hops):
             ctx.sync()
             x, ora = _oracle_on_pixels(oracle, sc, pix, ref, w * hop + 1, N)

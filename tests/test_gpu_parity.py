@@ -568,3 +568,49 @@ def test_commit_frames_into_attached_ring(Q, oracle, accum_name):
     ctx.sync()
     check_float_maps(_maps(ctx), oracle_maps(oracle, stream[:N], ref), what="after reset")
     ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ A5 through the copy engines
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("accum_name,refs", [("INT_BINS", [{"num": 1, "den": 6}]), ("INT_BINS", [{"num": 1, "den": 4}]), ("INT_BINS", [{"num": 3, "den": 8}]),
+                                             ("INT_BINS", [{"num": 1, "den": 4}, {"num": 1, "den": 4, "phase_quarter": 1}]),
+                                             ("FP32", [{"nu": 0.0937, "phase": 0.3}]), ("FP32", [{"nu": 0.21}, {"num": 1, "den": 6}])])
+@pytest.mark.parametrize("hop,cap,partial", [(32, 170, True), (32, 170, False), (40, 173, False), (5, 140, False), (64, 200, True), (16, 150, False)])
+@pytest.mark.parametrize("dtype,H,W,maps", [(np.uint16, 12, 128, "all"), (np.uint16, 37, 72, "amp"), (np.uint8, 9, 144, "all")])
+def test_slide_bulk_kernel(Q, oracle, accum_name, refs, hop, cap, partial, dtype, H, W, maps):
+    """k_slide_bulk (forced onto small frames): stored sums, expired partial sums and maps travel by bulk copies through
+    shared memory; frames by TMA.  Ragged last tile (37 x 72 = 2664 pixels = 2 tiles + 616), hops that are not a multiple of
+    a stage, runs that wrap around the ring, one and two references, all maps or the amplitude only: every window equals
+    the oracle's direct recomputation, integer bins bit-exact."""
+    N = 128
+    T = N + 7 * hop
+    rng = np.random.default_rng(hop + cap + H)
+    hi = 4096 if dtype == np.uint16 else 256
+    stream = _rand_stack(rng, T, H, W, dtype, hi=hi)
+    try:
+        ctx = Q.QLD(H, W, "u8" if dtype == np.uint8 else "u16", N, refs, ring_frames=cap, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=hi - 1,
+                    slide_hop=hop if partial else 0, maps=Q.QLD_MAP_ALL if maps == "all" else Q.QLD_MAP_AMP, resync_hops=-1,
+                    debug_tile=("stream", 512, 16) if partial else None)
+    except Q.QLDError as e:
+        assert partial and e.status == Q.QLD_E_UNSUPPORTED
+        return
+    ctx.debug_set_tile("slide", 1)
+    ctx.push_frames(stream[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    for w in range(0, (T - N) // hop + 1):
+        if w > 0:
+            ctx.push_frames(stream[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+            # (two fp32 references with partial sums and all maps need 100 KB of state per tile: no room for the pipeline,
+            # the launcher falls back to k_demod_stream)
+            assert ctx.last_kernel() == "k_slide_bulk" or (accum_name == "FP32" and len(refs) == 2 and partial and maps == "all")
+        ctx.sync()
+        a = w * hop
+        for k, ref in enumerate(refs):
+            ora = oracle_maps(oracle, stream[a:a + N], ref, s_first=a + 1)
+            check_float_maps(_maps(ctx, k), ora, rel=1e-6 if accum_name == "INT_BINS" else 1e-5, what=f"window {w} k={k}")
+            if accum_name == "INT_BINS":
+                den, num = ref["den"], ref["num"]
+                B = oracle.bins(stream[a:a + N], num, den, s_first=a + 1)
+                assert np.array_equal(ctx.get_bins(k).cpu().numpy(), B[:den // 2] - B[den // 2:]), f"window {w} k={k}"
+    ctx.destroy()
