@@ -38,7 +38,12 @@ extern "C" {
 
 typedef struct qld_ctx qld_ctx; /* opaque; one per stream of frames */
 
-typedef enum { QLD_U8 = 0, QLD_U16 = 1 } qld_dtype;
+/* Sample formats.  QLD_U16 is a little-endian uint16 array.  QLD_U16_BE is the camera's raw 16-bit stream as it arrives over
+ * a Camera-Link style interface with the most significant byte first ("a stream of 16-bit binary data (2-bytes)"
+ * "stitch pairs of bytes and store values in an array of the appropriate data type"): the pairs are stitched inside the
+ * kernels' loads (a byte-permute selector on the CUDA cores, the roles of the two accumulator rows on the tensor cores), so
+ * the paper's thread T2 and its extra pass over the data do not exist.  Frames keep their size: 2 bytes per sample. */
+typedef enum { QLD_U8 = 0, QLD_U16 = 1, QLD_U16_BE = 2 } qld_dtype;
 
 typedef enum {
     QLD_OK = 0,

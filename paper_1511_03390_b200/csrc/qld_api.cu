@@ -40,6 +40,7 @@ struct DemodEvent {
 struct qld_ctx {
     // configuration
     int H, W, dtype, bytes, N, K, accum, norm, maps, resync_hops;
+    int big_endian;          // QLD_U16_BE: byte pairs stitched most significant byte first
     int64_t HW;
     uint32_t max_value;
     int cap, cap_w;          // frame store capacity, weight table capacity
@@ -146,7 +147,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     auto bad = [&](int code, const char *m) { *err = m; return code; };
     if (!cfg) return bad(QLD_E_INVAL, "config is NULL");
     if (cfg->H < 1 || cfg->W < 1) return bad(QLD_E_INVAL, "H and W must be >= 1");
-    if (cfg->dtype != QLD_U8 && cfg->dtype != QLD_U16) return bad(QLD_E_INVAL, "dtype must be QLD_U8 or QLD_U16");
+    if (cfg->dtype != QLD_U8 && cfg->dtype != QLD_U16 && cfg->dtype != QLD_U16_BE) return bad(QLD_E_INVAL, "dtype must be QLD_U8, QLD_U16 or QLD_U16_BE");
     if (cfg->N < 1) return bad(QLD_E_INVAL, "N must be >= 1");
     if (cfg->K < 1 || cfg->K > QLD_MAX_K || !cfg->refs) return bad(QLD_E_INVAL, "K must be 1..8 with refs given");
     if (cfg->ring_frames < -1 || (cfg->ring_frames > 0 && cfg->ring_frames <= cfg->N))
@@ -449,7 +450,7 @@ int run_whole_tc(qld_ctx *c)
     }
     TcParams p;
     memset(&p, 0, sizeof p);
-    p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes;
+    p.HW = c->HW; p.row_bytes = c->HW * c->bytes; p.N = c->N; p.bytes = c->bytes; p.big_endian = c->big_endian;
     p.digits = c->digits; p.sums_out = c->sums;
     next_counters(c, &p.tile_counter, &p.tile_counter_next);
     p.force_T = c->dbg_tc[0]; p.force_stages = c->dbg_tc[1]; p.force_kc = c->dbg_tc[2];
@@ -465,6 +466,7 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     if (c->is_fixed) return run_whole_tc(c);
     DemodParams p;
     memset(&p, 0, sizeof p);
+    p.big_endian = c->big_endian;
     p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
     p.cap = c->cap; p.slot0 = (int)(a % c->cap); p.n = c->N;
     p.cap_w = c->cap_w; p.w0 = (int)((a + 1) % c->cap_w);
@@ -524,6 +526,7 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
     if (add && sub) {                                       // steady state: every byte through the copy engines
         DemodParams q;
         memset(&q, 0, sizeof q);
+        q.big_endian = c->big_endian;
         q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
         q.cap = c->cap; q.cap_w = c->cap_w;
         q.cum_lo = (int)(a_win % c->cap_w); q.cum_hi = (int)((a_win + c->N) % c->cap_w);
@@ -542,6 +545,7 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
     if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
     DemodParams p;
     memset(&p, 0, sizeof p);
+    p.big_endian = c->big_endian;
     p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
     p.cap = c->cap; p.cap_w = c->cap_w;
     p.cum_lo = (int)(a_win % c->cap_w); p.cum_hi = (int)((a_win + c->N) % c->cap_w);
@@ -592,6 +596,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         // {expired, -w} + {new, +w} added to the stored sums: k_slide_bulk when the frames are large enough
         DemodParams q;
         memset(&q, 0, sizeof q);
+        q.big_endian = c->big_endian;
         q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
         q.cap = c->cap; q.cap_w = c->cap_w;
         q.cum_lo = (int)(a_new % c->cap_w); q.cum_hi = (int)((a_new + c->N) % c->cap_w);
@@ -610,7 +615,8 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
     if (sh.seg > 0 && hop >= sh.kc) {
         DemodParams p;
         memset(&p, 0, sizeof p);
-        p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+        p.big_endian = c->big_endian;
+    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
         p.cap = c->cap; p.cap_w = c->cap_w;
         p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
         p.wtab = c->wtab; p.cum = c->cum;
@@ -634,6 +640,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
     }
     SlideParams p;
     memset(&p, 0, sizeof p);
+    p.big_endian = c->big_endian;
     p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
     p.cap = c->cap; p.cap_w = c->cap_w; p.hop = hop;
     p.new_slot0 = (int)((a_old + c->N) % c->cap);          // first new frame is a_old+N+1 -> slot (a_old+N) mod cap
@@ -681,6 +688,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     qld_ctx *c = new (std::nothrow) qld_ctx();
     if (!c) return fail(nullptr, QLD_E_NOMEM, "host allocation failed");
     c->H = pl.H; c->W = pl.W; c->dtype = pl.dtype; c->bytes = pl.bytes; c->N = pl.N; c->K = pl.K;
+    c->big_endian = pl.dtype == QLD_U16_BE ? 1 : 0;
     c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops;
     c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
     c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->rows = pl.rows; c->rows_pad = pl.rows_pad;

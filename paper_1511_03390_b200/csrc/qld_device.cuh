@@ -48,18 +48,20 @@ struct Pix {
             w[0] = *ptr;
         }
     }
+    // bsw: selector mask that stitches the byte pair of a 16-bit sample the other way round (QLD_U16_BE, a Camera-Link style
+    // stream with the most significant byte first): 0x11 swaps the two low selector nibbles, 0 = little endian
     // sample j as an unsigned integer
-    __device__ __forceinline__ static uint32_t geti(const uint32_t (&w)[NW], int j)
+    __device__ __forceinline__ static uint32_t geti(const uint32_t (&w)[NW], int j, uint32_t bsw = 0)
     {
         // one byte-permute (selector nibble 4 = a zero byte of the second operand)
-        if constexpr (sizeof(T) == 2) return __byte_perm(w[j >> 1], 0u, (j & 1) ? 0x4432u : 0x4410u);
+        if constexpr (sizeof(T) == 2) return __byte_perm(w[j >> 1], 0u, ((j & 1) ? 0x4432u : 0x4410u) ^ bsw);
         else return __byte_perm(w[j >> 2], 0u, 0x4440u | (uint32_t)(j & 3));
     }
     // sample j as the float 2^23 + x (one byte-permute: the integer lands in the mantissa of 0x4B000000)
-    __device__ __forceinline__ static float getf_biased(const uint32_t (&w)[NW], int j)
+    __device__ __forceinline__ static float getf_biased(const uint32_t (&w)[NW], int j, uint32_t bsw = 0)
     {
         uint32_t r;
-        if constexpr (sizeof(T) == 2) r = __byte_perm(w[j >> 1], 0x4B000000u, (j & 1) ? 0x7632u : 0x7610u);
+        if constexpr (sizeof(T) == 2) r = __byte_perm(w[j >> 1], 0x4B000000u, ((j & 1) ? 0x7632u : 0x7610u) ^ bsw);
         else r = __byte_perm(w[j >> 2], 0x4B000000u, 0x7650u | (uint32_t)(j & 3));
         return __uint_as_float(r);
     }
@@ -179,12 +181,12 @@ __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c)
 // acc[r][v] += x_v * w_r for one frame.  Float: x is pedestal-subtracted exactly, (2^23+x) - (2^23+ped).
 template <typename T, typename ACC, int ROWS, int V>
 __device__ __forceinline__ void accumulate(const uint32_t (&w)[Pix<T, V>::NW], const ACC (&wt)[ROWS], const float (&pedm)[V],
-                                           ACC (&acc)[ROWS][V])
+                                           ACC (&acc)[ROWS][V], uint32_t bsw = 0)
 {
     if constexpr (std::is_same<ACC, float>::value && V % 2 == 0) {
 #pragma unroll
         for (int v = 0; v < V; v += 2) {
-            const uint64_t x = sub2(pack2(Pix<T, V>::getf_biased(w, v), Pix<T, V>::getf_biased(w, v + 1)), pack2(pedm[v], pedm[v + 1]));
+            const uint64_t x = sub2(pack2(Pix<T, V>::getf_biased(w, v, bsw), Pix<T, V>::getf_biased(w, v + 1, bsw)), pack2(pedm[v], pedm[v + 1]));
 #pragma unroll
             for (int r = 0; r < ROWS; ++r) {
                 const uint64_t a = fma2(x, pack2(wt[r], wt[r]), pack2(acc[r][v], acc[r][v + 1]));
@@ -195,11 +197,11 @@ __device__ __forceinline__ void accumulate(const uint32_t (&w)[Pix<T, V>::NW], c
 #pragma unroll
         for (int v = 0; v < V; ++v) {
             if constexpr (std::is_same<ACC, float>::value) {
-                float x = Pix<T, V>::getf_biased(w, v) - pedm[v];
+                float x = Pix<T, V>::getf_biased(w, v, bsw) - pedm[v];
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) acc[r][v] = fmaf(x, wt[r], acc[r][v]);
             } else {
-                int x = (int)Pix<T, V>::geti(w, v);
+                int x = (int)Pix<T, V>::geti(w, v, bsw);
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) acc[r][v] += x * wt[r];
             }
@@ -211,14 +213,14 @@ __device__ __forceinline__ void accumulate(const uint32_t (&w)[Pix<T, V>::NW], c
 // (+1 or -1 in one row, zeros elsewhere).  The row is the same for every thread (it depends on the frame only):
 // branch on it and update that row alone -- V integer multiply-adds per frame instead of ROWS * V.
 template <typename T, int ROWS, int V>
-__device__ __forceinline__ void accumulate_onehot(const uint32_t (&w)[Pix<T, V>::NW], const int (&wt)[ROWS], int (&acc)[ROWS][V])
+__device__ __forceinline__ void accumulate_onehot(const uint32_t (&w)[Pix<T, V>::NW], const int (&wt)[ROWS], int (&acc)[ROWS][V], uint32_t bsw = 0)
 {
     int sgn = 0;
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) sgn += wt[r];
     int x[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) x[v] = (int)Pix<T, V>::geti(w, v);
+    for (int v = 0; v < V; ++v) x[v] = (int)Pix<T, V>::geti(w, v, bsw);
     bool done = false;
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) {

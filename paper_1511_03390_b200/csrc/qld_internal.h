@@ -63,7 +63,8 @@ struct DemodParams {
     DemodRun run[4];
     void *part;              // block-partial sliding (8(f3)): [ROWS][HW] slot of the partial-sum ring; this launch's sums are
                              // stored there, after the slot's previous content was taken off acc_out when part_sub is set
-    int32_t part_sub, reserved;
+    int32_t part_sub;
+    int32_t big_endian;      // 16-bit samples arrive most significant byte first (QLD_U16_BE): stitched in the load
     const float *ped_in;     // FP32: pedestal to subtract (the one acc_out was seeded with); NULL: the first sample
     FinParams fin;
 };
@@ -77,6 +78,7 @@ struct SlideParams {
     int32_t new_slot0, old_slot0;   // slots of the first new / first expired frame
     int32_t new_w0, old_w0;         // weight entries of the same
     int32_t hop;
+    int32_t big_endian;
     int32_t cum_lo, cum_hi;         // entries of frame (window first - 1) and window last, after the update
     const void *wtab;
     const double *cum;

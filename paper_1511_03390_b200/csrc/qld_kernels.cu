@@ -37,6 +37,7 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
     const unsigned char *base = static_cast<const unsigned char *>(p.frames) + pix0 * (int64_t)sizeof(T);
     const ACC *wtab = static_cast<const ACC *>(p.wtab);
 
+    const uint32_t bsw = p.big_endian ? 0x11u : 0u;
     ACC acc[ROWS][V];
 #pragma unroll
     for (int r = 0; r < ROWS; ++r)
@@ -52,7 +53,7 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
             uint32_t w0[PX::NW];
             PX::load(base + (int64_t)p.slot0 * p.frame_stride, w0);
 #pragma unroll
-            for (int v = 0; v < V; ++v) pedm[v] = PX::getf_biased(w0, v);
+            for (int v = 0; v < V; ++v) pedm[v] = PX::getf_biased(w0, v, bsw);
             if (ty == 0) {
 #pragma unroll
                 for (int v = 0; v < V; ++v) pedsm[v * BX + tx] = pedm[v] - 8388608.0f;
@@ -79,7 +80,7 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
                 if (e >= p.cap_w) e -= p.cap_w;
                 ACC wt[ROWS];
                 load_weights<ACC, ROWS>(wtab + (int64_t)e * ROWS, wt);
-                accumulate<T, ACC, ROWS, V>(w[u], wt, pedm, acc);
+                accumulate<T, ACC, ROWS, V>(w[u], wt, pedm, acc, bsw);
             }
             slot += U;
             if (slot >= p.cap) slot -= p.cap;
@@ -91,7 +92,7 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
             PX::load(base + (int64_t)slot * p.frame_stride, w);
             ACC wt[ROWS];
             load_weights<ACC, ROWS>(wtab + (int64_t)we * ROWS, wt);
-            accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc);
+            accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc, bsw);
             if (++slot >= p.cap) slot -= p.cap;
             if (++we >= p.cap_w) we -= p.cap_w;
         }
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(256) k_demod_whole(const DemodParams p)
 // ---------------------------------------------------------------------------------------------------
 template <typename T, typename ACC, int ROWS, int V>
 __device__ __forceinline__ void hop_partial(const unsigned char *base, int64_t stride, int cap, int slot, const ACC *wtab, int cap_w,
-                                            int we, int hop, const float (&pedm)[V], ACC (&acc)[ROWS][V])
+                                            int we, int hop, const float (&pedm)[V], ACC (&acc)[ROWS][V], uint32_t bsw)
 {
     using PX = Pix<T, V>;
     constexpr int U = (ROWS * V >= 64) ? 2 : 4;
@@ -168,7 +169,7 @@ __device__ __forceinline__ void hop_partial(const unsigned char *base, int64_t s
             if (e >= cap_w) e -= cap_w;
             ACC wt[ROWS];
             load_weights<ACC, ROWS>(wtab + (int64_t)e * ROWS, wt);
-            accumulate<T, ACC, ROWS, V>(w[u], wt, pedm, acc);
+            accumulate<T, ACC, ROWS, V>(w[u], wt, pedm, acc, bsw);
         }
         slot += U;
         if (slot >= cap) slot -= cap;
@@ -180,7 +181,7 @@ __device__ __forceinline__ void hop_partial(const unsigned char *base, int64_t s
         PX::load(base + (int64_t)slot * stride, w);
         ACC wt[ROWS];
         load_weights<ACC, ROWS>(wtab + (int64_t)we * ROWS, wt);
-        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc);
+        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc, bsw);
         if (++slot >= cap) slot -= cap;
         if (++we >= cap_w) we -= cap_w;
     }
@@ -207,8 +208,8 @@ __global__ void __launch_bounds__(128) k_demod_slide(const SlideParams p)
             a_new[r][v] = 0;
             a_old[r][v] = 0;
         }
-    hop_partial<T, ACC, ROWS, V>(base, p.frame_stride, p.cap, p.new_slot0, wtab, p.cap_w, p.new_w0, p.hop, pedm, a_new);
-    hop_partial<T, ACC, ROWS, V>(base, p.frame_stride, p.cap, p.old_slot0, wtab, p.cap_w, p.old_w0, p.hop, pedm, a_old);
+    hop_partial<T, ACC, ROWS, V>(base, p.frame_stride, p.cap, p.new_slot0, wtab, p.cap_w, p.new_w0, p.hop, pedm, a_new, p.big_endian ? 0x11u : 0u);
+    hop_partial<T, ACC, ROWS, V>(base, p.frame_stride, p.cap, p.old_slot0, wtab, p.cap_w, p.old_w0, p.hop, pedm, a_old, p.big_endian ? 0x11u : 0u);
 
 #pragma unroll
     for (int v = 0; v < V; ++v) {

@@ -257,6 +257,9 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
 
     // ===== consumers =====
     const int ct = (int)threadIdx.x - 32;                  // consumer thread: pixels 4*ct .. 4*ct+3 of the tile
+    const uint32_t bsw = p.big_endian ? 0x11u : 0u;
+    // dp2a operands: (pixel v of frame f, of frame f+1) as two 16-bit halves; QLD_U16_BE swaps the bytes of each half
+    const uint32_t sel_lo = p.big_endian ? 0x4501u : 0x5410u, sel_hi = p.big_endian ? 0x6723u : 0x7632u;
     double wsum[ROWS];
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) wsum[r] = 0.0;
@@ -321,10 +324,10 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                         if constexpr (sizeof(T) == 2) {
                             const uint2 f0 = *reinterpret_cast<const uint2 *>(d + (size_t)(2 * q) * SEG);
                             const uint2 f1 = *reinterpret_cast<const uint2 *>(d + (size_t)(2 * q + 1) * SEG);
-                            px[0] = __byte_perm(f0.x, f1.x, 0x5410);
-                            px[1] = __byte_perm(f0.x, f1.x, 0x7632);
-                            px[2] = __byte_perm(f0.y, f1.y, 0x5410);
-                            px[3] = __byte_perm(f0.y, f1.y, 0x7632);
+                            px[0] = __byte_perm(f0.x, f1.x, sel_lo);
+                            px[1] = __byte_perm(f0.x, f1.x, sel_hi);
+                            px[2] = __byte_perm(f0.y, f1.y, sel_lo);
+                            px[3] = __byte_perm(f0.y, f1.y, sel_hi);
 #pragma unroll
                             for (int r = 0; r < ROWS; ++r)
 #pragma unroll
@@ -358,14 +361,14 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             load_weights_shared<ACC, ROWS>(wrow + (fr + u) * ROWS, wt[u]);
                         }
 #pragma unroll
-                        for (int u = 0; u < 4; ++u) accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc);
+                        for (int u = 0; u < 4; ++u) accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc, bsw);
                     }
                     for (; fr < nf; ++fr) {
                         uint32_t w[PX::NW];
                         ACC wt[ROWS];
                         PX::load_shared(d + (size_t)fr * SEG, w);
                         load_weights_shared<ACC, ROWS>(wrow + fr * ROWS, wt);
-                        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc);
+                        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc, bsw);
                     }
                 }
                 __syncwarp();

@@ -329,6 +329,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
     }
 
     // ===== consumers =====
+    const uint32_t bsw = p.big_endian ? 0x11u : 0u;
     const int cw = warp - 1, cg = cw % CG, ts = cw / CG;
     const int col = (cg * 32 + lane) * VB;                 // byte offset of this thread's pixels inside the segment
     const int tcol = cg * 32 + lane;                       // thread column inside the tile
@@ -411,7 +412,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
                         uint32_t w0[PX::NW];
                         PX::load_shared(d, w0);
 #pragma unroll
-                        for (int v = 0; v < V; ++v) pedm[v] = PX::getf_biased(w0, v);
+                        for (int v = 0; v < V; ++v) pedm[v] = PX::getf_biased(w0, v, bsw);
                     }
                 }
                 int f = ts;
@@ -428,9 +429,9 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
 #pragma unroll
                         for (int u = 0; u < 4; ++u) {
                             if constexpr (IS_INT) {
-                                if (p.onehot) { accumulate_onehot<T, ROWS, V>(w[u], wt[u], acc); continue; }
+                                if (p.onehot) { accumulate_onehot<T, ROWS, V>(w[u], wt[u], acc, bsw); continue; }
                             }
-                            accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc);
+                            accumulate<T, ACC, ROWS, V>(w[u], wt[u], pedm, acc, bsw);
                         }
                     }
                 } else {
@@ -440,9 +441,9 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
                         PX::load_shared(d + (size_t)f * SEG, w);
                         load_weights_shared<ACC, ROWS>(wrow + f * ROWS, wt);
                         if constexpr (IS_INT) {
-                            if (p.onehot) { accumulate_onehot<T, ROWS, V>(w, wt, acc); continue; }
+                            if (p.onehot) { accumulate_onehot<T, ROWS, V>(w, wt, acc, bsw); continue; }
                         }
-                        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc);
+                        accumulate<T, ACC, ROWS, V>(w, wt, pedm, acc, bsw);
                     }
                 }
                 __syncwarp();

@@ -397,11 +397,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                         v[rr] = (long long)(int)r[g][4 * rr] + ((long long)(int)r[g][4 * rr + 1] << 8) + ((long long)(int)r[g][4 * rr + 2] << 16) +
                                 ((long long)(int)r[g][4 * rr + 3] << 24);
                     if (BYTES == 2) {
-                        // even row = low byte, odd row = high byte of the same pixel: x = lo + 256 * hi
+                        // even row = low byte, odd row = high byte of the same pixel (the other way round for QLD_U16_BE): x = lo + 256 * hi
 #pragma unroll
                         for (int rr = 0; rr < 4; ++rr) {
                             const long long o = __shfl_xor_sync(0xffffffffu, v[rr], 1);
-                            v[rr] = (lane & 1) ? (o + (v[rr] << 8)) : (v[rr] + (o << 8));
+                            v[rr] = (((lane & 1) != 0) != (p.big_endian != 0)) ? (o + (v[rr] << 8)) : (v[rr] + (o << 8));
                         }
                     }
                     // this group holds references 2g and 2g+1; with 16-bit samples the lane pair splits them

@@ -15,7 +15,7 @@ struct TcParams {
     unsigned int *tile_counter; // device counter for the dynamic tile scheduler: zero on entry
     unsigned int *tile_counter_next; // the next launch's counter, zeroed by this launch (the two alternate)
     int32_t force_T, force_stages, force_kc;   // debug override of the tile shape (qld_debug_set_tile), 0 = automatic
-    int32_t reserved;
+    int32_t big_endian;       // 16-bit samples most significant byte first: the even accumulator row is the high byte
     FinParams fin;
 };
 

@@ -14,7 +14,7 @@ from typing import Optional, Sequence
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libqld.so")
 
-QLD_U8, QLD_U16 = 0, 1
+QLD_U8, QLD_U16, QLD_U16_BE = 0, 1, 2
 QLD_OK, QLD_E_INVAL, QLD_E_NOMEM, QLD_E_CUDA, QLD_E_STATE, QLD_E_OVERRUN, QLD_E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 QLD_ACC_AUTO, QLD_ACC_FP32, QLD_ACC_INT_BINS, QLD_ACC_FIXED = 0, 1, 2, 3
 QLD_NORM_PAPER, QLD_NORM_AMPLITUDE = 0, 1
@@ -132,7 +132,7 @@ class QLD:
         self._torch = torch
         self.lib = load_library()
         self.H, self.W, self.N, self.K = int(H), int(W), int(N), len(refs)
-        self.dtype = QLD_U8 if str(dtype) in ("u8", "uint8", "torch.uint8", "0") else QLD_U16
+        self.dtype = QLD_U8 if str(dtype) in ("u8", "uint8", "torch.uint8", "0") else (QLD_U16_BE if str(dtype) in ("u16be", "2") else QLD_U16)
         self._refs = make_refs(refs)
         cfg = qld_config()
         cfg.H, cfg.W, cfg.dtype, cfg.N, cfg.K = self.H, self.W, self.dtype, self.N, self.K

@@ -614,3 +614,64 @@ def test_slide_bulk_kernel(Q, oracle, accum_name, refs, hop, cap, partial, dtype
                 B = oracle.bins(stream[a:a + N], num, den, s_first=a + 1)
                 assert np.array_equal(ctx.get_bins(k).cpu().numpy(), B[:den // 2] - B[den // 2:]), f"window {w} k={k}"
     ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ f4: camera byte stream
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("path", ["whole_fp32", "whole_bins", "stream_fp32", "stream_bins", "stream_bins_k2", "tc_fixed", "slide_small", "slide_bulk_bins",
+                                  "slide_bulk_fp32", "slide_partial"])
+def test_big_endian_byte_stream(Q, oracle, path):
+    """QLD_U16_BE (the camera's 16-bit stream, pairs of bytes stitched into values): the bytes arrive most
+    significant first and are joined inside the kernels' loads.  Oracle: stitch on the host, then the definition."""
+    rng = np.random.default_rng(len(path))
+    H, W, N = 24, 128, 96
+    x = rng.integers(0, 65536, size=(N + 6 * 16, H, W)).astype(np.uint16)      # full range: both bytes matter
+    raw = x.byteswap()                                                          # what the wire carries, viewed as uint16 words
+    assert np.array_equal(raw.view(np.uint8).reshape(-1, 2)[:, 0].astype(np.uint16) * 256 + raw.view(np.uint8).reshape(-1, 2)[:, 1], x.reshape(-1))
+    ring = path.startswith("slide")
+    hop = 32 if path == "slide_partial" else 16               # the partial-sum seeding needs a hop of at least one stage
+    kw = dict(max_value=65535)
+    if path in ("whole_fp32", "stream_fp32", "slide_small", "slide_bulk_fp32"):
+        refs, kw["accum"] = [{"nu": 0.0937, "phase": 0.3}], Q.QLD_ACC_FP32
+    elif path == "stream_bins_k2":
+        refs, kw["accum"] = [{"num": 1, "den": 4}, {"num": 1, "den": 8}], Q.QLD_ACC_INT_BINS
+    elif path == "tc_fixed":
+        refs, kw["accum"] = [{"nu": 0.0937}, {"num": 1, "den": 6}], Q.QLD_ACC_FIXED
+    else:
+        refs, kw["accum"] = [{"num": 1, "den": 6}], Q.QLD_ACC_INT_BINS
+    if path.startswith("stream"):
+        kw["debug_tile"] = ("stream", 1024, 16)
+    if ring:
+        kw["ring_frames"] = N + 40
+        kw["resync_hops"] = -1
+    if path == "slide_partial":
+        kw["slide_hop"] = hop
+        kw["debug_tile"] = ("stream", 512, 16)
+    ctx = Q.QLD(H, W, "u16be", N, refs, **kw)
+    if path.startswith("slide_bulk") or path == "slide_partial":
+        ctx.debug_set_tile("slide", 1)
+    ctx.push_frames(raw[:N])
+    tol = 1e-5 if kw["accum"] == Q.QLD_ACC_FP32 else 1e-6
+    if not ring:
+        ctx.demod(Q.QLD_WHOLE)
+        ctx.sync()
+        for k, ref in enumerate(refs):
+            check_float_maps(_maps(ctx, k), oracle_maps(oracle, x[:N], ref), rel=tol, what=f"{path} k={k}")
+        if kw["accum"] == Q.QLD_ACC_INT_BINS:
+            B = oracle.bins(x[:N], refs[0]["num"], refs[0]["den"])
+            h = refs[0]["den"] // 2
+            assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:h] - B[h:])
+    else:
+        ctx.demod(Q.QLD_SLIDE, hop)
+        for w in range(96 // hop + 1):
+            if w > 0:
+                ctx.push_frames(raw[N + (w - 1) * hop:N + w * hop])
+                ctx.demod(Q.QLD_SLIDE, hop)
+                assert (ctx.last_kernel() == "k_slide_bulk") == (path != "slide_small")
+            ctx.sync()
+            a = w * hop
+            check_float_maps(_maps(ctx, 0), oracle_maps(oracle, x[a:a + N], refs[0], s_first=a + 1), rel=tol, what=f"{path} window {w}")
+            if kw["accum"] == Q.QLD_ACC_INT_BINS:
+                B = oracle.bins(x[a:a + N], 1, 6, s_first=a + 1)
+                assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:3] - B[3:]), f"window {w}"
+    ctx.destroy()
