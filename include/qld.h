@@ -118,6 +118,12 @@ typedef struct {
                                 (H*W*bytes a multiple of 16, at least one 2 KB segment per SM, slide_hop >= 16..64
                                 depending on the frame size): QLD_E_UNSUPPORTED otherwise.  Results are identical to the
                                 frame re-reading update (bit-exact for INT_BINS). */
+    int32_t window_relative; /* ring contexts: 1 = the I, Q and phase maps of a window that starts after a frames are turned back by
+                                2 pi nu a, i.e. they are what references counted from the window's own first frame (s = 1)
+                                would give: successive windows of a steady source then show a steady phase (reading G10,
+                                P:181-183).  0 (default): references by absolute frame index.  The amplitude is the same either
+                                way; qld_get_bins / qld_get_sums_i64 always hold absolute-index sums. */
+    int32_t reserved2;
     int32_t ref_tables_supplied; /* 1: the caller supplies every reference table with qld_set_ref_tables before the first
                                 qld_demod (QLD_E_STATE otherwise); refs[k].nu / num / den are then not used and not validated, so
                                 nu = 0 and nu = 1/2 (reading G18) can be expressed.  FP32 / FIXED (or AUTO) on whole-window stores. */

@@ -41,6 +41,7 @@ struct qld_ctx {
     // configuration
     int H, W, dtype, bytes, N, K, accum, norm, maps, resync_hops;
     int big_endian;          // QLD_U16_BE: byte pairs stitched most significant byte first
+    int window_relative;     // cfg.window_relative: I / Q / phase maps turned back to window-relative references
     int64_t HW;
     uint32_t max_value;
     int cap, cap_w;          // frame store capacity, weight table capacity
@@ -158,6 +159,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     if (cfg->slide_hop > 0 && cfg->ring_frames <= 0) return bad(QLD_E_INVAL, "slide_hop needs a ring context");
     if (cfg->norm != QLD_NORM_PAPER && cfg->norm != QLD_NORM_AMPLITUDE) return bad(QLD_E_INVAL, "unknown norm");
     if (cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64)) return bad(QLD_E_INVAL, "unknown bits in maps");
+    if (cfg->window_relative != 0 && cfg->window_relative != 1) return bad(QLD_E_INVAL, "window_relative must be 0 or 1");
     if (cfg->ref_tables_supplied != 0 && cfg->ref_tables_supplied != 1) return bad(QLD_E_INVAL, "ref_tables_supplied must be 0 or 1");
     if (cfg->ref_tables_supplied && cfg->ring_frames > 0) return bad(QLD_E_UNSUPPORTED, "ref_tables_supplied: whole-window stores only");
     if (cfg->ref_tables_supplied && cfg->accum == QLD_ACC_INT_BINS) return bad(QLD_E_UNSUPPORTED, "ref_tables_supplied: FP32 or FIXED accumulation");
@@ -405,7 +407,22 @@ FinParams fin_with_maps(const qld_ctx *c)
 {
     FinParams f = c->fin;
     f.I = c->mapI; f.Q = c->mapQ; f.amp = c->mapA; f.phase = c->mapP;
+    f.rot = (c->window_relative && c->ring) ? reinterpret_cast<const double *>(reinterpret_cast<const unsigned char *>(c->tile_counter) + 256) : nullptr;
     return f;
+}
+
+// window-relative maps: the rotation factors of the window that starts after `a` frames, ahead of the demod kernel
+int set_window_rotation(qld_ctx *c, int64_t a)
+{
+    if (!(c->window_relative && c->ring)) return QLD_OK;
+    TableFillParams tp;
+    memset(&tp, 0, sizeof tp);
+    tp.K = c->K;
+    for (int k = 0; k < c->K; ++k) tp.ref[k] = c->ref[k];
+    double *rot = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(c->tile_counter) + 256);
+    CU(c, qld_launch_window_rotation(tp, a, rot, c->s_comp));
+    c->launches++;
+    return QLD_OK;
 }
 
 int record_demod(qld_ctx *c, int64_t oldest_read)
@@ -689,6 +706,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     if (!c) return fail(nullptr, QLD_E_NOMEM, "host allocation failed");
     c->H = pl.H; c->W = pl.W; c->dtype = pl.dtype; c->bytes = pl.bytes; c->N = pl.N; c->K = pl.K;
     c->big_endian = pl.dtype == QLD_U16_BE ? 1 : 0;
+    c->window_relative = cfg->window_relative == 1;
     c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops;
     c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
     c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
@@ -821,7 +839,8 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (mode == QLD_WHOLE) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames stored");
         const int64_t a = c->ring ? c->pushed - c->N : 0;
-        int rc = c->ring ? seed_window(c, a) : run_whole(c, a, false);
+        int rc = set_window_rotation(c, a);
+        if (rc == QLD_OK) rc = c->ring ? seed_window(c, a) : run_whole(c, a, false);
         if (rc) return rc;
         if (c->ring) { c->seeded = true; c->win_start = a; c->hops_since_seed = 0; }
         c->windows_done++;
@@ -830,7 +849,8 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (!c->ring) return fail(c, QLD_E_STATE, "demod: QLD_SLIDE needs a ring context (ring_frames > N)");
     if (!c->seeded) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames pushed");
-        int rc = seed_window(c, 0);
+        int rc = set_window_rotation(c, 0);
+        if (rc == QLD_OK) rc = seed_window(c, 0);
         if (rc) return rc;
         c->seeded = true; c->win_start = 0; c->hops_since_seed = 0; c->windows_done++;
         return QLD_OK;
@@ -838,7 +858,8 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (hop < 1 || hop > c->N) return fail(c, QLD_E_INVAL, "demod: hop must be 1..N");
     if (c->slide_hop > 0 && hop != c->slide_hop) return fail(c, QLD_E_INVAL, "demod: this context slides by cfg.slide_hop only");
     if (c->pushed < c->win_start + hop + c->N) return fail(c, QLD_E_STATE, "demod: fewer than hop new frames pushed");
-    int rc;
+    int rc = set_window_rotation(c, c->win_start + hop);
+    if (rc) return rc;
     // FP32 ring sums random-walk away from a recompute (each hop adds rounding of its own): resynchronise from the ring
     // every resync_hops hops; 0 = automatic (16 windows' worth of hops: 1/16 more traffic), negative = never
     const int64_t resync = c->resync_hops > 0 ? c->resync_hops : (c->resync_hops == 0 ? 16 * (int64_t)((c->N + hop - 1) / hop) : 0);

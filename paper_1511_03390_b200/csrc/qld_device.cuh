@@ -232,6 +232,18 @@ __device__ __forceinline__ void accumulate_onehot(const uint32_t (&w)[Pix<T, V>:
     }
 }
 
+// window-relative I / Q: turn (I, Q) = (S, C) of reference k back by the angle the absolute-index references are ahead
+// (I' = I cos d - Q sin d, Q' = Q cos d + I sin d); rot == nullptr: nothing to do
+__device__ __forceinline__ void rotate_iq(const double *rot, int k, double &S, double &C)
+{
+    if (rot) {
+        const double c = rot[2 * k], s = rot[2 * k + 1];
+        const double S2 = S * c - C * s;
+        C = C * c + S * s;
+        S = S2;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // A4: finalise one pixel from its ROWS sums (already including the pedestal term), all in fp64.
 // ---------------------------------------------------------------------------------------------------
@@ -256,6 +268,7 @@ __device__ __forceinline__ void finalise_pixel(const FinParams &f, const double 
                     C = val[r + 1];
                 }
         }
+        rotate_iq(f.rot, k, S, C);
         S *= f.scale;
         C *= f.scale;
         const int64_t o = (int64_t)k * HW + pixel;
@@ -273,6 +286,7 @@ __device__ __forceinline__ void finalise_pixel_t(const FinParams &f, const RED (
                                                  int64_t HW)
 {
     auto emit = [&](int k, double S, double C) {
+        rotate_iq(f.rot, k, S, C);
         S *= f.scale;
         C *= f.scale;
         const int64_t o = (int64_t)k * HW + pixel;

@@ -29,6 +29,8 @@ struct FinParams {
     double cw[QLD_MAX_ROWS];
     double scale;            // 1 (PAPER) or 2/N (AMPLITUDE)
     float *I, *Q, *amp, *phase;   // [K][HW] or null
+    const double *rot;       // window-relative I/Q (reading G10): device array {cos d_k, sin d_k}, d_k = 2 pi nu_k (frames before
+                             // the window); null: references by absolute frame index only
 };
 
 // A run of consecutive store slots (no wrap inside a run) whose frames enter the sums with weight sign * w:
@@ -102,6 +104,8 @@ cudaError_t qld_launch_demod_slide(int dtype, int is_int, int rows, const SlideP
 cudaError_t qld_launch_table_fill(const TableFillParams &p, cudaStream_t st);
 // rows (row0, row0 + 1) of the float table from caller-supplied doubles tab[2][n] (sin, cos), frames 1..n; recomputes cum
 cudaError_t qld_launch_table_from_doubles(const double *tab, int n, int row0, int rows, int cap_w, void *wtab, double *cum, cudaStream_t st);
+// rot[2k], rot[2k+1] = cos, sin of 2 pi nu_k a (a = frames before the window), exactly reduced
+cudaError_t qld_launch_window_rotation(const TableFillParams &p, int64_t a, double *rot, cudaStream_t st);
 cudaError_t qld_launch_bin_weights(const TableFillParams &p, double *out32 /* device: sw[16], cw[16] */, cudaStream_t st);
 int qld_pixels_per_thread(int dtype, int rows, int64_t HW, const void *frames, int64_t frame_stride);
 

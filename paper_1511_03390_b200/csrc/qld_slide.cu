@@ -423,6 +423,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             C = (double)a[r + 1][v] + (double)pedf[v] * wsum[r + 1];
                         }
                 }
+                rotate_iq(f.rot, k, S, C);
                 S *= f.scale;
                 C *= f.scale;
                 o[0][v] = (float)S;

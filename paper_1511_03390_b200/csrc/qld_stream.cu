@@ -270,6 +270,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
                         S[j] = (double)a[j][0] + pedv[j] * wsum.a[0];       // sum x w = sum (x - ped) w + ped * sum w
                         C[j] = (double)a[j][1] + pedv[j] * wsum.a[1];
                     }
+                    rotate_iq(f.rot, 0, S[j], C[j]);
                     S[j] *= f.scale;
                     C[j] *= f.scale;
                 }
@@ -548,6 +549,7 @@ k_demod_stream(const __grid_constant__ CUtensorMap tmap, const __grid_constant__
                                 C = (double)a[r + 1][v] + (double)pedf[v] * wc;
                             }
                     }
+                    rotate_iq(f.rot, k, S, C);
                     S *= f.scale;
                     C *= f.scale;
                     oI[v] = (float)S;

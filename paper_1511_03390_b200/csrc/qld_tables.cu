@@ -104,7 +104,28 @@ __global__ void k_table_from_doubles(const double *tab, int n, int row0, int row
     }
 }
 
+// Window-relative I / Q (reading G10): a window that starts after `a` frames sees references that are
+// d = 2 pi nu a ahead of window-relative ones; the epilogues turn (I, Q) back by d.  rot = {cos d, sin d} per reference.
+__global__ void k_window_rotation(const TableFillParams p, int64_t a, double *rot)
+{
+    const int k = threadIdx.x;
+    if (k >= p.K) return;
+    RefPlan rf = p.ref[k];
+    rf.phase = 0.0;
+    rf.phase_quarter = 0;
+    double sn, cs;
+    sincospi(half_turns_of(rf, a), &sn, &cs);
+    rot[2 * k] = cs;
+    rot[2 * k + 1] = sn;
+}
+
 }  // namespace
+
+cudaError_t qld_launch_window_rotation(const TableFillParams &p, int64_t a, double *rot, cudaStream_t st)
+{
+    k_window_rotation<<<1, 32, 0, st>>>(p, a, rot);
+    return cudaGetLastError();
+}
 
 cudaError_t qld_launch_table_from_doubles(const double *tab, int n, int row0, int rows, int cap_w, void *wtab, double *cum, cudaStream_t st)
 {

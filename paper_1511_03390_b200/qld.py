@@ -39,7 +39,7 @@ class qld_config(C.Structure):
     _fields_ = [("H", C.c_int32), ("W", C.c_int32), ("dtype", C.c_int32), ("N", C.c_int32), ("K", C.c_int32),
                 ("refs", C.POINTER(qld_ref)), ("ring_frames", C.c_int32), ("accum", C.c_int32), ("norm", C.c_int32),
                 ("maps", C.c_int32), ("max_value", C.c_uint32), ("resync_hops", C.c_int32), ("external_store", C.c_int32),
-                ("slide_hop", C.c_int32), ("ref_tables_supplied", C.c_int32),
+                ("slide_hop", C.c_int32), ("window_relative", C.c_int32), ("reserved2", C.c_int32), ("ref_tables_supplied", C.c_int32),
                 ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
                 ("compute_stream", C.c_void_p), ("copy_stream", C.c_void_p)]
 
@@ -127,7 +127,7 @@ class QLD:
                  accum: int = QLD_ACC_AUTO, norm: int = QLD_NORM_PAPER, maps: int = QLD_MAP_ALL, max_value: int = 0,
                  resync_hops: int = 0, device=None, copy_stream=None, torch_workspace: bool = True,
                  external_store: bool = False, slide_hop: int = 0, debug_tile=None,
-                 ref_tables_supplied: bool = False):
+                 ref_tables_supplied: bool = False, window_relative: bool = False):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -141,6 +141,7 @@ class QLD:
         cfg.max_value, cfg.resync_hops, cfg.external_store = int(max_value), int(resync_hops), int(bool(external_store))
         cfg.slide_hop = int(slide_hop)
         cfg.ref_tables_supplied = int(bool(ref_tables_supplied))
+        cfg.window_relative = int(bool(window_relative))
         self._ctx = C.c_void_p()
         nbytes = C.c_size_t()
         rc = self.lib.qld_workspace_bytes(C.byref(cfg), C.byref(nbytes))

@@ -675,3 +675,46 @@ def test_big_endian_byte_stream(Q, oracle, path):
                 B = oracle.bins(x[a:a + N], 1, 6, s_first=a + 1)
                 assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:3] - B[3:]), f"window {w}"
     ctx.destroy()
+
+
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("path", ["small", "stream", "bulk", "bulk_partial"])
+@pytest.mark.parametrize("accum_name,refs", [("INT_BINS", [{"num": 1, "den": 6}]), ("FP32", [{"nu": 0.0937, "phase": 0.3}]),
+                                             ("FP32", [{"nu": 0.21, "phase": -1.0}, {"num": 3, "den": 16}])])
+def test_window_relative_maps(Q, oracle, path, accum_name, refs):
+    """cfg.window_relative (reading G10): the I, Q and phase maps of every window equal the definition with the frame index
+    counted from the window's own first frame (s = 1) -- a steady source shows a steady phase from window to
+    window -- while the integer bins stay the absolute-index sums."""
+    rng = np.random.default_rng(11)
+    H, W, N, hop = 16, 128, 128, 32
+    T = N + 6 * hop
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    kw = dict(ring_frames=N + 2 * hop + 5, accum=getattr(Q, "QLD_ACC_" + accum_name), max_value=4095, window_relative=True, resync_hops=3)
+    if path in ("stream", "bulk_partial"):
+        kw["debug_tile"] = ("stream", 512, 16)
+    if path == "bulk_partial":
+        kw["slide_hop"] = hop
+    ctx = Q.QLD(H, W, "u16", N, refs, **kw)
+    if path.startswith("bulk"):
+        ctx.debug_set_tile("slide", 1)
+    elif path == "stream":
+        ctx.debug_set_tile("slide", 2)
+    ctx.push_frames(stream[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    for w in range(7):
+        if w > 0:
+            ctx.push_frames(stream[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+        ctx.sync()
+        a = w * hop
+        for k, ref in enumerate(refs):
+            ora = oracle_maps(oracle, stream[a:a + N], ref, s_first=1)                 # window-relative: the window's first frame is s = 1
+            check_float_maps(_maps(ctx, k), ora, rel=1e-6 if accum_name == "INT_BINS" else 1e-5, what=f"{path} window {w} k={k}")
+        if accum_name == "INT_BINS":
+            B = oracle.bins(stream[a:a + N], 1, 6, s_first=a + 1)                      # bins: absolute frame index
+            assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:3] - B[3:])
+    # a whole-window demod on the ring (most recent N frames) is window-relative too
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    check_float_maps(_maps(ctx, 0), oracle_maps(oracle, stream[T - N:T], refs[0], s_first=1), rel=1e-6 if accum_name == "INT_BINS" else 1e-5, what="whole on ring")
+    ctx.destroy()
