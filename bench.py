@@ -386,7 +386,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     kernel = ctx.last_kernel()
     mode = ctx.accum_name()
     n_rows = ctx.get_bins(0).shape[0] if mode == "INT_BINS" else 2 * K
-    acc_bytes = 4 if mode == "INT_BINS" else 8
+    acc_bytes = 4 if mode == "INT_BINS" else 8                # int32 bins; fp64 (FP32 mode) or int64 (FIXED) stored sums
     samples = float(hop) * H * W                              # new pixel-samples consumed per step
     res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
            "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel, "gpu_launches": int(launches),
@@ -410,7 +410,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     res["roofline"]["frac_moved"] = res["roofline"]["frac"]
     res["roofline"]["survey_A5_bytes_per_launch"] = survey
     res["roofline"]["frac_survey_A5"] = survey / (ms / steps * 1e-3) / 1e9 / peak
-    res["dtype"] = {"INT_BINS": "int32", "FP32": "f32"}[mode]
+    res["dtype"] = {"INT_BINS": "int32", "FP32": "f32", "FIXED": "int64 (Q1.30 references)"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "hop": hop, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": "amplitude", "step": "qld_commit_frames(hop) + qld_demod(QLD_SLIDE, hop) over the resident ring",
                      "update": "block partial sums (cfg.slide_hop = hop): only the new frames are read" if slide_hop else "expired frames re-read",

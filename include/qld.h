@@ -68,7 +68,11 @@ typedef enum {
  *             computed on the tcgen05 tensor cores as a [pixel bytes x frames].[frames x reference digits]
  *             int8 contraction (A6).  Bit-exact against an integer oracle with the same
  *             table; |R*2^-30 - sin| <= 2^-31, so the maps also agree with the float definition to ~1e-9.
- *             Whole-window stores only (ring_frames 0 or -1), H*W*bytes a multiple of 16, N <= 65536.
+ *             Whole-window stores (ring_frames 0 or -1): H*W*bytes a multiple of 16, N <= 65536.
+ *             Rings (ring_frames > N, at most 2 references): the same exact sums, kept as int64 across hops by the
+ *             bulk-copy sliding kernel (64-bit integer multiply-add on the CUDA cores) -- the sliding window of P:181-183
+ *             with float references and no drift at all, at any nu; the table entry of a frame is a function of its
+ *             absolute index and is extended per push.
  *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds; else FIXED for
  *             K >= 4 references on a whole-window store that meets FIXED's conditions (the CUDA-core kernel is
  *             instruction-bound there, the contraction is HBM-bound and more accurate than fp32); else FP32. */
@@ -220,9 +224,11 @@ int qld_set_ref_tables(qld_ctx *ctx, int k, const double *sin_tab, const double 
  * arrays of n == N entries, entry i belongs to frame i+1, each in [-2^30, 2^30]); blocks until the device
  * table is rebuilt.  qld_read_ref_table_fixed copies the table in use back to the host (blocks). */
 int qld_set_ref_table_fixed(qld_ctx *ctx, int k, const int32_t *sin_q30, const int32_t *cos_q30, int n);
+/* N entries each.  Whole-window store: frames 1..N.  Ring: the N most recently pushed frames. */
 int qld_read_ref_table_fixed(qld_ctx *ctx, int k, int32_t *sin_q30, int32_t *cos_q30);
 
-/* QLD_ACC_FIXED with QLD_MAP_SUMS_I64: device pointers to the exact sums sum_s x_s R(s) of reference k,
+/* QLD_ACC_FIXED with QLD_MAP_SUMS_I64 (whole-window stores) or QLD_ACC_FIXED on a ring (always available: the sums the
+ * context keeps across hops): device pointers to the exact sums sum_s x_s R(s) of reference k over the current window,
  * [H][W] int64 each (I*2^30 and Q*2^30 before normalisation), valid like the maps. */
 int qld_get_sums_i64(qld_ctx *ctx, int k, const int64_t **I, const int64_t **Q);
 

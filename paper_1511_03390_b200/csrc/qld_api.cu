@@ -47,6 +47,7 @@ struct qld_ctx {
     int cap, cap_w;          // frame store capacity, weight table capacity
     bool ring, external;     // ring buffer / frames attached by the caller
     bool is_int, is_fixed;
+    bool fix_ring;           // FIXED on a ring: Q1.30 references, int64 sums kept across hops by k_slide_bulk
     int rows, rows_pad;
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
@@ -133,7 +134,7 @@ int64_t gcd64(int64_t a, int64_t b) { while (b) { int64_t t = a % b; a = b; b = 
 
 struct Plan {
     int H, W, dtype, bytes, N, K, accum, norm, maps, cap, cap_w, rows, rows_pad;
-    bool ring, external, is_int, is_fixed;
+    bool ring, external, is_int, is_fixed, fix_ring;
     int64_t HW;
     RefPlan ref[QLD_MAX_K];
     FinParams fin;
@@ -226,15 +227,22 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         if (!bins_rows(&rows)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
         if (!bins_fit()) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
     }
-    if (acc == QLD_ACC_FIXED) {
-        if (pl->ring) return bad(QLD_E_UNSUPPORTED, "FIXED (tensor-core) accumulation works on whole-window stores, not rings");
+    if (acc == QLD_ACC_FIXED && pl->ring) {
+        if (cfg->K > 2) return bad(QLD_E_UNSUPPORTED, "FIXED on a ring: at most 2 references");
+        if ((pl->HW * pl->bytes) % 16 != 0) return bad(QLD_E_UNSUPPORTED, "FIXED: H*W*bytes_per_sample must be a multiple of 16");
+        if ((int64_t)cfg->N > 65536) return bad(QLD_E_UNSUPPORTED, "FIXED: N must be <= 65536");
+        const int nm = cfg->K * (((pl->maps & QLD_MAP_I) != 0) + ((pl->maps & QLD_MAP_Q) != 0) + ((pl->maps & QLD_MAP_AMP) != 0) + ((pl->maps & QLD_MAP_PHASE) != 0));
+        if (qld_slide_shape(cfg->dtype, 2, cfg->K == 1 ? 2 : 4, cfg->slide_hop > 0, nm, pl->HW, reinterpret_cast<const void *>(16), 1, 1).seg == 0)
+            return bad(QLD_E_UNSUPPORTED, "FIXED on a ring: the per-tile state (sums, partial sums, maps) does not fit shared memory: request fewer maps");
+    } else if (acc == QLD_ACC_FIXED) {
         if ((pl->HW * pl->bytes) % 16 != 0) return bad(QLD_E_UNSUPPORTED, "FIXED: H*W*bytes_per_sample must be a multiple of 16 (TMA row pitch)");
         if ((int64_t)cfg->N > 65536) return bad(QLD_E_UNSUPPORTED, "FIXED: N must be <= 65536 for exact int32 partial sums");
     }
     if ((pl->maps & QLD_MAP_SUMS_I64) && acc != QLD_ACC_FIXED) return bad(QLD_E_INVAL, "QLD_MAP_SUMS_I64 needs QLD_ACC_FIXED");
     pl->accum = acc;
     pl->is_int = acc == QLD_ACC_INT_BINS;
-    pl->is_fixed = acc == QLD_ACC_FIXED;
+    pl->is_fixed = acc == QLD_ACC_FIXED && !pl->ring;
+    pl->fix_ring = acc == QLD_ACC_FIXED && pl->ring;
     FinParams &f = pl->fin;
     f.K = cfg->K; f.is_int = pl->is_int;
     f.scale = cfg->norm == QLD_NORM_AMPLITUDE ? 2.0 / (double)cfg->N : 1.0;
@@ -291,7 +299,7 @@ int fill_tables(qld_ctx *c, int64_t s_first, int n, cudaStream_t st)
 {
     TableFillParams tp;
     memset(&tp, 0, sizeof tp);
-    tp.K = c->K; tp.is_int = c->is_int; tp.rows = c->rows_pad;
+    tp.K = c->K; tp.is_int = c->is_int ? 1 : (c->fix_ring ? 2 : 0); tp.rows = c->rows_pad;
     for (int k = 0; k < c->K; ++k) tp.ref[k] = c->ref[k];
     tp.s_first = s_first; tp.n = n; tp.cap_w = c->cap_w; tp.wtab = c->wtab; tp.cum = c->cum;
     CU(c, qld_launch_table_fill(tp, st));
@@ -518,7 +526,8 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
 int try_slide_bulk(qld_ctx *c, const DemodParams &p)
 {
     const int n_map_rows = c->K * ((c->mapI != nullptr) + (c->mapQ != nullptr) + (c->mapA != nullptr) + (c->mapP != nullptr));
-    const SlideShape sh = qld_slide_shape(c->dtype, c->is_int, c->rows_pad, p.part != nullptr, n_map_rows, c->HW, c->frames, c->n_sms, c->dbg_slide);
+    const int kind = c->is_int ? 1 : (c->fix_ring ? 2 : 0);
+    const SlideShape sh = qld_slide_shape(c->dtype, kind, c->rows_pad, p.part != nullptr, n_map_rows, c->HW, c->frames, c->n_sms, c->fix_ring ? 1 : c->dbg_slide);
     if (sh.seg == 0) return 0;
     if (c->slide_tmap_frames != c->frames || sh.seg != c->slide_shape.seg || sh.kc != c->slide_shape.kc) {
         cudaError_t e = qld_slide_encode_tmap(c->slide_tmap, c->frames, c->HW * c->bytes, c->cap, sh);
@@ -528,7 +537,7 @@ int try_slide_bulk(qld_ctx *c, const DemodParams &p)
     }
     unsigned int *cur, *nxt;
     next_counters(c, &cur, &nxt);
-    cudaError_t e = qld_launch_slide_bulk(c->dtype, c->is_int, c->rows_pad, c->slide_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp);
+    cudaError_t e = qld_launch_slide_bulk(c->dtype, kind, c->rows_pad, c->slide_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp);
     if (e != cudaSuccess) return cuda_fail(c, e, "qld_launch_slide_bulk");
     c->launches++;
     c->last_kernel = "k_slide_bulk";
@@ -558,6 +567,7 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
         const int rc = try_slide_bulk(c, q);
         if (rc != 0) return rc < 0 ? rc : QLD_OK;
     }
+    if (c->fix_ring) return fail(c, QLD_E_UNSUPPORTED, "FIXED on a ring: the state of a tile does not fit the bulk-copy kernel's shared memory");
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
     DemodParams p;
@@ -589,8 +599,40 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
 }
 
 // window a+1 .. a+N from scratch: the sums, and (block-partial mode) the N/hop per-batch partials
+// FIXED on a ring: the window from scratch through k_slide_bulk -- the stored sums (and partial sums) are zeroed and the
+// window's frames are "added" to them
+int seed_fix_ring(qld_ctx *c, int64_t a)
+{
+    const size_t rowset = (size_t)c->rows_pad * c->HW * 8;
+    CU(c, cudaMemsetAsync(c->acc, 0, rowset, c->s_comp));
+    if (c->slide_hop > 0) CU(c, cudaMemsetAsync(c->part, 0, rowset * c->n_part, c->s_comp));
+    const int n_launch = c->slide_hop > 0 ? c->n_part : 1;
+    for (int b = 0; b < n_launch; ++b) {
+        DemodParams q;
+        memset(&q, 0, sizeof q);
+        q.big_endian = c->big_endian;
+        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
+        q.cap = c->cap; q.cap_w = c->cap_w;
+        q.wtab = c->wtab; q.cum = c->cum;
+        q.acc_out = c->acc; q.acc_add = 1;
+        q.fin = fin_with_maps(c);
+        if (c->slide_hop > 0) {
+            q.part = c->part + (size_t)b * rowset;
+            q.part_sub = 1;
+            q.n_runs = add_runs(c, q.run, 0, a + (int64_t)b * c->slide_hop, c->slide_hop, +1);
+        } else {
+            q.n_runs = add_runs(c, q.run, 0, a, c->N, +1);
+        }
+        const int rc = try_slide_bulk(c, q);
+        if (rc < 0) return rc;
+        if (rc == 0) return fail(c, QLD_E_UNSUPPORTED, "FIXED on a ring: the state of a tile does not fit the bulk-copy kernel's shared memory");
+    }
+    return record_demod(c, a + 1);
+}
+
 int seed_window(qld_ctx *c, int64_t a)
 {
+    if (c->fix_ring) return seed_fix_ring(c, a);
     if (c->slide_hop == 0) return run_whole(c, a, true);
     for (int b = 0; b < c->n_part; ++b) {
         int rc = run_partial_batch(c, a, a + (int64_t)b * c->slide_hop, b, b > 0, false, b == 0);
@@ -626,6 +668,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         q.n_runs = add_runs(c, q.run, n, a_old + c->N, hop, +1);
         const int rc = try_slide_bulk(c, q);
         if (rc != 0) return rc < 0 ? rc : record_demod(c, a_old + 1);
+        if (c->fix_ring) return fail(c, QLD_E_UNSUPPORTED, "FIXED on a ring: the state of a tile does not fit the bulk-copy kernel's shared memory");
     }
     // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
@@ -709,7 +752,7 @@ int qld_create(const qld_config *cfg, qld_ctx **ctx_out)
     c->window_relative = cfg->window_relative == 1;
     c->accum = pl.accum; c->norm = pl.norm; c->maps = pl.maps; c->resync_hops = cfg->resync_hops;
     c->HW = pl.HW; c->max_value = cfg->max_value; c->cap = pl.cap; c->cap_w = pl.cap_w;
-    c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
+    c->ring = pl.ring; c->external = pl.external; c->is_int = pl.is_int; c->is_fixed = pl.is_fixed; c->fix_ring = pl.fix_ring; c->rows = pl.rows; c->rows_pad = pl.rows_pad;
     for (int k = 0; k < pl.K; ++k) c->ref[k] = pl.ref[k];
     c->fin = pl.fin;
     c->ws_bytes = pl.total;
@@ -863,7 +906,7 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     // FP32 ring sums random-walk away from a recompute (each hop adds rounding of its own): resynchronise from the ring
     // every resync_hops hops; 0 = automatic (16 windows' worth of hops: 1/16 more traffic), negative = never
     const int64_t resync = c->resync_hops > 0 ? c->resync_hops : (c->resync_hops == 0 ? 16 * (int64_t)((c->N + hop - 1) / hop) : 0);
-    if (!c->is_int && resync > 0 && c->hops_since_seed + 1 >= resync) {
+    if (!c->is_int && !c->fix_ring && resync > 0 && c->hops_since_seed + 1 >= resync) {
         rc = seed_window(c, c->win_start + hop);
         c->hops_since_seed = 0;
     } else {
@@ -910,7 +953,7 @@ int qld_read_map(qld_ctx *c, int k, int which, float *host_dst)
 int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out, float *cos_out)
 {
     if (!c || k < 0 || k >= c->K || n < 1 || s_first < 1) return c ? fail(c, QLD_E_INVAL, "read_ref_table: bad argument") : QLD_E_INVAL;
-    if (c->is_int || c->is_fixed) return fail(c, QLD_E_STATE, "read_ref_table: this context has no float table");
+    if (c->is_int || c->is_fixed || c->fix_ring) return fail(c, QLD_E_STATE, "read_ref_table: this context has no float table");
     if (c->ring && (s_first + n - 1 > c->pushed || s_first + c->cap_w <= c->pushed + 1)) return fail(c, QLD_E_STATE, "read_ref_table: frames not in the ring");
     if (!c->ring && s_first + n - 1 > c->N) return fail(c, QLD_E_INVAL, "read_ref_table: beyond the window");
     CU(c, cudaStreamSynchronize(c->s_copy));
@@ -977,6 +1020,19 @@ int qld_set_ref_table_fixed(qld_ctx *c, int k, const int32_t *sin_q30, const int
 int qld_read_ref_table_fixed(qld_ctx *c, int k, int32_t *sin_q30, int32_t *cos_q30)
 {
     if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "read_ref_table_fixed: bad argument") : QLD_E_INVAL;
+    if (c->fix_ring) {                                       // ring: the entries of the N most recently pushed frames
+        if (c->pushed < c->N) return fail(c, QLD_E_STATE, "read_ref_table_fixed: fewer than N frames pushed");
+        int rc = qld_sync(c);
+        if (rc) return rc;
+        for (int i = 0; i < c->N; ++i) {
+            const int64_t e = (c->pushed - c->N + 1 + i) % c->cap_w;
+            int32_t w[2];
+            CU(c, cudaMemcpy(w, static_cast<const int32_t *>(c->wtab) + e * c->rows_pad + 2 * k, sizeof w, cudaMemcpyDeviceToHost));
+            if (sin_q30) sin_q30[i] = w[0];
+            if (cos_q30) cos_q30[i] = w[1];
+        }
+        return QLD_OK;
+    }
     if (!c->is_fixed) return fail(c, QLD_E_STATE, "read_ref_table_fixed: context does not use QLD_ACC_FIXED");
     int rc = qld_sync(c);
     if (rc) return rc;
@@ -988,6 +1044,12 @@ int qld_read_ref_table_fixed(qld_ctx *c, int k, int32_t *sin_q30, int32_t *cos_q
 int qld_get_sums_i64(qld_ctx *c, int k, const int64_t **I, const int64_t **Q)
 {
     if (!c || k < 0 || k >= c->K) return c ? fail(c, QLD_E_INVAL, "get_sums_i64: k out of range") : QLD_E_INVAL;
+    if (c->fix_ring) {                                       // the stored sums of the current window are the exact int64 sums
+        int64_t *a = static_cast<int64_t *>(c->acc);
+        if (I) *I = a + (size_t)(2 * k) * c->HW;
+        if (Q) *Q = a + (size_t)(2 * k + 1) * c->HW;
+        return QLD_OK;
+    }
     if (!c->sums) return fail(c, QLD_E_STATE, "get_sums_i64: needs QLD_ACC_FIXED and QLD_MAP_SUMS_I64");
     if (I) *I = c->sums + (size_t)(2 * k) * c->HW;
     if (Q) *Q = c->sums + (size_t)(2 * k + 1) * c->HW;

@@ -90,7 +90,7 @@ struct SlideParams {
 };
 
 struct TableFillParams {
-    int32_t K, is_int, rows;        // rows = padded row count (table row stride)
+    int32_t K, is_int, rows;        // is_int: 0 float rows, 1 integer bin indicators, 2 Q1.30 integers; rows = padded row count (row stride)
     RefPlan ref[QLD_MAX_K];
     int64_t s_first;
     int32_t n, cap_w;

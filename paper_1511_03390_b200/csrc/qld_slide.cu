@@ -83,13 +83,18 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
              unsigned int *tile_counter, unsigned int *counter_next)
 {
     using PX = Pix<T, SL_V>;
+    // ACC = float: fp32 partial sums of pedestal-subtracted samples, fp64 stored sums;  ACC = int: integer phase bins (exact);
+    // ACC = long long: Q1.30 fixed-point references, exact int64 sums (drift-free sliding at any nu)
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
-    using RED = typename std::conditional<IS_INT, int, double>::type;
+    constexpr bool IS_FIX = std::is_same<ACC, long long>::value;
+    constexpr bool IS_F32 = std::is_same<ACC, float>::value;
+    using WT = typename std::conditional<IS_F32, float, int>::type;                        // weight table entries
+    using RED = typename std::conditional<IS_F32, double, ACC>::type;                      // stored sums
     constexpr int V = SL_V, TP = SL_TP;
     constexpr int VB = V * (int)sizeof(T);
 
     const int SEG = sh.seg, KC = sh.kc, STAGES = sh.stages, NSB = sh.nsb;
-    const SlideSmem SM(SEG, KC, STAGES, NSB, ROWS, (int)sizeof(RED), PART, !IS_INT, n_map_rows);
+    const SlideSmem SM(SEG, KC, STAGES, NSB, ROWS, (int)sizeof(RED), PART, IS_F32, n_map_rows);
 
     extern __shared__ unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
@@ -130,7 +135,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
 
     if (warp == 0) {
         // ===== producer: tile scheduler, state rows (bulk copies), frame boxes (TMA) + weight rows =====
-        const ACC *wtab = static_cast<const ACC *>(p.wtab);
+        const WT *wtab = static_cast<const WT *>(p.wtab);
         int stage = 0;
         uint32_t phase = 0;
         int next = (int)blockIdx.x;
@@ -158,18 +163,18 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                 mbar_wait(&state_empty[sb], (uint32_t)((it / NSB) & 1) ^ 1u);
                 unsigned char *st = sState + (size_t)sb * SM.state_bytes;
                 const uint32_t rb = (uint32_t)(npx * (int)sizeof(RED));
-                uint32_t bytes = (uint32_t)ROWS * rb * (PART ? 2u : 1u) + (IS_INT ? 0u : (uint32_t)(npx * 4));
+                uint32_t bytes = (uint32_t)ROWS * rb * (PART ? 2u : 1u) + (IS_F32 ? (uint32_t)(npx * 4) : 0u);
                 mbar_expect_tx(&state_full[sb], bytes);
 #pragma unroll
                 for (int r = 0; r < ROWS; ++r) {
                     bulk_load(st + SM.off_acc + (size_t)r * TP * sizeof(RED), accg + (int64_t)r * p.HW + pix0, rb, &state_full[sb]);
                     if (PART) bulk_load(st + SM.off_part + (size_t)r * TP * sizeof(RED), partg + (int64_t)r * p.HW + pix0, rb, &state_full[sb]);
                 }
-                if (!IS_INT) bulk_load(st + SM.off_ped, p.ped_in + pix0, (uint32_t)(npx * 4), &state_full[sb]);
+                if (IS_F32) bulk_load(st + SM.off_ped, p.ped_in + pix0, (uint32_t)(npx * 4), &state_full[sb]);
             }
             for (int run = 0; run < p.n_runs; ++run) {
                 const int rn = p.run[run].n, rslot = p.run[run].slot0, rw0 = p.run[run].w0;
-                const ACC sgn = (ACC)p.run[run].sign;
+                const WT sgn = (WT)p.run[run].sign;
                 for (int c0 = 0; c0 < rn; c0 += KC) {
                     const int nf = min(KC, rn - c0);
                     mbar_wait(&empty[stage], phase ^ 1);
@@ -201,7 +206,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             wdst[i] = (int)word;
                         }
                     } else {
-                        ACC *wdst = reinterpret_cast<ACC *>(smem + SM.off_w + (size_t)stage * SM.w_stage);
+                        WT *wdst = reinterpret_cast<WT *>(smem + SM.off_w + (size_t)stage * SM.w_stage);
                         for (int i = lane; i < nf * ROWS; i += 32) {
                             int e = rw0 + c0 + i / ROWS;
                             if (e >= p.cap_w) e -= p.cap_w;
@@ -263,7 +268,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     double wsum[ROWS];
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) wsum[r] = 0.0;
-    if constexpr (!IS_INT) {
+    if constexpr (IS_F32) {
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) wsum[r] = p.cum[(int64_t)p.cum_hi * ROWS + r] - p.cum[(int64_t)p.cum_lo * ROWS + r];
     }
@@ -292,7 +297,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
         float pedm[V], pedf[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) { pedm[v] = 8388608.0f; pedf[v] = 0.0f; }
-        if constexpr (!IS_INT) {
+        if constexpr (IS_F32) {
             // the pedestal the stored sums were seeded with (exact integer) is needed before the first frame
             mbar_wait(&state_full[sb], spar);
             const float4 pd = *reinterpret_cast<const float4 *>(st + SM.off_ped + (size_t)ct * 16);
@@ -349,6 +354,22 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                                 for (int v = 0; v < V; ++v) acc[r][v] = dp4a_u8_s8(px[v], wt[r], acc[r][v]);
                         }
                     }
+                } else if constexpr (IS_FIX) {
+                    // exact: unsigned sample times Q1.30 reference, 64-bit multiply-add
+                    const int *wrow = reinterpret_cast<const int *>(smem + SM.off_w + (size_t)stage * SM.w_stage);
+#pragma unroll 4
+                    for (int fr = 0; fr < nf; ++fr) {
+                        uint32_t w[PX::NW];
+                        int wt[ROWS];
+                        PX::load_shared(d + (size_t)fr * SEG, w);
+                        load_weights_shared<int, ROWS>(wrow + fr * ROWS, wt);
+#pragma unroll
+                        for (int v = 0; v < V; ++v) {
+                            const long long x = (long long)PX::geti(w, v, bsw);
+#pragma unroll
+                            for (int r = 0; r < ROWS; ++r) acc[r][v] += x * (long long)wt[r];
+                        }
+                    }
                 } else {
                     const ACC *wrow = reinterpret_cast<const ACC *>(smem + SM.off_w + (size_t)stage * SM.w_stage);
                     int fr = 0;
@@ -378,7 +399,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
         }
 
         // ---- update the stored sums (A5) in place in the state buffer, then A4 ----
-        if constexpr (IS_INT) mbar_wait(&state_full[sb], spar);
+        if constexpr (!IS_F32) mbar_wait(&state_full[sb], spar);
         RED a[ROWS][V];
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
@@ -415,6 +436,13 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             S = fma((double)a[r][v], f.sw[r], S);
                             C = fma((double)a[r][v], f.cw[r], C);
                         }
+                } else if constexpr (IS_FIX) {
+#pragma unroll
+                    for (int r = 0; r + 1 < ROWS; r += 2)
+                        if (r == 2 * k) {
+                            S = (double)a[r][v] * 9.31322574615478515625e-10;         // 2^-30
+                            C = (double)a[r + 1][v] * 9.31322574615478515625e-10;
+                        }
                 } else {
 #pragma unroll
                     for (int r = 0; r + 1 < ROWS; r += 2)
@@ -450,7 +478,8 @@ template <typename T, typename ACC, int ROWS, bool PART>
 cudaError_t launch_slide_n(const void *tmap, const DemodParams &p, const SlideShape &sh, int n_map_rows, unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
-    const SlideSmem SM(sh.seg, sh.kc, sh.stages, sh.nsb, ROWS, IS_INT ? 4 : 8, PART, !IS_INT, n_map_rows);
+    constexpr bool IS_F32 = std::is_same<ACC, float>::value;
+    const SlideSmem SM(sh.seg, sh.kc, sh.stages, sh.nsb, ROWS, IS_INT ? 4 : 8, PART, IS_F32, n_map_rows);
     auto kern = k_slide_bulk<T, ACC, ROWS, PART>;
     static int smem_set_dev[64] = {0};
     int dev = 0;
@@ -486,7 +515,7 @@ int count_map_rows(const DemodParams &p) { return p.fin.K * ((p.fin.I != nullptr
 // Shape for this (dtype, rows, frame size), or seg = 0 when the kernel does not apply: rows beyond 4, a row pitch or base that
 // is not 16-byte aligned, a frame too small to give every SM a tile (unless forced), or state buffers that leave no room for
 // two frame stages.  force: 0 automatic, 1 use it whatever the frame size, 2 never.
-SlideShape qld_slide_shape(int dtype, int is_int, int rows, int part, int n_map_rows, int64_t HW, const void *frames, int n_sms, int force)
+SlideShape qld_slide_shape(int dtype, int kind, int rows, int part, int n_map_rows, int64_t HW, const void *frames, int n_sms, int force)
 {
     SlideShape sh = {0, 0, 0, 0};
     if (force == 2 || rows > 4) return sh;
@@ -495,18 +524,20 @@ SlideShape qld_slide_shape(int dtype, int is_int, int rows, int part, int n_map_
     const int64_t n_tiles = (HW + SL_TP - 1) / SL_TP;
     if (force != 1 && n_tiles < n_sms) return sh;
     const int seg = SL_TP * bytes;
-    const int kc = 16;
-    const int budget = 224 * 1024;
-    for (int nsb = 3; nsb >= 2; --nsb) {
-        const SlideSmem one(seg, kc, 1, nsb, rows, is_int ? 4 : 8, part != 0, !is_int, n_map_rows);
-        const int fixed = nsb * one.state_bytes + 512;
-        int stages = (budget - fixed) / (one.data_stage + one.w_stage);
-        if (stages > 12) stages = 12;
-        if (stages >= (nsb == 3 ? 3 : 2)) {
-            sh.seg = seg; sh.kc = kc; sh.stages = stages; sh.nsb = nsb;
-            return sh;
+    const int budget = 226 * 1024;
+    // 16-frame stages with three state buffers when they fit; a large state (two references, partial sums, every map) leaves
+    // room for two buffers and shorter stages only
+    for (int kc = 16; kc >= 8; kc /= 2)
+        for (int nsb = 3; nsb >= 2; --nsb) {
+            const SlideSmem one(seg, kc, 1, nsb, rows, kind == 1 ? 4 : 8, part != 0, kind == 0, n_map_rows);
+            const int fixed = nsb * one.state_bytes + 512;
+            int stages = (budget - fixed) / (one.data_stage + one.w_stage);
+            if (stages > 12) stages = 12;
+            if (stages >= (nsb == 3 ? 3 : 2)) {
+                sh.seg = seg; sh.kc = kc; sh.stages = stages; sh.nsb = nsb;
+                return sh;
+            }
         }
-    }
     return sh;
 }
 
@@ -532,11 +563,18 @@ cudaError_t qld_slide_encode_tmap(void *tmap_out, const void *frames, int64_t ro
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-cudaError_t qld_launch_slide_bulk(int dtype, int is_int, int rows, const void *tmap, const DemodParams &p, const SlideShape &sh,
+cudaError_t qld_launch_slide_bulk(int dtype, int kind, int rows, const void *tmap, const DemodParams &p, const SlideShape &sh,
                                   unsigned int *counter, unsigned int *counter_next, int n_sms, cudaStream_t st)
 {
     const int n_map_rows = count_map_rows(p);
-    if (dtype == QLD_U8)
-        return is_int ? launch_slide_r<uint8_t, int>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st) : launch_slide_r<uint8_t, float>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st);
-    return is_int ? launch_slide_r<uint16_t, int>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st) : launch_slide_r<uint16_t, float>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st);
+    const bool u8 = dtype == QLD_U8;
+    switch (kind) {
+    case 0: return u8 ? launch_slide_r<uint8_t, float>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st)
+                      : launch_slide_r<uint16_t, float>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st);
+    case 1: return u8 ? launch_slide_r<uint8_t, int>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st)
+                      : launch_slide_r<uint16_t, int>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st);
+    case 2: return u8 ? launch_slide_r<uint8_t, long long>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st)
+                      : launch_slide_r<uint16_t, long long>(rows, tmap, p, sh, n_map_rows, counter, counter_next, n_sms, st);
+    default: return cudaErrorInvalidValue;
+    }
 }

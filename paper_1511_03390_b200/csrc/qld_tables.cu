@@ -27,6 +27,13 @@ __global__ void k_table_fill(const TableFillParams p)
             float *w = static_cast<float *>(p.wtab) + e * p.rows + rf.row_off;
             w[0] = (float)sn;
             w[1] = (float)cs;
+        } else if (p.is_int == 2) {
+            // Q1.30 fixed-point references (drift-free sliding at any nu): rint(2^30 sin), rint(2^30 cos)
+            double sn, cs;
+            sincospi(half_turns_of(rf, s), &sn, &cs);
+            int *w = static_cast<int *>(p.wtab) + e * p.rows + rf.row_off;
+            w[0] = (int)rint(sn * 1073741824.0);
+            w[1] = (int)rint(cs * 1073741824.0);
         } else {
             const int64_t r = bin_of(rf, s);
             int *w = static_cast<int *>(p.wtab) + e * p.rows + rf.row_off;

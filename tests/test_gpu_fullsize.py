@@ -174,6 +174,7 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
     tile = np.empty((sc.n_frames, 128, 128), dtype=np.uint16)
     keep = {}                                                     # window -> (I, Q, amp, phase[, bins]) on the host
     is_int = None
+    is_fix, fix = None, {}
     nt = oracle.max_threads()
     w = 0
     for i in range(n_batches):
@@ -188,9 +189,13 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
             ctx.demod(Q.QLD_SLIDE, hop)
             if is_int is None:
                 is_int = ctx.accum_name() == "INT_BINS"
+            if is_fix is None:
+                is_fix = ctx.accum_name() == "FIXED"
             if w in full_windows or w % tile_every == 0:
                 ctx.sync()
                 maps = ctx.get_maps(0)
+                if is_fix:                                            # exact sums on the tile + the table entries of this window
+                    fix[w] = ctx.read_ref_table_fixed(0) + tuple(t[y0:y0 + 128, x0:x0 + 128].cpu().numpy() for t in ctx.get_sums_i64(0))
                 if w in full_windows:
                     keep[w] = [m.cpu().numpy() for m in maps] + ([ctx.get_bins(0).cpu().numpy()] if is_int else [])
                 else:
@@ -200,7 +205,7 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
     ctx.sync()
     assert w == n_win and ctx.counters() == (sc.n_frames, n_win)
     ctx.destroy()
-    rel = 1e-6 if is_int else 1e-5
+    rel = 1e-6 if (is_int or is_fix) else 1e-5
     curve = []
     for ww in sorted(keep):
         a = ww * hop
@@ -213,6 +218,12 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
         strict = check_float_maps(tuple(keep[ww][:4]), ora, rel=rel, what=f"cfg3 stream window {ww}")
         med = float(np.median(ora[2]))
         curve.append((ww, float(np.abs(keep[ww][2] - ora[2]).max() / med), strict))
+        if is_fix:
+            gs, gc, gI, gQ = fix[ww]
+            osn, ocs = oracle.ref_tables(ref, a + 1, N)
+            assert np.abs(gs - np.rint(osn * 2.0 ** 30)).max() <= 1 and np.abs(gc - np.rint(ocs * 2.0 ** 30)).max() <= 1
+            oI, oQ = oracle.demod_int(tile[a:a + N], gs.astype(np.int64), gc.astype(np.int64), nthreads=nt)
+            assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"exact sums of window {ww}"
         if is_int:
             B = oracle.bins(x, ref["num"], ref["den"], s_first=a + 1)
             h = ref["den"] // 2
@@ -244,3 +255,12 @@ def test_cfg3_full_stream_fp32_drift(Q, oracle, resync_hops):
     curve = _stream_cfg3(Q, oracle, {"nu": 0.0937, "phase": 0.3}, Q.QLD_ACC_FP32, 0, resync_hops, (0, 255, 496), tile_every=8,
                          curve_path=os.path.join(root, "gpurun_out", f"cfg3_fp32_drift_resync{resync_hops}.txt"))
     assert max(c[1] for c in curve) <= 1e-5
+
+
+@pytest.mark.parametrize("slide_hop", [0, 32])
+def test_cfg3_full_stream_fixed_point_no_drift(Q, oracle, slide_hop):
+    """Float references (nu = 0.0937) with QLD_ACC_FIXED on the wrapping ring: after 496 add/subtract updates the int64 sums
+    still equal the integer oracle bit for bit (checked on a 128 x 128 tile at every 8th window and at the last one), and the
+    maps meet the float definition to 1e-6: there is no drift to bound and no resynchronisation."""
+    curve = _stream_cfg3(Q, oracle, {"nu": 0.0937, "phase": 0.3}, Q.QLD_ACC_FIXED, slide_hop, 0, (0, 496), tile_every=8)
+    assert max(c[1] for c in curve) <= 1e-6

@@ -206,3 +206,50 @@ def test_slow_epilogue_against_a_fast_main_loop(Q, oracle, tile, H, W, N, K):
         assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"k={k}"
     check_float_maps(_maps(ctx, K - 1), oracle_maps(oracle, x, refs[K - 1]), rel=1e-6, what="slow epilogue")
     ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ FIXED on a ring (drift-free A5)
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("dtype,H,W", [("u16", 12, 128), ("u16", 37, 72), ("u8", 9, 144), ("u16be", 16, 64)])
+@pytest.mark.parametrize("hop,cap,partial", [(32, 170, False), (32, 170, True), (5, 140, False), (40, 173, False), (64, 200, True)])
+@pytest.mark.parametrize("refs", [[{"nu": 0.0937, "phase": 0.3}], [{"nu": 0.4321}, {"num": 1, "den": 6}]])
+def test_fixed_point_sliding_is_exact(Q, oracle, dtype, H, W, hop, cap, partial, refs):
+    """QLD_ACC_FIXED on a ring (SURVEY.md 8(c) precision ladder item 3): Q1.30 references indexed by absolute
+    frame number, int64 sums kept across hops -- every window's sums equal the integer oracle on the same table bit for bit
+    (no drift to bound), the table is the rounded oracle table, and the maps meet the float definition to 1e-6."""
+    N = 128
+    T = N + 7 * hop
+    rng = np.random.default_rng(hop + cap + H)
+    npdt = np.uint8 if dtype == "u8" else np.uint16
+    x = rng.integers(0, 256 if dtype == "u8" else 65536, size=(T, H, W)).astype(npdt)
+    raw = x.byteswap() if dtype == "u16be" else x
+    ctx = Q.QLD(H, W, dtype, N, refs, ring_frames=cap, accum=Q.QLD_ACC_FIXED, slide_hop=hop if partial else 0)
+    assert ctx.accum_name() == "FIXED"
+    ctx.push_frames(raw[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    nt = oracle.max_threads()
+    for w in range(0, (T - N) // hop + 1):
+        if w > 0:
+            ctx.push_frames(raw[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+        ctx.sync()
+        assert ctx.last_kernel() == "k_slide_bulk"
+        a = w * hop
+        for k, ref in enumerate(refs):
+            gs, gc = ctx.read_ref_table_fixed(k)                       # entries of frames a+1 .. a+N
+            osn, ocs = oracle.ref_tables(ref, a + 1, N)
+            assert np.abs(gs - np.rint(osn * 2.0 ** 30)).max() <= 1 and np.abs(gc - np.rint(ocs * 2.0 ** 30)).max() <= 1
+            oI, oQ = oracle.demod_int(x[a:a + N], gs.astype(np.int64), gc.astype(np.int64), nthreads=nt)
+            gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
+            assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"window {w} k={k}"
+            check_float_maps(_maps(ctx, k), oracle_maps(oracle, x[a:a + N], ref, s_first=a + 1), rel=1e-6, what=f"window {w} k={k}")
+    ctx.destroy()
+
+
+def test_fixed_point_ring_limits(Q):
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(8, 64, "u16", 32, [{"nu": 0.1}, {"nu": 0.2}, {"nu": 0.3}], ring_frames=64, accum=Q.QLD_ACC_FIXED)
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
+    with pytest.raises(Q.QLDError) as e:
+        Q.QLD(3, 5, "u16", 32, [{"nu": 0.1}], ring_frames=64, accum=Q.QLD_ACC_FIXED)          # 30 bytes per frame
+    assert e.value.status == Q.QLD_E_UNSUPPORTED
