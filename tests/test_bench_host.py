@@ -16,7 +16,7 @@ def _bench():
 
 def test_traffic_table_and_peaks():
     b = _bench()
-    for wl, kern in (("cfg2", "k_demod_stream"), ("cfg3", "k_demod_stream"), ("cfg4", "k_demod_tc")):
+    for wl, kern in (("cfg2", "k_demod_stream"), ("cfg3", "k_slide_bulk"), ("cfg4", "k_demod_tc")):
         v = b.load_traffic(wl, kern)
         assert isinstance(v, float) and v > 1e6, (wl, kern, v)
     assert b.load_traffic("cfg2", "no_such_kernel") is None
