@@ -135,6 +135,23 @@ __global__ void k_digit_pack(const int32_t *rfix, int n_stride, int n, int rows,
     }
 }
 
+// B operand of the integer-bin contraction: the same [step][n/8][k/16][n%8][k%16] tiles with 16 columns, column c = bin row c,
+// one signed byte (0, +1, -1) per frame
+__global__ void k_bins_pack(const int32_t *wtab, int cap_w, int rows, int n, int n_steps, int8_t *digits)
+{
+    constexpr int nc = 16;
+    const int64_t total = (int64_t)n_steps * nc * MMA_K;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int q = (int)(idx / (nc * MMA_K));
+        const int rem = (int)(idx % (nc * MMA_K));
+        const int k0 = rem & 15, n0 = (rem >> 4) & 7, k1 = (rem >> 7) & 1, n1 = rem >> 8;
+        const int c = n1 * 8 + n0, s = q * MMA_K + k1 * 16 + k0;          // frame s + 1
+        int d = 0;
+        if (s < n && c < rows) d = wtab[(int64_t)((s + 1) % cap_w) * rows + c];
+        digits[idx] = (int8_t)d;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // the contraction kernel
 // ---------------------------------------------------------------------------------------------------
@@ -185,7 +202,7 @@ struct TcSmem {
 
 // TT, KCC > 0: the tile shape as compile-time constants (the shape the launcher picks for large frames): the MMA warp's
 // loops over spans and K steps unroll and every descriptor is "stage base + immediate"; 0: run-time shape (T_rt, KC_rt).
-template <int NC, int BYTES, int TT, int KCC>
+template <int NC, int BYTES, int TT, int KCC, bool BINS>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap2, const __grid_constant__ CUtensorMap tmap4,
                                                      const TcParams p, const int T_rt, const int STAGES, const int KC_rt, const int use4d)
 {
@@ -388,6 +405,54 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                 tc_wait_ld();
                 tc_fence_before();
                 mbar_arrive(&tempty[abuf * T + t]);
+                if constexpr (BINS) {
+                    // integer phase bins (A3'): column c = bin row c, exact int32; the lane pair of a 16-bit pixel holds its
+                    // low-byte and high-byte sums: bin = lo + 256 * hi
+                    int bins[16];
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        int v = (int)r[0][c];
+                        if (BYTES == 2) {
+                            const int o = __shfl_xor_sync(0xffffffffu, v, 1);
+                            v = (((lane & 1) != 0) != (p.big_endian != 0)) ? (o + (v << 8)) : (v + (o << 8));
+                        }
+                        bins[c] = v;
+                    }
+                    if (valid) {
+                        const FinParams &f = p.fin;
+                        const bool odd = BYTES == 2 && (lane & 1);         // the lane pair shares the stores
+#pragma unroll
+                        for (int c = 0; c < 16; ++c)
+                            if (c < p.bins_rows && (BYTES == 1 || ((c & 1) != 0) == odd)) p.bins_out[(int64_t)c * p.bins_stride + pixel] = bins[c];
+                        for (int k = 0; k < f.K; ++k) {
+                            const int off = f.row_off[k], end = off + f.n_rows[k];
+                            double S = 0.0, C = 0.0;
+#pragma unroll
+                            for (int c = 0; c < 16; ++c)
+                                if (c >= off && c < end) {
+                                    S = fma((double)bins[c], f.sw[c], S);
+                                    C = fma((double)bins[c], f.cw[c], C);
+                                }
+                            if (f.rot) {
+                                const double rc = f.rot[2 * k], rs = f.rot[2 * k + 1], S2 = S * rc - C * rs;
+                                C = C * rc + S * rs;
+                                S = S2;
+                            }
+                            S *= f.scale;
+                            C *= f.scale;
+                            const int64_t o = (int64_t)k * p.HW + pixel;
+                            if (BYTES == 1 || !odd) {
+                                if (f.I) f.I[o] = (float)S;
+                                if (f.amp) f.amp[o] = (float)sqrt(S * S + C * C);
+                            }
+                            if (BYTES == 1 || odd) {
+                                if (f.Q) f.Q[o] = (float)C;
+                                if (f.phase) f.phase[o] = (S == 0.0 && C == 0.0) ? 0.0f : (float)atan2(C, S);
+                            }
+                        }
+                    }
+                    continue;
+                }
                 const double sc30 = p.fin.scale * 9.31322574615478515625e-10;                   // scale * 2^-30
 #pragma unroll
                 for (int g = 0; g < NC / 16; ++g) {       // 16 columns = 4 reference rows = 2 references per group
@@ -456,11 +521,11 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms, const int *force)
     return sh;
 }
 
-template <int NC, int BYTES, int TT, int KCC>
+template <int NC, int BYTES, int TT, int KCC, bool BINS>
 cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const TcShape &sh, int n_sms, cudaStream_t st)
 {
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
-    auto kern = k_demod_tc<NC, BYTES, TT, KCC>;
+    auto kern = k_demod_tc<NC, BYTES, TT, KCC, BINS>;
     // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
     // function, and re-setting it on every launch costs a driver call)
     static int smem_set_dev[64] = {0};
@@ -480,14 +545,14 @@ cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const T
     return cudaGetLastError();
 }
 
-template <int NC, int BYTES>
+template <int NC, int BYTES, bool BINS = false>
 cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
     const int force[3] = {p.force_T, p.force_stages, p.force_kc};
     const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
     // the shape of large frames (T = 8 spans = 1 KB of every frame, 64-frame stages) has its own instantiation
-    if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64>(tmaps, p, sh, n_sms, st);
-    return launch_tc_shape<NC, BYTES, 0, 0>(tmaps, p, sh, n_sms, st);
+    if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64, BINS>(tmaps, p, sh, n_sms, st);
+    return launch_tc_shape<NC, BYTES, 0, 0, BINS>(tmaps, p, sh, n_sms, st);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -567,9 +632,18 @@ cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int 
     return cudaGetLastError();
 }
 
+cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N, int8_t *digits, cudaStream_t st)
+{
+    const int n_steps = (N + KC_PAD - 1) / KC_PAD * (KC_PAD / MMA_K);
+    const int64_t total = (int64_t)n_steps * 16 * MMA_K;
+    k_bins_pack<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(wtab, cap_w, rows, N, n_steps, digits);
+    return cudaGetLastError();
+}
+
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
     const CUtensorMap *tm = reinterpret_cast<const CUtensorMap *>(tmaps);
+    if (p.bins_rows > 0) return p.bytes == 2 ? launch_tc<16, 2, true>(tm, p, n_sms, st) : launch_tc<16, 1, true>(tm, p, n_sms, st);
     const int nc = qld_tc_columns(p.fin.K);
     if (p.bytes == 2) {
         switch (nc) {

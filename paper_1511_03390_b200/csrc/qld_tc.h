@@ -16,15 +16,23 @@ struct TcParams {
     unsigned int *tile_counter_next; // the next launch's counter, zeroed by this launch (the two alternate)
     int32_t force_T, force_stages, force_kc;   // debug override of the tile shape (qld_debug_set_tile), 0 = automatic
     int32_t big_endian;       // 16-bit samples most significant byte first: the even accumulator row is the high byte
+    int32_t bins_rows;        // > 0: integer phase bins (A3'): the B operand holds one signed byte per bin row and frame (16
+                              // columns), the epilogue writes the exact int32 rows to bins_out and combines them with fin.sw / fin.cw
+    int32_t reserved2;
+    int32_t *bins_out;        // [bins_rows padded][HW] int32 (the context's accumulator rows)
+    int64_t bins_stride;      // elements between rows of bins_out (HW)
     FinParams fin;
 };
 
 int qld_tc_columns(int K);                       // N columns of the MMA: 8 per reference, padded to 16
 size_t qld_tc_digit_bytes(int K, int N);
+// K: references of a fixed-point contraction (8 columns each, padded to 16); K = 2 also describes the 16-column bins contraction
 cudaError_t qld_tc_encode_tmap(void *tmaps_out /*2 x 128 B, 64-aligned*/, const void *frames, int64_t row_bytes, int n_frames, int K, int n_sms,
                                const int *force /* {T, stages, kc} or zeros */);
 cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix, int n_stride, cudaStream_t st);
 // rfix rows (2k, 2k+1) = rint(2^30 * tab[2][n]) from caller-supplied doubles
 cudaError_t qld_launch_fixed_from_doubles(const double *tab, int n, int k, int32_t *rfix, int n_stride, cudaStream_t st);
+// B operand of the integer-bin contraction from the context's weight table wtab[cap_w][rows] (frames 1..N, entries s mod cap_w)
+cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N, int8_t *digits, cudaStream_t st);
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);

@@ -40,7 +40,7 @@ def _gpu_on_pixels(ctx, k, pix):
     return tuple(None if m is None else m.reshape(-1)[idx].cpu().numpy() for m in ctx.get_maps(k))
 
 
-@pytest.mark.parametrize("name,accum_name,kernel", [("cfg1", "AUTO", "k_demod_stream"), ("cfg1", "FP32", "k_demod_stream"),
+@pytest.mark.parametrize("name,accum_name,kernel", [("cfg1", "AUTO", "k_demod_tc"), ("cfg1", "FP32", "k_demod_stream"),
                                                    ("cfg2", "AUTO", "k_demod_stream"), ("cfg2", "FIXED", "k_demod_tc"),
                                                    ("cfg4", "AUTO", "k_demod_tc"), ("cfg4", "FP32", "k_demod_stream"), ("cfg4", "FIXED", "k_demod_tc")])
 def test_whole_window_full_size_sampled(Q, oracle, name, accum_name, kernel):

@@ -151,9 +151,9 @@ def test_fixed_rejects_what_it_cannot_do(Q):
     with pytest.raises(Q.QLDError) as e:
         Q.QLD(3, 17, "u8", 16, [{"nu": 0.1}], accum=Q.QLD_ACC_FIXED)            # 51 bytes per frame: not a TMA pitch
     assert e.value.status == Q.QLD_E_UNSUPPORTED
-    with pytest.raises(Q.QLDError) as e:
-        Q.QLD(4, 16, "u8", 16, [{"nu": 0.1}], ring_frames=40, accum=Q.QLD_ACC_FIXED)
-    assert e.value.status == Q.QLD_E_UNSUPPORTED
+    ctx = Q.QLD(4, 16, "u8", 16, [{"nu": 0.1}], ring_frames=40, accum=Q.QLD_ACC_FIXED)    # rings: int64 sums through k_slide_bulk
+    assert ctx.accum_name() == "FIXED"
+    ctx.destroy()
 
 
 def test_auto_moves_k_ge_4_to_the_tensor_cores(Q, oracle):
@@ -253,3 +253,32 @@ def test_fixed_point_ring_limits(Q):
     with pytest.raises(Q.QLDError) as e:
         Q.QLD(3, 5, "u16", 32, [{"nu": 0.1}], ring_frames=64, accum=Q.QLD_ACC_FIXED)          # 30 bytes per frame
     assert e.value.status == Q.QLD_E_UNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------------------ integer bins on the tensor cores
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("tile", ["8,3,64", "4,5,64", "2,8,32", "1,8,64"])
+@pytest.mark.parametrize("dtype,H,W,N", [("u8", 50, 128, 70), ("u16", 37, 48, 129), ("u16", 16, 200, 64), ("u16be", 24, 128, 33), ("u8", 33, 256, 9)])
+@pytest.mark.parametrize("refs", [[{"num": 1, "den": 8}], [{"num": 1, "den": 6}], [{"num": 1, "den": 4}, {"num": 3, "den": 16, "phase": 0.4}], [{"num": 2, "den": 5}]])
+def test_integer_bins_on_the_tensor_cores(Q, oracle, tile, dtype, H, W, N, refs):
+    """A3' as a one-digit int8 contraction (the bin indicators 0, +1, -1 are the B operand): int32 bins bit-exact against the
+    int64 oracle for every tile shape, sample format and bin layout (even den: difference rows; odd den: plain bins; two
+    references), maps to 1e-6."""
+    rng = np.random.default_rng(H * N)
+    npdt = np.uint8 if dtype == "u8" else np.uint16
+    x = rng.integers(0, 256 if dtype == "u8" else 65536, size=(N, H, W)).astype(npdt)
+    raw = x.byteswap() if dtype == "u16be" else x
+    mk = forced(Q, "tc", tile)
+    ctx = mk(H, W, dtype, N, refs, accum=Q.QLD_ACC_INT_BINS)
+    ctx.push_frames(raw)
+    ctx.demod()
+    ctx.demod()
+    ctx.sync()
+    assert ctx.last_kernel() == "k_demod_tc"
+    for k, ref in enumerate(refs):
+        den, num = ref["den"], ref["num"]
+        B = oracle.bins(x, num, den)
+        exp = B[:den // 2] - B[den // 2:] if den % 2 == 0 else B
+        assert np.array_equal(ctx.get_bins(k).cpu().numpy(), exp), f"k={k}"
+        check_float_maps(_maps(ctx, k), oracle_maps(oracle, x, ref), rel=1e-6, what=f"tc bins k={k}")
+    ctx.destroy()
