@@ -535,7 +535,62 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     return res
 
 
-RUNNERS = {"cfg0": bench_whole, "cfg1": bench_whole, "cfg2": bench_whole, "cfg3": bench_slide, "cfg4": bench_whole}
+def bench_spectrum(env: Env, args, workload: str, accum_name: str, steps: int, warmup: int, e2e_steps: int, with_cpu: bool):
+    """unknown-frequency search (qld_dominant_bin) over every DFT bin 1..N/2-1 of the cfg2-shaped stack
+    (1280x1024, N = 1024, uint16): 32 bins per pass on the tensor cores, arg-max fused into the epilogue."""
+    torch = env.torch
+    from paper_1511_03390_b200 import qld
+    wl = build_workload("cfg2", env.rank)
+    sc = wl.scene
+    N, H, W = wl.N, sc.H, sc.W
+    frames = qld.synth_fill(sc, 1, N, device=env.dev)
+    q_lo, q_hi = 1, N // 2 - 1
+    n_pass = -(-(q_hi - q_lo + 1) // 32)
+    out = {}
+
+    def step():
+        out["amp"], out["bin"] = qld.dominant_bin(frames, q_lo, q_hi)
+
+    steps = max(3, min(steps, 10))
+    ms, clocks, _ = env.timed(step, steps, 5, keep_busy=None, counter=None)
+    samples = float(N) * H * W
+    stack = samples * 2
+    res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps, "maps_per_s": env.world * steps / (ms * 1e-3),
+           "clocks": clocks, "kernel": "k_demod_tc", "gpu_launches": (n_pass + 1) * steps, "dtype": "int8 x int8 -> int32 -> int64 (tcgen05)"}
+    res["roofline"] = roofline_hbm(n_pass * stack + 8.0 * H * W, ms / steps, workload, "k_demod_tc",
+                                   f"{n_pass} passes over the {stack / 1e9:.2f} GB stack (32 of the {q_hi - q_lo + 1} bins per pass, 256 MMA columns); a single pass "
+                                   f"would move {stack / 1e9:.2f} GB and be bound by the int8 tensor rate instead (about 5 ms for this shape)")
+    res["roofline"]["traffic"] = None
+    res["config"] = {"workload": "f2: qld_dominant_bin on the cfg2 stack", "H": H, "W": W, "N": N, "bins": [q_lo, q_hi], "passes": n_pass,
+                     "step": "qld_dominant_bin(bins 1..N/2-1): digit tiles + one tcgen05 launch per 32 bins, blocking call",
+                     "cache": f"input {stack / 1e6:.0f} MB per pass > 126 MB L2: no flush needed",
+                     "parallelism": f"{env.world} x independent stacks"}
+    if with_cpu and env.rank == 0:
+        import numpy as np
+        import oracle
+        nt = oracle.max_threads()
+        rng = np.random.default_rng(0)
+        pix = np.unique(rng.integers(0, H * W, size=384))
+        sub = frames.view(torch.int16).reshape(N, -1)[:, torch.from_numpy(pix).to(env.dev)].cpu().numpy().view(np.uint16).reshape(N, 1, -1)
+        t0 = time.perf_counter()
+        best, idx, second = oracle.dominant_bin(sub, q_lo, q_hi, nthreads=nt)
+        secs = time.perf_counter() - t0
+        amp = out["amp"].reshape(-1)[torch.from_numpy(pix).to(env.dev)].cpu().numpy().astype(np.float64)
+        bins = out["bin"].reshape(-1)[torch.from_numpy(pix).to(env.dev)].cpu().numpy()
+        best, idx, second = best.reshape(-1), idx.reshape(-1), second.reshape(-1)
+        assert np.all(np.abs(amp - best) <= 1e-6 * best + 2.0 ** -23 * best), "f2 parity: amplitude"
+        unique = second < best * (1.0 - 1e-6)
+        assert np.array_equal(bins[unique], idx[unique]), "f2 parity: bin"
+        res["cpu_baseline"] = {"value": float(sub.size) / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
+                               "sample": f"{len(pix)} random pixels x {N} frames x {q_hi - q_lo + 1} bins (one QLD per bin), {secs:.2f} s"}
+        res["parity"] = {"pixels_checked": int(len(pix)), "tolerance": "amplitude 1e-6; bin equal wherever the runner-up is not within 1e-6",
+                         "unique_fraction": float(unique.mean()), "ok": True}
+    del frames
+    torch.cuda.empty_cache()
+    return res
+
+
+RUNNERS = {"f2": bench_spectrum, "cfg0": bench_whole, "cfg1": bench_whole, "cfg2": bench_whole, "cfg3": bench_slide, "cfg4": bench_whole}
 
 
 def spawn_ranks(n: int):
@@ -583,7 +638,7 @@ def main():
                     "(SURVEY.md 8(a) A5 as literally stated) instead of keeping per-batch partial sums (8(f3), cfg.slide_hop: "
                     "identical results, fewer bytes, and the faster of the two on B200: the default)")
     ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly first, one compact JSON line each "
-                    "(default: cfg2,cfg3,cfg1 when --workload is cfg4 on one GPU; 'none' to skip)")
+                    "(default: cfg2,cfg3,cfg1,f2 when --workload is cfg4 on one GPU; 'none' to skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -596,7 +651,7 @@ def main():
     env = Env(args)
     names = args.also
     if names == "default":
-        names = "cfg2,cfg3,cfg1" if (args.workload == "cfg4" and env.world == 1 and args.accum == "auto") else "none"
+        names = "cfg2,cfg3,cfg1,f2" if (args.workload == "cfg4" and env.world == 1 and args.accum == "auto") else "none"
     also = {}
     if names != "none":
         for w in [x for x in names.split(",") if x and x != args.workload]:

@@ -279,8 +279,9 @@ int qld_cnr(const float *map_device, int32_t H, int32_t W, int32_t y0, int32_t x
  * SURVEY.md 8(f2)): demodulate the N-frame stack `frames_device` (frame-major, device memory, qld_dtype) at every DFT
  * bin q = q_lo..q_hi (nu = q/N, 1 <= q_lo <= q_hi, 2*q_hi < N) and keep, per pixel, the largest amplitude R_q = |F_q|
  * and its bin (the lowest bin on a tie): amp_max_device [H][W] float32, bin_device [H][W] int32 (device memory).
- * Eight bins per pass over the stack, exact fixed-point sums on the tensor cores where QLD_ACC_FIXED applies, FP32
- * otherwise.  Work is enqueued on `stream` (cudaStream_t; NULL = the legacy default stream); the call returns after
+ * Frames whose byte size is a multiple of 16: 32 bins per pass over the stack, one tcgen05 launch per pass (Q1.30 references,
+ * exact sums, arg-max fused into the epilogue), N/64 passes in all.  Other frame sizes: eight bins per pass through a context
+ * (FP32).  Work is enqueued on `stream` (cudaStream_t; NULL = the legacy default stream); the call returns after
  * the last pass has finished. */
 int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_t H, int32_t W, int32_t N, int32_t q_lo, int32_t q_hi,
                      float *amp_max_device, int32_t *bin_device, void *stream);

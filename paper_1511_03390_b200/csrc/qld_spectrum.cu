@@ -1,14 +1,19 @@
 // Unknown-frequency search: the paper's Fourier decomposition "is essentially a series of QLDs being
 // performed at different frequencies", and the FFT image is |F(j,k,omega_q)|^2 at the bin of interest
 // (PAPER.md:99).  When the modulation frequency is not known, every bin q_lo..q_hi of the N-frame window (nu = q/N) is
-// demodulated -- eight bins per pass over the stack, on the tensor-core path where it applies -- and each pixel keeps
-// the bin with the largest amplitude R_q = |F_q|.  Built on the public C ABI only (qld_create .. qld_destroy) plus one
-// small kernel that folds a pass's amplitude maps into the running maximum.
+// demodulated and each pixel keeps the bin with the largest amplitude R_q = |F_q|.
+//
+// Fast path (frames whose byte size is a multiple of 16): 32 bins per pass over the stack as ONE launch of the tcgen05
+// contraction with 256 columns (32 bins x sin, cos x 4 digits of the Q1.30 references), the arg-max fused into its epilogue;
+// the digit tiles of all bins are built once, there is no context and no map per pass: N/64 passes, each HBM-bound.
+// Fallback (other frame sizes): eight bins per pass through the public C ABI (qld_create .. qld_destroy) plus one small
+// kernel that folds a pass's amplitude maps into the running maximum.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>
 
 #include "qld.h"
+#include "qld_tc.h"
 
 namespace {
 
@@ -35,6 +40,41 @@ extern "C" int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_
     if (q_lo < 1 || q_hi < q_lo || 2 * (int64_t)q_hi >= N) return QLD_E_INVAL;       // 0 < q/N < 1/2 (reading G18)
     cudaStream_t st = stream ? static_cast<cudaStream_t>(stream) : cudaStreamLegacy;
     const int64_t HW = (int64_t)H * W;
+    const int bytes = dtype == QLD_U8 ? 1 : 2;
+    if (dtype != QLD_U8 && dtype != QLD_U16 && dtype != QLD_U16_BE) return QLD_E_INVAL;
+    if ((HW * bytes) % 16 == 0 && (reinterpret_cast<uintptr_t>(frames_device) & 15) == 0 && N <= 65536) {
+        // ---- 32 bins per pass on the tensor cores, arg-max in the epilogue
+        const int n_bins = q_hi - q_lo + 1;
+        size_t pass_bytes = 0;
+        const size_t dig_bytes = qld_tc_spectrum_digit_bytes(N, n_bins, &pass_bytes);
+        unsigned char *scratch = nullptr;                    // digit tiles + two tile counters
+        // stream-ordered allocation: no device-wide synchronisation on either side of the search
+        if (cudaMallocAsync(reinterpret_cast<void **>(&scratch), dig_bytes + 256, st) != cudaSuccess) { (void)cudaGetLastError(); return QLD_E_NOMEM; }
+        int8_t *digits = reinterpret_cast<int8_t *>(scratch);
+        unsigned int *counters = reinterpret_cast<unsigned int *>(scratch + dig_bytes);
+        int rc = QLD_OK;
+        alignas(64) unsigned char tmaps[256];
+        const int force[3] = {1, 4, 128};
+        int n_sms = qld_sm_count();
+        if (cudaMemsetAsync(counters, 0, 8, st) != cudaSuccess) rc = QLD_E_CUDA;
+        if (rc == QLD_OK && qld_launch_spectrum_digits(N, q_lo, n_bins, digits, st) != cudaSuccess) rc = QLD_E_CUDA;
+        if (rc == QLD_OK && qld_tc_encode_tmap(tmaps, frames_device, HW * bytes, N, 32 /* 256 columns */, n_sms, force) != cudaSuccess) rc = QLD_E_CUDA;
+        for (int P = 0; rc == QLD_OK && P * 32 < n_bins; ++P) {
+            TcParams p;
+            memset(&p, 0, sizeof p);
+            p.HW = HW; p.row_bytes = HW * bytes; p.N = N; p.bytes = bytes; p.big_endian = dtype == QLD_U16_BE;
+            p.digits = digits + (size_t)P * pass_bytes;
+            p.tile_counter = counters + (P & 1); p.tile_counter_next = counters + ((P + 1) & 1);
+            p.fin.K = 1; p.fin.scale = 1.0;
+            p.spec_amp = amp_max_device; p.spec_bin = bin_device;
+            p.spec_q0 = q_lo + 32 * P; p.spec_nbins = n_bins - 32 * P < 32 ? n_bins - 32 * P : 32; p.spec_first = P == 0;
+            if (qld_launch_demod_tc_spectrum(tmaps, p, n_sms, st) != cudaSuccess) rc = QLD_E_CUDA;
+        }
+        cudaFreeAsync(scratch, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) rc = QLD_E_CUDA;
+        (void)cudaGetLastError();
+        return rc;
+    }
     int first = 1;
     for (int q0 = q_lo; q0 <= q_hi; q0 += 8) {
         const int K = q_hi - q0 + 1 < 8 ? q_hi - q0 + 1 : 8;

@@ -152,6 +152,38 @@ __global__ void k_bins_pack(const int32_t *wtab, int cap_w, int rows, int n, int
     }
 }
 
+// Digit tiles of the unknown-frequency search: pass P holds the DFT bins q_lo + 32 P .. (nu = q / N, reduced exactly as
+// (q s) mod N), 256 columns: column c = 4 * (2 * b + row) + j = digit j of sin (row 0) / cos (row 1) of bin b of the pass.
+// Steps (32 frames) are padded to a multiple of 4: the search runs 128-frame stages.
+__global__ void k_spectrum_digits(int N, int q_lo, int n_bins, int n_steps, int8_t *digits)
+{
+    constexpr int nc = 256;
+    const int n_pass = (n_bins + 31) / 32;
+    const int64_t total = (int64_t)n_pass * n_steps * nc * MMA_K;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int P = (int)(idx / ((int64_t)n_steps * nc * MMA_K));
+        const int64_t in_pass = idx % ((int64_t)n_steps * nc * MMA_K);
+        const int q = (int)(in_pass / (nc * MMA_K));
+        const int rem = (int)(in_pass % (nc * MMA_K));
+        const int k0 = rem & 15, n0 = (rem >> 4) & 7, k1 = (rem >> 7) & 1, n1 = rem >> 8;
+        const int c = n1 * 8 + n0, s = q * MMA_K + k1 * 16 + k0;          // frame s + 1
+        const int b = c >> 3, row = (c >> 2) & 1, j = c & 3;
+        const int bin = P * 32 + b;
+        int d = 0;
+        if (s < N && bin < n_bins) {
+            const uint64_t r = ((uint64_t)(q_lo + bin) * (uint64_t)(s + 1)) % (uint64_t)N;
+            double sn, cs;
+            sincospi(2.0 * (double)r / (double)N, &sn, &cs);
+            int32_t v = (int32_t)rint((row ? cs : sn) * 1073741824.0);
+            for (int t = 0; t <= j; ++t) {
+                d = ((v + 128) & 255) - 128;
+                v = (v - d) >> 8;
+            }
+        }
+        digits[idx] = (int8_t)d;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------
 // the contraction kernel
 // ---------------------------------------------------------------------------------------------------
@@ -196,13 +228,14 @@ struct TcSmem {
         b_stage = (kc / MMA_K) * nc * MMA_K;
         off_b = stages * a_stage;
         off_bar = off_b + stages * b_stage;
-        total = off_bar + (2 * stages + 2 + TC_MAX_SPANS) * 8 + 16 + 8 + TC_TQ * 4 + 8;   // barriers, TMEM slot, tile queue, tbuf_tile
+        total = off_bar + (2 * stages + 2 + TC_MAX_SPANS) * 8 + 16 + 8 + TC_TQ * 4 + 8 + 2 * 192 * 8;   // barriers, TMEM slot, tile queue, tbuf_tile, search exchange
     }
 };
 
 // TT, KCC > 0: the tile shape as compile-time constants (the shape the launcher picks for large frames): the MMA warp's
 // loops over spans and K steps unroll and every descriptor is "stage base + immediate"; 0: run-time shape (T_rt, KC_rt).
-template <int NC, int BYTES, int TT, int KCC, bool BINS>
+// MODE: 0 = fixed-point references (A3 / A6), 1 = integer phase bins (A3'), 2 = unknown-frequency search (32 DFT bins per launch)
+template <int NC, int BYTES, int TT, int KCC, int MODE>
 __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constant__ CUtensorMap tmap2, const __grid_constant__ CUtensorMap tmap4,
                                                      const TcParams p, const int T_rt, const int STAGES, const int KC_rt, const int use4d)
 {
@@ -220,6 +253,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + TC_MAX_SPANS);
     volatile int *tile_q = reinterpret_cast<volatile int *>(tmem_slot + 2);      // [TC_TQ] tile ids, producer -> MMA warp
     volatile int *tbuf_tile = tile_q + TC_TQ;                                        // [2] tile id per accumulator buffer
+    double *spec_x = reinterpret_cast<double *>(const_cast<int *>(tbuf_tile) + 2);     // [2][192] search mode: quartet 1 -> quartet 0
 
     // the warp index as a broadcast: the compiler then knows that the role branches below are warp-uniform and keeps the MMA
     // warp's loop state in uniform registers
@@ -237,7 +271,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
             mbar_init(&empty[i], 1);
         }
         for (int i = 0; i < 2; ++i) mbar_init(&tfull[i], 2);
-        for (int i = 0; i < TC_MAX_SPANS; ++i) mbar_init(&tempty[i], 128);
+        for (int i = 0; i < TC_MAX_SPANS; ++i) mbar_init(&tempty[i], MODE == 2 ? 128 * EPI_SETS : 128);   // search mode: both quartets drain every span
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 1) {
@@ -316,7 +350,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
             const int tile = __shfl_sync(0xffffffffu, tile_q[it & (TC_TQ - 1)], 0);
             // The first span of every epilogue quartet (spans 0 .. EPI_SETS-1 of this accumulator set) is drained: each
             // quartet is then past the hand-off that used tfull[buf] / tbuf_tile[buf] two tiles ago, so both may be reused.
-            for (int e = 0; e < EPI_SETS && e < T; ++e) mbar_wait(&tempty[abuf * T + e], epar ^ 1u);
+            for (int e = 0; e < (MODE == 2 ? 1 : EPI_SETS) && e < T; ++e) mbar_wait(&tempty[abuf * T + e], epar ^ 1u);
             if (leader) tbuf_tile[buf] = tile;
             if (tile < 0) {
                 if (leader) { mbar_arrive(&tfull[buf]); mbar_arrive(&tfull[buf]); }
@@ -380,7 +414,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
         const int q = warp & 3;                         // TMEM lane quarter this warp may read
         const int eset = (warp - 2) >> 2;               // which quartet of epilogue warps: it drains spans t % EPI_SETS == eset
         const int m = q * 32 + lane;                    // accumulator row = byte index inside the 128-byte span
-        for (int it = 0; eset < T; ++it) {              // a quartet without spans (T < EPI_SETS) has nothing to do
+        for (int it = 0; MODE == 2 || eset < T; ++it) { // a quartet without spans (T < EPI_SETS) has nothing to do
             const int buf = it & 1;
             const int abuf = NBUF == 2 ? buf : 0;
             mbar_wait(&tfull[buf], (it >> 1) & 1);
@@ -388,7 +422,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
             if (tile < 0) break;
             const int nv = min(T, n_sub - tile * T);
             tc_fence_after();
-            for (int t = eset; t < T; t += EPI_SETS) {
+            for (int t = (MODE == 2 ? 0 : eset); t < T; t += (MODE == 2 ? 1 : EPI_SETS)) {
                 if (t >= nv) {                                // span beyond the frame: nothing was accumulated, hand it back
                     mbar_arrive(&tempty[abuf * T + t]);
                     continue;
@@ -397,6 +431,67 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                 const int64_t byte0 = (int64_t)(tile * T + t) * SUB_BYTES + m;
                 const int64_t pixel = BYTES == 2 ? (byte0 >> 1) : byte0;
                 const bool valid = byte0 < p.row_bytes;
+                if constexpr (MODE == 2) {
+                    // unknown-frequency search: 32 bins = 16 groups of 16 columns; quartet e takes the groups g = e mod 2.  The
+                    // squared amplitude of every bin is compared in fp64 against the thread's running best (strictly greater:
+                    // the lowest bin wins a tie); the two quartets meet through shared memory, then one read-modify-write of
+                    // the maps that persist across the passes.
+                    double best = -1.0;
+                    int best_q = 0;
+                    // the running maximum of earlier passes is requested now and used at the very end
+                    const bool writer = eset == 0 && valid && (BYTES == 1 || !(lane & 1));
+                    float prev_amp = -1.0f;
+                    if (writer && !p.spec_first) prev_amp = __ldg(p.spec_amp + pixel);
+                    uint32_t rn[16];
+                    tc_ld16(taddr + eset * 16, rn);                             // software pipeline: the next group's columns are in flight
+                    for (int g = eset; g < NC / 16; g += EPI_SETS) {
+                        uint32_t r[16];
+                        tc_wait_ld();
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) r[i] = rn[i];
+                        if (g + EPI_SETS < NC / 16) tc_ld16(taddr + (g + EPI_SETS) * 16, rn);
+                        long long v[4];
+#pragma unroll
+                        for (int rr = 0; rr < 4; ++rr)
+                            v[rr] = (long long)(int)r[4 * rr] + ((long long)(int)r[4 * rr + 1] << 8) + ((long long)(int)r[4 * rr + 2] << 16) +
+                                    ((long long)(int)r[4 * rr + 3] << 24);
+                        if (BYTES == 2) {
+#pragma unroll
+                            for (int rr = 0; rr < 4; ++rr) {
+                                const long long o = __shfl_xor_sync(0xffffffffu, v[rr], 1);
+                                v[rr] = (((lane & 1) != 0) != (p.big_endian != 0)) ? (o + (v[rr] << 8)) : (v[rr] + (o << 8));
+                            }
+                        }
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+                            if (BYTES == 2 && (lane & 1) != kk) continue;      // the lane pair of a 16-bit pixel splits the two bins
+                            const int b = 2 * g + kk;
+                            const double S = (double)v[2 * kk], C = (double)v[2 * kk + 1];
+                            const double a2 = fma(S, S, C * C);
+                            if (b < p.spec_nbins && a2 > best) { best = a2; best_q = p.spec_q0 + b; }
+                        }
+                    }
+                    tc_fence_before();
+                    mbar_arrive(&tempty[abuf * T + t]);
+                    if (BYTES == 2) {                                           // even bins sit in the even lane, odd bins in the odd lane
+                        const double ob = __shfl_xor_sync(0xffffffffu, best, 1);
+                        const int oq = __shfl_xor_sync(0xffffffffu, best_q, 1);
+                        if (ob > best || (ob == best && oq < best_q)) { best = ob; best_q = oq; }
+                    }
+                    double *sx = spec_x + (size_t)(it & 1) * 192;              // 128 doubles + 128 ints per buffer
+                    if (eset == 1) { sx[m] = best; reinterpret_cast<int *>(sx + 128)[m] = best_q; }
+                    named_barrier(2, 128 * EPI_SETS);
+                    if (eset == 0) {
+                        const double ob = sx[m];
+                        const int oq = reinterpret_cast<const int *>(sx + 128)[m];
+                        if (ob > best || (ob == best && oq < best_q)) { best = ob; best_q = oq; }
+                        if (writer && best >= 0.0) {
+                            const float amp = (float)(sqrt_newton(best) * (p.fin.scale * 9.31322574615478515625e-10));
+                            if (p.spec_first || amp > prev_amp) { p.spec_amp[pixel] = amp; p.spec_bin[pixel] = best_q; }
+                        }
+                    }
+                    continue;
+                }
                 // all NC columns of the span into registers with one wait, then the span goes straight back to the MMA warp:
                 // the arithmetic below runs out of registers while the next tile's MMAs already overwrite the columns
                 uint32_t r[NC / 16][16];
@@ -405,7 +500,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                 tc_wait_ld();
                 tc_fence_before();
                 mbar_arrive(&tempty[abuf * T + t]);
-                if constexpr (BINS) {
+                if constexpr (MODE == 1) {
                     // integer phase bins (A3'): column c = bin row c, exact int32; the lane pair of a 16-bit pixel holds its
                     // low-byte and high-byte sums: bin = lo + 256 * hi
                     int bins[16];
@@ -514,18 +609,18 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms, const int *force)
     sh.stages = (225 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
     if (force && force[0] > 0) {                          // debug / test override (qld_debug_set_tile): T, STAGES, KC
         const int t = force[0], s2 = force[1], kc = force[2];
-        if (t * nc <= 512 && t <= TC_MAX_SPANS / 2 && s2 >= 2 && (kc == 32 || kc == 64) && TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
+        if (t * nc <= 512 && t <= TC_MAX_SPANS / 2 && s2 >= 2 && (kc == 32 || kc == 64 || kc == 128) && TcSmem(nc, t, s2, kc).total + 1024 <= 227 * 1024) { sh.T = t; sh.stages = s2; sh.kc = kc; }
     }
     if (sh.stages > TC_MAX_STAGES) sh.stages = TC_MAX_STAGES;
     sh.use4d = (row_bytes % SUB_BYTES == 0 && N >= GRP) ? 1 : 0;
     return sh;
 }
 
-template <int NC, int BYTES, int TT, int KCC, bool BINS>
+template <int NC, int BYTES, int TT, int KCC, int MODE>
 cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const TcShape &sh, int n_sms, cudaStream_t st)
 {
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
-    auto kern = k_demod_tc<NC, BYTES, TT, KCC, BINS>;
+    auto kern = k_demod_tc<NC, BYTES, TT, KCC, MODE>;
     // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
     // function, and re-setting it on every launch costs a driver call)
     static int smem_set_dev[64] = {0};
@@ -545,14 +640,14 @@ cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const T
     return cudaGetLastError();
 }
 
-template <int NC, int BYTES, bool BINS = false>
+template <int NC, int BYTES, int MODE = 0>
 cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
     const int force[3] = {p.force_T, p.force_stages, p.force_kc};
     const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
     // the shape of large frames (T = 8 spans = 1 KB of every frame, 64-frame stages) has its own instantiation
-    if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64, BINS>(tmaps, p, sh, n_sms, st);
-    return launch_tc_shape<NC, BYTES, 0, 0, BINS>(tmaps, p, sh, n_sms, st);
+    if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64, MODE>(tmaps, p, sh, n_sms, st);
+    return launch_tc_shape<NC, BYTES, 0, 0, MODE>(tmaps, p, sh, n_sms, st);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -632,6 +727,33 @@ cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int 
     return cudaGetLastError();
 }
 
+size_t qld_tc_spectrum_digit_bytes(int N, int n_bins, size_t *pass_bytes)
+{
+    const int n_steps = ((N + 127) / 128) * 4;
+    const size_t per_pass = (size_t)n_steps * 256 * MMA_K;
+    if (pass_bytes) *pass_bytes = per_pass;
+    return per_pass * (size_t)((n_bins + 31) / 32);
+}
+
+cudaError_t qld_launch_spectrum_digits(int N, int q_lo, int n_bins, int8_t *digits, cudaStream_t st)
+{
+    const int n_steps = ((N + 127) / 128) * 4;
+    const int64_t total = (int64_t)((n_bins + 31) / 32) * n_steps * 256 * MMA_K;
+    k_spectrum_digits<<<(unsigned)((total + 255) / 256 < 65535 * 16 ? (total + 255) / 256 : 65535 * 16), 256, 0, st>>>(N, q_lo, n_bins, n_steps, digits);
+    return cudaGetLastError();
+}
+
+// one pass of the search: 32 bins, 256 columns, T = 1 span with two accumulator sets, 128-frame stages (the shape the tensor
+// maps must have been encoded for: force = {1, 4, 128})
+cudaError_t qld_launch_demod_tc_spectrum(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
+{
+    const CUtensorMap *tm = reinterpret_cast<const CUtensorMap *>(tmaps);
+    const int force[3] = {1, 4, 128};
+    const TcShape sh = tc_shape(256, p.row_bytes, p.N, n_sms, force);
+    if (sh.T != 1 || sh.kc != 128) return cudaErrorInvalidValue;
+    return p.bytes == 2 ? launch_tc_shape<256, 2, 1, 128, 2>(tm, p, sh, n_sms, st) : launch_tc_shape<256, 1, 1, 128, 2>(tm, p, sh, n_sms, st);
+}
+
 cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N, int8_t *digits, cudaStream_t st)
 {
     const int n_steps = (N + KC_PAD - 1) / KC_PAD * (KC_PAD / MMA_K);
@@ -643,7 +765,7 @@ cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
     const CUtensorMap *tm = reinterpret_cast<const CUtensorMap *>(tmaps);
-    if (p.bins_rows > 0) return p.bytes == 2 ? launch_tc<16, 2, true>(tm, p, n_sms, st) : launch_tc<16, 1, true>(tm, p, n_sms, st);
+    if (p.bins_rows > 0) return p.bytes == 2 ? launch_tc<16, 2, 1>(tm, p, n_sms, st) : launch_tc<16, 1, 1>(tm, p, n_sms, st);
     const int nc = qld_tc_columns(p.fin.K);
     if (p.bytes == 2) {
         switch (nc) {

@@ -21,6 +21,10 @@ struct TcParams {
     int32_t reserved2;
     int32_t *bins_out;        // [bins_rows padded][HW] int32 (the context's accumulator rows)
     int64_t bins_stride;      // elements between rows of bins_out (HW)
+    // unknown-frequency search (qld_dominant_bin): 32 DFT bins per launch (256 columns), running arg-max in spec_amp / spec_bin
+    float *spec_amp;          // [HW] largest amplitude so far (read unless spec_first)
+    int32_t *spec_bin;        // [HW] its bin
+    int32_t spec_q0, spec_nbins, spec_first, reserved3;
     FinParams fin;
 };
 
@@ -34,5 +38,10 @@ cudaError_t qld_launch_fixed_table_fill(const TableFillParams &p, int32_t *rfix,
 cudaError_t qld_launch_fixed_from_doubles(const double *tab, int n, int k, int32_t *rfix, int n_stride, cudaStream_t st);
 // B operand of the integer-bin contraction from the context's weight table wtab[cap_w][rows] (frames 1..N, entries s mod cap_w)
 cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N, int8_t *digits, cudaStream_t st);
+// digit tiles of the DFT bins q_lo .. q_lo + n_bins - 1 of an N-frame window (nu = q/N), 32 bins (256 columns) per pass, steps padded
+// to a multiple of 4 (128-frame stages); returns the bytes per pass through *pass_bytes
+size_t qld_tc_spectrum_digit_bytes(int N, int n_bins, size_t *pass_bytes);
+cudaError_t qld_launch_spectrum_digits(int N, int q_lo, int n_bins, int8_t *digits, cudaStream_t st);
+cudaError_t qld_launch_demod_tc_spectrum(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);

@@ -63,3 +63,19 @@ def test_dominant_bin_rejects_bad_ranges(Q):
         with pytest.raises(Q.QLDError) as e:
             Q.dominant_bin(x, lo, hi)
         assert e.value.status == Q.QLD_E_INVAL
+
+
+@pytest.mark.timeout(600, method="thread")
+@pytest.mark.parametrize("H,W,N,dtype,q_lo,q_hi", [(64, 256, 256, np.uint16, 1, 127), (96, 128, 200, np.uint8, 1, 99), (40, 200, 130, np.uint16, 3, 64),
+                                                   (128, 256, 520, np.uint16, 1, 70)])
+def test_dominant_bin_many_passes(Q, oracle, H, W, N, dtype, q_lo, q_hi):
+    """The 32-bins-per-pass tensor-core path: several passes (the running arg-max persists across launches), a ragged last
+    pass, windows that are not a multiple of the 128-frame stage, more tiles than SMs, full-range samples."""
+    rng = np.random.default_rng(N + q_hi)
+    hi = 256 if dtype == np.uint8 else 65536
+    x = rng.integers(0, hi, size=(N, H, W)).astype(dtype)
+    # a few strong tones so that the answer is unique on part of the frame
+    s = np.arange(1, N + 1)[:, None, None]
+    for q in (q_lo, (q_lo + q_hi) // 2, q_hi):
+        x[:, : H // 4, : W // 2] = np.clip(x[:, : H // 4, : W // 2].astype(np.int64) // 2 + (hi // 5) * (1 + np.sin(2 * np.pi * q * s / N)), 0, hi - 1).astype(dtype)
+    _check(Q, oracle, x, q_lo, q_hi)
