@@ -31,3 +31,15 @@ def test_reference_arm_prints_the_contract_line():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["metric"] == "qld_pixel_samples_per_s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0 and line["config"]["workload"] == "cfg1"
+
+
+def test_entry_points_parse_and_build():
+    """__graft_entry__ imports cleanly on a CPU box and build() produces both libraries (smoke() itself needs the GPU)."""
+    import importlib
+    sys.path.insert(0, ROOT)
+    g = importlib.import_module("__graft_entry__")
+    g.build()
+    assert os.path.exists(os.path.join(ROOT, "paper_1511_03390_b200", "libqld.so"))
+    import ast
+    ast.parse(open(os.path.join(ROOT, "__graft_entry__.py")).read())
+    assert callable(g.smoke)
