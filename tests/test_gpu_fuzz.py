@@ -71,7 +71,8 @@ def test_random_configuration(Q, oracle, seed):
     ctx.destroy()
 
 
-@pytest.mark.parametrize("seed", range(40))
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("seed", range(80))
 def test_random_sliding(Q, oracle, seed):
     rng = np.random.default_rng(5000 + seed)
     tile = rng.choice(["512,16", "1024,16", "2048,16", "1024,32", ""])
@@ -87,9 +88,13 @@ def test_random_sliding(Q, oracle, seed):
     kind = rng.choice(["bins", "fp32"])
     ref = {"num": 1, "den": int(rng.choice([4, 6, 8]))} if kind == "bins" else {"nu": float(rng.uniform(0.02, 0.48)), "phase": 0.3}
     stream = np.clip(rng.normal(1500, 60, size=(T, H, W)), 0, 4095).astype(np.uint16)
+    bulk = int(rng.integers(0, 3))                              # 0: automatic, 1: force k_slide_bulk, 2: never
+    if (H * W * 2) % 16 != 0 and bulk == 1:
+        bulk = 0
     try:
         ctx = mk(H, W, "u16", N, [ref], ring_frames=cap, accum=Q.QLD_ACC_INT_BINS if kind == "bins" else Q.QLD_ACC_FP32, max_value=4095,
                     slide_hop=hop if partial else 0)
+        ctx.debug_set_tile("slide", bulk)
         ctx.push_frames(stream[:N])
         ctx.demod(Q.QLD_SLIDE, hop)
     except Q.QLDError as e:
@@ -102,5 +107,5 @@ def test_random_sliding(Q, oracle, seed):
         ctx.sync()
         got = tuple(m.cpu().numpy() for m in ctx.get_maps(0))
         check_float_maps(got, oracle_maps(oracle, stream[w * hop:w * hop + N], ref, s_first=w * hop + 1), rel=1e-6 if kind == "bins" else 1e-5,
-                         what=f"seed {seed} window {w} {kind} {ctx.last_kernel()} {H}x{W} N={N} hop={hop} cap={cap} tile={tile!r} partial={partial}")
+                         what=f"seed {seed} window {w} {kind} {ctx.last_kernel()} {H}x{W} N={N} hop={hop} cap={cap} tile={tile!r} partial={partial} bulk={bulk}")
     ctx.destroy()
