@@ -77,6 +77,14 @@ struct SlideSmem {
     }
 };
 
+#ifdef QLD_SL_TRACE   // development builds only: time stamps of CTA 0
+__device__ unsigned long long g_sl_trace[8 * 64];
+__device__ __forceinline__ unsigned long long sl_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define SL_TRACE(kind, n) do { if (blockIdx.x == 0 && (n) < 64) g_sl_trace[(kind) * 64 + (n)] = sl_gtime(); } while (0)
+#else
+#define SL_TRACE(kind, n) do { } while (0)
+#endif
+
 template <typename T, typename ACC, int ROWS, bool PART>
 __global__ void __launch_bounds__(SL_THREADS, 1)
 k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ DemodParams p, const SlideShape sh, const int n_map_rows,
@@ -115,15 +123,21 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     for (int run = 0; run < p.n_runs; ++run) n_chunks += (p.run[run].n + KC - 1) / KC;
 
     if (threadIdx.x == 0) {
+        SL_TRACE(0, 0);
         if (blockIdx.x == 0) *counter_next = 0;   // the next launch's tile counter (the two alternate: no memset between launches)
-        for (int i = 0; i < STAGES; ++i) {
-            mbar_init(&full[i], 2);          // the producer's expect_tx arrival + its "weights written" arrival
-            mbar_init(&empty[i], SL_NW);
-        }
-        for (int i = 0; i < SL_MAX_SB; ++i) {
-            mbar_init(&state_full[i], 1);
-            mbar_init(&out_full[i], SL_NW * 32);
-            mbar_init(&state_empty[i], 1);
+    }
+    if (warp == 0) {
+        // barrier initialisation spread over the lanes of warp 0 (a serial loop in one thread cost 0.5 us of every launch)
+        const int n_bar = 2 * STAGES + 3 * SL_MAX_SB;
+        for (int i = lane; i < n_bar; i += 32) {
+            uint32_t count;
+            if (i < STAGES) count = 2;                                   // full: the producer's expect_tx arrival + its "weights written" arrival
+            else if (i < 2 * STAGES) count = SL_NW;                      // empty
+            else {
+                const int j = (i - 2 * STAGES) / SL_MAX_SB;              // state_full, out_full, state_empty
+                count = j == 1 ? SL_NW * 32 : 1;
+            }
+            mbar_init(&full[i], count);                                  // the barriers are contiguous: full, empty, state_full, out_full, state_empty
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -160,7 +174,9 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
             const int64_t pix0 = (int64_t)tile * TP;
             const int npx = (int)min((int64_t)TP, p.HW - pix0);
             if (lane == 0) {
+                SL_TRACE(1, it);
                 mbar_wait(&state_empty[sb], (uint32_t)((it / NSB) & 1) ^ 1u);
+                SL_TRACE(2, it);
                 unsigned char *st = sState + (size_t)sb * SM.state_bytes;
                 const uint32_t rb = (uint32_t)(npx * (int)sizeof(RED));
                 uint32_t bytes = (uint32_t)ROWS * rb * (PART ? 2u : 1u) + (IS_F32 ? (uint32_t)(npx * 4) : 0u);
@@ -252,6 +268,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             bulk_store(map_ptr[w] + (int64_t)k * p.HW + pix0, st + SM.off_map + (size_t)(k * n_which + map_slot[w]) * TP * 4, (uint32_t)(npx * 4));
                 bulk_commit();
                 bulk_wait_read0();                         // the copies have read the buffer (their global writes may still be in flight)
+                SL_TRACE(7, it);
                 mbar_arrive(&state_empty[sb]);
             }
             __syncwarp();
@@ -277,6 +294,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     uint32_t phase = 0;
     for (int it = 0;; ++it) {
         mbar_wait(&full[stage], phase);
+        if (ct == 0) SL_TRACE(3, it);
         const int tile = tile_q[it & (SL_TQ - 1)];
         const int sb = it % NSB;
         const uint32_t spar = (uint32_t)((it / NSB) & 1);
@@ -399,7 +417,9 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
         }
 
         // ---- update the stored sums (A5) in place in the state buffer, then A4 ----
+        if (ct == 0) SL_TRACE(4, it);
         if constexpr (!IS_F32) mbar_wait(&state_full[sb], spar);
+        if (ct == 0) SL_TRACE(5, it);
         RED a[ROWS][V];
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
@@ -465,6 +485,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                     store_vec<float, V>(reinterpret_cast<float *>(st + SM.off_map) + (size_t)(k * n_which + map_slot[w]) * TP + (size_t)ct * V, o[w]);
         }
         fence_async_smem();                                // generic-proxy writes before the store warp's bulk copies read them
+        if (ct == 0) SL_TRACE(6, it);
         if (ct == 0) out_tile[sb] = tile;
         mbar_arrive(&out_full[sb]);
     }
@@ -578,3 +599,10 @@ cudaError_t qld_launch_slide_bulk(int dtype, int kind, int rows, const void *tma
     default: return cudaErrorInvalidValue;
     }
 }
+
+#ifdef QLD_SL_TRACE
+extern "C" int qld_sl_trace_read(unsigned long long *out, int n)
+{
+    return (int)cudaMemcpyFromSymbol(out, g_sl_trace, sizeof(unsigned long long) * (size_t)n);
+}
+#endif
