@@ -147,14 +147,24 @@ class Env:
         self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
         self.world = int(os.environ.get("WORLD_SIZE", "1"))
         assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
-        torch.cuda.set_device(self.local_rank)
-        self.dev = torch.device("cuda", self.local_rank)
+        n_dev = torch.cuda.device_count()
+        # fewer GPUs than ranks (a one-GPU box exercising the N > 1 code path): ranks share devices and the host-side
+        # collectives go over gloo -- the ranks' kernels are independent of one another, only the timing barriers are shared.
+        # Such a run checks the plumbing; its numbers are not a scaling measurement and the line says so.
+        self.oversubscribed = self.world > n_dev
+        self.local_dev = self.local_rank % n_dev
+        torch.cuda.set_device(self.local_dev)
+        self.dev = torch.device("cuda", self.local_dev)
         self.dist = None
         if self.world > 1:
             import torch.distributed as dist
             os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-            dist.init_process_group("nccl", device_id=self.dev)
+            if self.oversubscribed:
+                dist.init_process_group("gloo")
+            else:
+                dist.init_process_group("nccl", device_id=self.dev)
             self.dist = dist
+        self.red_dev = torch.device("cpu") if self.oversubscribed else self.dev
 
     def barrier(self):
         if self.dist is not None:
@@ -164,14 +174,14 @@ class Env:
     def max_over_ranks(self, x: float) -> float:
         if self.dist is None:
             return x
-        t = self.torch.tensor([x], device=self.dev, dtype=self.torch.float64)
+        t = self.torch.tensor([x], device=self.red_dev, dtype=self.torch.float64)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
         return float(t.item())
 
     def sum_over_ranks(self, x: float) -> float:
         if self.dist is None:
             return x
-        t = self.torch.tensor([x], device=self.dev, dtype=self.torch.float64)
+        t = self.torch.tensor([x], device=self.red_dev, dtype=self.torch.float64)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
         return float(t.item())
 
@@ -184,7 +194,7 @@ class Env:
         for _ in range(warmup):
             step()
         self.barrier()
-        sampler = ClockSampler(self.local_rank)
+        sampler = ClockSampler(self.local_dev)
         sampler.start()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         self.barrier()
@@ -676,6 +686,8 @@ def main():
                      "data": "synthetic", "dtype": r["dtype"], "vs_baseline": None, "scaling": r.get("scaling", "weak"),
                      "higher_is_better": True, "ms_per_step": r["ms_per_step"], "warmup": args.warmup, "steps": args.steps,
                      "n_gpus": env.world, "unit": UNIT, "value": r["value"], "metric": METRIC})
+        if env.oversubscribed:
+            line["oversubscribed"] = f"{env.world} ranks on {env.torch.cuda.device_count()} GPU(s): a plumbing check, not a scaling measurement"
         if "window_samples_per_s" in r:
             line["window_samples_per_s"] = r["window_samples_per_s"]
         print(json.dumps(line), flush=True)

@@ -118,3 +118,25 @@ def test_row_bands_through_libqld_on_one_gpu(name, shape, accum_name):
     for ctx, _, _ in keep:
         ctx.destroy()
     whole.destroy()
+
+
+@pytest.mark.gpu
+@pytest.mark.timeout(600, method="thread")
+@pytest.mark.parametrize("shard_mode,scaling", [("rows", "strong"), ("stacks", "weak")])
+def test_bench_spawns_ranks_and_shards(shard_mode, scaling):
+    """`python bench.py --gpus 2` outside torchrun re-executes itself with two ranks (on a one-GPU box they share the device and
+    the host collectives go over gloo: a plumbing check).  --shard rows: the two ranks split ONE cfg1 frame into row bands, each
+    through libqld; rank 0's band is checked against the oracle inside the bench; the line says n_gpus = 2."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--shard", shard_mode, "--workload", "cfg1", "--steps", "10",
+                          "--e2e-steps", "1", "--also", "none", "--ref-rows", "16"], capture_output=True, text=True, timeout=500, env=env)
+    assert out.returncode == 0, out.stderr[-800:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == scaling and line["value"] > 0 and line["parity"]["ok"]
+    assert line["e2e"]["value"] > 0 and line["gpu_launches"] >= 10
+    import torch
+    assert ("oversubscribed" in line) == (torch.cuda.device_count() < 2)
