@@ -92,6 +92,8 @@ struct qld_ctx {
     cudaEvent_t push_ev[N_PUSH_EVENTS];
     int push_ev_next;
     bool push_pending;
+    uint64_t push_seq, waited_seq;   // push events recorded / the last one the compute stream was made to wait for
+    int64_t tab_filled;      // ring: reference tables are filled up to this absolute frame index (they may run ahead of the frames)
     DemodEvent demod_ev[N_DEMOD_EVENTS];
     int demod_ev_next;
     cudaEvent_t tables_ev;
@@ -383,9 +385,10 @@ int wait_for_readers(qld_ctx *c, int64_t last_overwritten)
 }
 
 // src == NULL: the frames were written in place by the caller (qld_commit_frames); nothing is copied
-int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
+int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind, bool producer_wait = false)
 {
     const size_t fb = (size_t)c->HW * c->bytes;
+    bool enqueued = src != nullptr || producer_wait || !c->ring;
     if (!c->ring) {
         if (c->pushed + n > c->N) return fail(c, QLD_E_OVERRUN, "push: whole-window store already holds N frames (qld_reset first)");
         // frames still being read by an earlier demod of the previous stack
@@ -406,14 +409,30 @@ int push_common(qld_ctx *c, const void *src, int n, cudaMemcpyKind kind)
             CU(c, cudaMemcpyAsync(c->frames + (size_t)slot * fb, src, (size_t)n1 * fb, kind, c->s_copy));
             if (n1 < n) CU(c, cudaMemcpyAsync(c->frames, static_cast<const unsigned char *>(src) + (size_t)n1 * fb, (size_t)(n - n1) * fb, kind, c->s_copy));
         }
-        int rc = fill_tables(c, first, n, c->s_copy);
-        if (rc) return rc;
+        if (last > c->tab_filled) {
+            // The table entry of a frame depends on its index only, so the tables may run ahead of the frames as far as the
+            // table ring allows: an entry may be overwritten once no issued or pending window needs it (a window that starts
+            // after a frames reads the entries of frames a .. a + N).  With a roomy ring most pushes then launch nothing.
+            int64_t floor_needed = c->seeded ? c->win_start : 0;
+            for (int i = 0; i < N_DEMOD_EVENTS; ++i)
+                if (c->demod_ev[i].used && c->demod_ev[i].oldest_read - 1 < floor_needed) floor_needed = c->demod_ev[i].oldest_read - 1;
+            int64_t target = floor_needed + c->cap_w - 1;
+            if (target > last + 4096) target = last + 4096;
+            if (target < last) target = last;                 // the frames themselves always fit (checked above)
+            int rc = fill_tables(c, c->tab_filled + 1, (int)(target - c->tab_filled), c->s_copy);
+            if (rc) return rc;
+            c->tab_filled = target;
+            enqueued = true;
+        }
     }
     c->pushed += n;
-    cudaEvent_t ev = c->push_ev[c->push_ev_next];
-    c->push_ev_next = (c->push_ev_next + 1) % N_PUSH_EVENTS;
-    CU(c, cudaEventRecord(ev, c->s_copy));
-    c->push_pending = true;
+    if (enqueued) {                                           // nothing new on the copy stream: the last event still stands
+        cudaEvent_t ev = c->push_ev[c->push_ev_next];
+        c->push_ev_next = (c->push_ev_next + 1) % N_PUSH_EVENTS;
+        CU(c, cudaEventRecord(ev, c->s_copy));
+        c->push_seq++;
+        c->push_pending = true;
+    }
     return QLD_OK;
 }
 
@@ -877,7 +896,7 @@ int qld_commit_frames(qld_ctx *c, int n_frames, void *producer_stream)
         CU(c, cudaEventRecord(c->tables_ev, static_cast<cudaStream_t>(producer_stream)));
         CU(c, cudaStreamWaitEvent(c->s_copy, c->tables_ev, 0));
     }
-    return push_common(c, nullptr, n_frames, cudaMemcpyDefault);
+    return push_common(c, nullptr, n_frames, cudaMemcpyDefault, producer_stream != nullptr);
 }
 
 int qld_attach_frames_device(qld_ctx *c, const void *device_frames)
@@ -914,7 +933,10 @@ int qld_demod(qld_ctx *c, int mode, int hop)
     if (mode != QLD_WHOLE && mode != QLD_SLIDE) return fail(c, QLD_E_INVAL, "demod: unknown mode");
     if (!c->frames) return fail(c, QLD_E_STATE, "demod: no frames attached");
     if (c->tables_supplied && c->tables_set != (1u << c->K) - 1u) return fail(c, QLD_E_STATE, "demod: qld_set_ref_tables has not been called for every reference");
-    if (c->push_pending || c->pushed > 0) CU(c, cudaStreamWaitEvent(c->s_comp, last_push_event(c), 0));
+    if (c->push_seq != c->waited_seq) {                      // order the kernels after every push issued so far (once per event)
+        CU(c, cudaStreamWaitEvent(c->s_comp, last_push_event(c), 0));
+        c->waited_seq = c->push_seq;
+    }
     if (mode == QLD_WHOLE) {
         if (c->pushed < c->N) return fail(c, QLD_E_STATE, "demod: fewer than N frames stored");
         const int64_t a = c->ring ? c->pushed - c->N : 0;
@@ -990,7 +1012,7 @@ int qld_read_ref_table(qld_ctx *c, int k, int64_t s_first, int n, float *sin_out
 {
     if (!c || k < 0 || k >= c->K || n < 1 || s_first < 1) return c ? fail(c, QLD_E_INVAL, "read_ref_table: bad argument") : QLD_E_INVAL;
     if (c->is_int || c->is_fixed || c->fix_ring) return fail(c, QLD_E_STATE, "read_ref_table: this context has no float table");
-    if (c->ring && (s_first + n - 1 > c->pushed || s_first + c->cap_w <= c->pushed + 1)) return fail(c, QLD_E_STATE, "read_ref_table: frames not in the ring");
+    if (c->ring && (s_first + n - 1 > c->pushed || s_first + c->cap_w <= (c->tab_filled > c->pushed ? c->tab_filled : c->pushed) + 1)) return fail(c, QLD_E_STATE, "read_ref_table: frames not in the ring");
     if (!c->ring && s_first + n - 1 > c->N) return fail(c, QLD_E_INVAL, "read_ref_table: beyond the window");
     CU(c, cudaStreamSynchronize(c->s_copy));
     for (int i = 0; i < n; ++i) {
@@ -1115,7 +1137,7 @@ int qld_reset(qld_ctx *c)
     if (c->sticky) return QLD_E_CUDA;
     int rc = qld_sync(c);
     if (rc) return rc;
-    c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0;
+    c->pushed = 0; c->windows_done = 0; c->seeded = false; c->win_start = 0; c->hops_since_seed = 0; c->tab_filled = 0;
     for (int i = 0; i < N_DEMOD_EVENTS; ++i) c->demod_ev[i].used = false;
     if (!c->ring && c->frames != c->own_frames) {          // an attached stack is detached (an attached ring stays attached)
         c->frames = c->own_frames; c->tmap_valid = false; c->stream_tmap_frames = nullptr; c->slide_tmap_frames = nullptr;
