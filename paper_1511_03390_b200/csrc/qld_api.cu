@@ -56,7 +56,7 @@ struct qld_ctx {
     int32_t *rfix;           // [2K][N] Q30 references
     int8_t *digits;          // digit tiles for the MMA B operand
     int64_t *sums;           // optional [2K][HW] exact sums
-    unsigned int *tile_counter;   // two counters that alternate between launches: each launch zeroes the other one
+    unsigned int *tile_counter;   // three counters in rotation: each launch zeroes the next launch's one
     unsigned int counter_flip;
     alignas(64) unsigned char tmap[256];   // two CUtensorMap (qld_tc_encode_tmap)
     bool tmap_valid;
@@ -315,7 +315,7 @@ int fill_tables(qld_ctx *c, int64_t s_first, int n, cudaStream_t st)
 
 int init_device_state(qld_ctx *c)
 {
-    CU(c, cudaMemsetAsync(c->tile_counter, 0, 2 * sizeof(unsigned int), c->s_copy));
+    CU(c, cudaMemsetAsync(c->tile_counter, 0, 3 * sizeof(unsigned int), c->s_copy));
     // tables zeroed (padding rows stay zero; cum entry of frame 0 is zero), then filled for the whole store
     if (!c->is_fixed) {
         CU(c, cudaMemsetAsync(c->wtab, 0, (size_t)c->cap_w * c->rows_pad * 4, c->s_copy));
@@ -367,8 +367,10 @@ int fetch_bin_weights(qld_ctx *c)
 // the tile counter of the next persistent-kernel launch (zero) and the one that launch has to zero
 void next_counters(qld_ctx *c, unsigned int **cur, unsigned int **nxt)
 {
-    *cur = c->tile_counter + (c->counter_flip & 1u);
-    *nxt = c->tile_counter + ((c->counter_flip + 1u) & 1u);
+    // three counters in rotation: a launch that starts early (programmatic dependent launch, k_slide_bulk) zeroes a counter that the
+    // launch still running before it does not use
+    *cur = c->tile_counter + (c->counter_flip % 3u);
+    *nxt = c->tile_counter + ((c->counter_flip + 1u) % 3u);
     c->counter_flip++;
 }
 

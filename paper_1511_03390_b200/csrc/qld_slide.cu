@@ -16,6 +16,8 @@
 //
 // Arithmetic is that of k_demod_stream / k_demod_slide: int32 bins exact; fp32 partial sums of pedestal-subtracted samples
 // added into fp64 stored sums.
+#include <string.h>
+
 #include "qld_device.cuh"
 #include "qld_ptx.cuh"
 #include "qld_slide.h"
@@ -124,7 +126,10 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
 
     if (threadIdx.x == 0) {
         SL_TRACE(0, 0);
-        if (blockIdx.x == 0) *counter_next = 0;   // the next launch's tile counter (the two alternate: no memset between launches)
+        if (blockIdx.x == 0) {
+            *counter_next = 0;                    // the next launch's tile counter (three rotate: no memset between launches)
+            __threadfence();
+        }
     }
     if (warp == 0) {
         // barrier initialisation spread over the lanes of warp 0 (a serial loop in one thread cost 0.5 us of every launch)
@@ -143,6 +148,10 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     }
     __syncthreads();
     (void)row_bytes;
+    // Programmatic dependent launch: the next launch of the stream may start on SMs as they free up -- its CTAs initialise their
+    // barriers and put the frames of their first tile in flight while this launch drains -- but it touches the sums this launch
+    // updates only after griddepcontrol.wait (producer, below), i.e. after this grid has completed and its writes are visible.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     RED *accg = static_cast<RED *>(p.acc_out);
     RED *partg = static_cast<RED *>(p.part);
@@ -175,6 +184,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
             const int npx = (int)min((int64_t)TP, p.HW - pix0);
             if (lane == 0) {
                 SL_TRACE(1, it);
+                if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's sums are final from here on
                 mbar_wait(&state_empty[sb], (uint32_t)((it / NSB) & 1) ^ 1u);
                 SL_TRACE(2, it);
                 unsigned char *st = sState + (size_t)sb * SM.state_bytes;
@@ -513,8 +523,18 @@ cudaError_t launch_slide_n(const void *tmap, const DemodParams &p, const SlideSh
         smem_set = SM.total + 128;
     }
     const int n_tiles = (int)((p.HW + SL_TP - 1) / SL_TP);
-    kern<<<n_tiles < n_sms ? n_tiles : n_sms, SL_THREADS, SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, n_map_rows, counter, counter_next);
-    return cudaGetLastError();
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    lc.gridDim = dim3((unsigned)(n_tiles < n_sms ? n_tiles : n_sms));
+    lc.blockDim = dim3(SL_THREADS);
+    lc.dynamicSmemBytes = (size_t)SM.total + 128;
+    lc.stream = st;
+    cudaLaunchAttribute at;
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;    // may overlap the tail of the launch before it (see the kernel)
+    at.val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = &at;
+    lc.numAttrs = 1;
+    return cudaLaunchKernelEx(&lc, kern, *reinterpret_cast<const CUtensorMap *>(tmap), p, sh, n_map_rows, counter, counter_next);
 }
 
 template <typename T, typename ACC>

@@ -48,7 +48,19 @@ extern "C" int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_
         size_t pass_bytes = 0;
         const size_t dig_bytes = qld_tc_spectrum_digit_bytes(N, n_bins, &pass_bytes);
         unsigned char *scratch = nullptr;                    // digit tiles + two tile counters
-        // stream-ordered allocation: no device-wide synchronisation on either side of the search
+        // stream-ordered allocation: no device-wide synchronisation on either side of the search; the default pool is told to
+        // keep what it has at synchronisation points (it otherwise returns the block to the driver after every call, which
+        // costs milliseconds now and then)
+        {
+            int dev = 0;
+            cudaMemPool_t pool;
+            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                uint64_t keep = 64ull << 20, cur = 0;
+                if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &cur) == cudaSuccess && cur < keep)
+                    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            (void)cudaGetLastError();
+        }
         if (cudaMallocAsync(reinterpret_cast<void **>(&scratch), dig_bytes + 256, st) != cudaSuccess) { (void)cudaGetLastError(); return QLD_E_NOMEM; }
         int8_t *digits = reinterpret_cast<int8_t *>(scratch);
         unsigned int *counters = reinterpret_cast<unsigned int *>(scratch + dig_bytes);
