@@ -66,7 +66,8 @@ extern "C" int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_
         unsigned int *counters = reinterpret_cast<unsigned int *>(scratch + dig_bytes);
         int rc = QLD_OK;
         alignas(64) unsigned char tmaps[256];
-        const int force[3] = {1, 4, 128};
+        int force[3];
+        qld_tc_spectrum_shape(force);
         int n_sms = qld_sm_count();
         if (cudaMemsetAsync(counters, 0, 8, st) != cudaSuccess) rc = QLD_E_CUDA;
         if (rc == QLD_OK && qld_launch_spectrum_digits(N, q_lo, n_bins, digits, st) != cudaSuccess) rc = QLD_E_CUDA;

@@ -32,6 +32,12 @@
 using namespace qld_ptx;
 using qld_angle::half_turns_of;
 
+// tile shape of the unknown-frequency search (256 columns): T = 2 spans share every digit tile (the digit tiles are twice the
+// bytes of a span's frames: with T = 1 the L2 -> shared-memory traffic, three times the HBM traffic, is the bound), one
+// accumulator set handed back span by span
+#define QLD_SPEC_T 2
+#define QLD_SPEC_STAGES 3
+
 namespace {
 
 constexpr int KC_PAD = 64;        // the digit tiles are padded to a multiple of this many frames
@@ -444,7 +450,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                     if (writer && !p.spec_first) prev_amp = __ldg(p.spec_amp + pixel);
                     uint32_t rn[16];
                     tc_ld16(taddr + eset * 16, rn);                             // software pipeline: the next group's columns are in flight
+#ifdef QLD_SPEC_PROBE
+                    for (int g = eset; g < QLD_SPEC_PROBE; g += EPI_SETS) {
+#else
                     for (int g = eset; g < NC / 16; g += EPI_SETS) {
+#endif
                         uint32_t r[16];
                         tc_wait_ld();
 #pragma unroll
@@ -743,15 +753,17 @@ cudaError_t qld_launch_spectrum_digits(int N, int q_lo, int n_bins, int8_t *digi
     return cudaGetLastError();
 }
 
-// one pass of the search: 32 bins, 256 columns, T = 1 span with two accumulator sets, 128-frame stages (the shape the tensor
-// maps must have been encoded for: force = {1, 4, 128})
+// one pass of the search: 32 bins, 256 columns, QLD_SPEC_T spans per tile, 128-frame stages (the shape the tensor maps must have
+// been encoded for: qld_tc_spectrum_shape)
+void qld_tc_spectrum_shape(int force_out[3]) { force_out[0] = QLD_SPEC_T; force_out[1] = QLD_SPEC_STAGES; force_out[2] = 128; }
+
 cudaError_t qld_launch_demod_tc_spectrum(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st)
 {
     const CUtensorMap *tm = reinterpret_cast<const CUtensorMap *>(tmaps);
-    const int force[3] = {1, 4, 128};
+    const int force[3] = {QLD_SPEC_T, QLD_SPEC_STAGES, 128};
     const TcShape sh = tc_shape(256, p.row_bytes, p.N, n_sms, force);
-    if (sh.T != 1 || sh.kc != 128) return cudaErrorInvalidValue;
-    return p.bytes == 2 ? launch_tc_shape<256, 2, 1, 128, 2>(tm, p, sh, n_sms, st) : launch_tc_shape<256, 1, 1, 128, 2>(tm, p, sh, n_sms, st);
+    if (sh.T != QLD_SPEC_T || sh.kc != 128) return cudaErrorInvalidValue;
+    return p.bytes == 2 ? launch_tc_shape<256, 2, QLD_SPEC_T, 128, 2>(tm, p, sh, n_sms, st) : launch_tc_shape<256, 1, QLD_SPEC_T, 128, 2>(tm, p, sh, n_sms, st);
 }
 
 cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N, int8_t *digits, cudaStream_t st)

@@ -42,6 +42,7 @@ cudaError_t qld_launch_bins_pack(const int32_t *wtab, int cap_w, int rows, int N
 // to a multiple of 4 (128-frame stages); returns the bytes per pass through *pass_bytes
 size_t qld_tc_spectrum_digit_bytes(int N, int n_bins, size_t *pass_bytes);
 cudaError_t qld_launch_spectrum_digits(int N, int q_lo, int n_bins, int8_t *digits, cudaStream_t st);
+void qld_tc_spectrum_shape(int force_out[3]);     // {T, stages, KC} the search's tensor maps are encoded for
 cudaError_t qld_launch_demod_tc_spectrum(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);
 cudaError_t qld_launch_digit_pack(const int32_t *rfix, int n_stride, int N, int K, int8_t *digits, cudaStream_t st);
 cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms, cudaStream_t st);
