@@ -134,7 +134,7 @@ def run_reference(args, rank, world):
 
 
 
-ACCUM_NAMES = {"auto": 0, "fp32": 1, "bins": 2, "fixed": 3}
+ACCUM_NAMES = {"auto": 0, "fp32": 1, "bins": 2, "fixed": 3, "refs": 4}
 
 
 class Env:
@@ -288,7 +288,7 @@ def bench_whole(env: Env, args, workload: str, accum_name: str, steps: int, warm
     in_l2 = samples * b <= 126e6
     res["roofline"] = roofline_hbm(algo, ms / steps, workload, kernel,
                                    "input fits the 126 MB L2 and is re-read every step: L2-resident, not an HBM number" if in_l2 else None)
-    res["dtype"] = {"INT_BINS": "int32", "FIXED": "int8 x int8 -> int32 -> int64 (tcgen05)", "FP32": "f32"}[mode]
+    res["dtype"] = {"INT_BINS": "int32", "INT_REFS": "int32", "FIXED": "int8 x int8 -> int32 -> int64 (tcgen05)", "FP32": "f32"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": map_names, "step": "qld_demod(QLD_WHOLE) over the resident stack",
                      "cache": f"input {samples * b / 1e6:.0f} MB per step " + ("<= 126 MB L2: L2-resident" if in_l2 else "> 126 MB L2: no flush needed"),
@@ -395,8 +395,9 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     ms, clocks, launches = env.timed(step, steps, warmup, keep_busy=step, counter=ctx.kernel_launches)
     kernel = ctx.last_kernel()
     mode = ctx.accum_name()
-    n_rows = ctx.get_bins(0).shape[0] if mode == "INT_BINS" else 2 * K
-    acc_bytes = 4 if mode == "INT_BINS" else 8                # int32 bins; fp64 (FP32 mode) or int64 (FIXED) stored sums
+    is_int = mode in ("INT_BINS", "INT_REFS")
+    n_rows = ctx.get_bins(0).shape[0] if is_int else 2 * K
+    acc_bytes = 4 if is_int else 8                # int32 bins; fp64 (FP32 mode) or int64 (FIXED) stored sums
     samples = float(hop) * H * W                              # new pixel-samples consumed per step
     res = {"workload": workload, "value": env.world * samples * steps / (ms * 1e-3), "ms_per_step": ms / steps,
            "maps_per_s": env.world * K * steps / (ms * 1e-3), "clocks": clocks, "kernel": kernel, "gpu_launches": int(launches),
@@ -420,7 +421,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
     res["roofline"]["frac_moved"] = res["roofline"]["frac"]
     res["roofline"]["survey_A5_bytes_per_launch"] = survey
     res["roofline"]["frac_survey_A5"] = survey / (ms / steps * 1e-3) / 1e9 / peak
-    res["dtype"] = {"INT_BINS": "int32", "FP32": "f32", "FIXED": "int64 (Q1.30 references)"}[mode]
+    res["dtype"] = {"INT_BINS": "int32", "INT_REFS": "int32", "FP32": "f32", "FIXED": "int64 (Q1.30 references)"}[mode]
     res["config"] = {"workload": workload, "H": H, "W": W, "N": N, "hop": hop, "K": K, "input_dtype": sc.dtype, "accum": mode,
                      "maps": "amplitude", "step": "qld_commit_frames(hop) + qld_demod(QLD_SLIDE, hop) over the resident ring",
                      "update": "block partial sums (cfg.slide_hop = hop): only the new frames are read" if slide_hop else "expired frames re-read",
@@ -459,12 +460,12 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
                 done += 1
                 for k in range(K):
                     got = tuple(None if m is None else m[r0:r0 + rows].cpu().numpy() for m in pctx.get_maps(k))
-                    worst = max(worst, check_float_maps(got, out[k], rel=1e-6 if mode == "INT_BINS" else 1e-5, what=f"bench parity cfg3 window {w}"))
+                    worst = max(worst, check_float_maps(got, out[k], rel=1e-6 if is_int else 1e-5, what=f"bench parity cfg3 window {w}"))
         res["cpu_baseline"] = {"value": done * float(hop) * rows * W / secs, "unit": UNIT, "cores": nt, "kind": "oracle",
                                "sample": f"{done} windows (w = {check_at}) recomputed directly from the definition on rows {r0}..{r0 + rows - 1}: "
                                          f"{done} x {N} x {rows} x {W} sample-products, {secs:.2f} s; value counts hop x rows x W new samples per window",
                                "window_samples_per_s": done * float(N) * rows * W / secs}
-        res["parity"] = {"rows_checked": rows, "windows_checked": check_at, "tolerance": "1e-6" if mode == "INT_BINS" else "1e-5 floored",
+        res["parity"] = {"rows_checked": rows, "windows_checked": check_at, "tolerance": "1e-6" if is_int else "1e-5 floored",
                          "strict_max_rel_err_amp": worst, "ok": True}
         pctx.destroy()
     ctx.destroy()
@@ -537,7 +538,7 @@ def bench_slide(env: Env, args, workload: str, accum_name: str, steps: int, warm
                 sub = hs[w * hop:w * hop + N, r0:r0 + rows, :].numpy()
                 out = oracle.qld(sub, refs[0], s_first=w * hop + 1, nthreads=nt)
                 got = (None, None, kept[w][0, r0:r0 + rows].numpy(), None)
-                worst = max(worst, check_float_maps(got, out, rel=1e-6 if mode == "INT_BINS" else 1e-5, what=f"e2e stream window {w}"))
+                worst = max(worst, check_float_maps(got, out, rel=1e-6 if is_int else 1e-5, what=f"e2e stream window {w}"))
             res["e2e"]["parity"] = {"windows_checked": check_at, "rows_checked": rows, "strict_max_rel_err_amp": worst, "ok": True,
                                     "note": "amplitude maps of the streamed run (ring wrapped " + str((sc.n_frames - 1) // ring_frames) + " times) vs the oracle's direct recomputation"}
         ectx.destroy()

@@ -63,6 +63,11 @@ typedef enum {
  *             in int32, exact; I, Q = sum_r B_r * sin/cos(2*pi*r/den + phase) in fp64.  For den = 4 and a
  *             phase that is a multiple of pi/2 the references are integers {0, +-1} and I, Q are exact
  *             integers ("integer-valued reference" path).  QLD_E_UNSUPPORTED if a bin could overflow int32.
+ *  INT_REFS : INT_BINS with the most compact exact form where one exists: for den = 3 or 6 and no phase offset the scaled
+ *             references (2/sqrt3) sin theta_s in {0, +-1} and 2 cos theta_s in {+-1, +-2} are integers, so TWO exact int32 sums
+ *             per reference suffice (2Q = 2B0+B1-B2-2B3-B4+B5, (2/sqrt3) I = B1+B2-B4-B5) instead of three bin
+ *             rows: I = (sqrt3/2) row 0, Q = row 1 / 2.  Other references of the context keep their bin rows.  A third less
+ *             accumulator traffic in a sliding update.  qld_get_bins then returns those two integer-reference sums.
  *  FIXED    : fixed-point references R(s) = rint(2^30 * sin/cos(theta_s)) (Q1.30 integers; the table can also
  *             be supplied, qld_set_ref_table_fixed).  I*2^30 = sum_s x_s R_sin(s), Q likewise, exact in int64:
  *             computed on the tcgen05 tensor cores as a [pixel bytes x frames].[frames x reference digits]
@@ -73,10 +78,10 @@ typedef enum {
  *             bulk-copy sliding kernel (64-bit integer multiply-add on the CUDA cores) -- the sliding window of P:181-183
  *             with float references and no drift at all, at any nu; the table entry of a frame is a function of its
  *             absolute index and is extended per push.
- *  AUTO     : INT_BINS when every reference is rational with den <= 16 and the bound holds; else FIXED for
+ *  AUTO     : INT_REFS (= INT_BINS, compact where possible) when every reference is rational with den <= 16 and the bound holds; else FIXED for
  *             K >= 4 references on a whole-window store that meets FIXED's conditions (the CUDA-core kernel is
  *             instruction-bound there, the contraction is HBM-bound and more accurate than fp32); else FP32. */
-typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2, QLD_ACC_FIXED = 3 } qld_accum;
+typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2, QLD_ACC_FIXED = 3, QLD_ACC_INT_REFS = 4 } qld_accum;
 
 typedef enum { QLD_NORM_PAPER = 0 /* no scaling (G3) */, QLD_NORM_AMPLITUDE = 1 /* I, Q, R times 2/N */ } qld_norm;
 
@@ -199,7 +204,7 @@ int qld_demod(qld_ctx *ctx, int mode, int hop);
  * Any out-pointer may be NULL.  A map that was not requested in cfg.maps comes back as NULL. */
 int qld_get_maps(qld_ctx *ctx, int k, const float **I, const float **Q, const float **amp, const float **phase);
 
-/* INT_BINS only: device pointer to the exact int32 accumulators of reference k, [n_rows][H][W].  For even
+/* INT_BINS / INT_REFS only: device pointer to the exact int32 accumulators of reference k, [n_rows][H][W].  For even
  * den the rows are the differences D_r = B_r - B_{r+den/2}, r = 0..den/2-1 (n_rows = den/2); for odd den the
  * bins B_r (n_rows = den).  For den = 4, phase 0: D_0 = Q, D_1 = I exactly. */
 int qld_get_bins(qld_ctx *ctx, int k, const int32_t **rows, int *n_rows);

@@ -158,7 +158,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     if (cfg->K < 1 || cfg->K > QLD_MAX_K || !cfg->refs) return bad(QLD_E_INVAL, "K must be 1..8 with refs given");
     if (cfg->ring_frames < -1 || (cfg->ring_frames > 0 && cfg->ring_frames <= cfg->N))
         return bad(QLD_E_INVAL, "ring_frames must be -1, 0, or > N");
-    if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_FIXED) return bad(QLD_E_INVAL, "unknown accum");
+    if (cfg->accum < QLD_ACC_AUTO || cfg->accum > QLD_ACC_INT_REFS) return bad(QLD_E_INVAL, "unknown accum");
     if (cfg->external_store != 0 && cfg->external_store != 1) return bad(QLD_E_INVAL, "external_store must be 0 or 1");
     if (cfg->slide_hop < 0 || cfg->slide_hop > cfg->N) return bad(QLD_E_INVAL, "slide_hop must be 0..N");
     if (cfg->slide_hop > 0 && cfg->ring_frames <= 0) return bad(QLD_E_INVAL, "slide_hop needs a ring context");
@@ -199,20 +199,26 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     }
     // accumulation mode
     const uint64_t vmax = cfg->max_value ? cfg->max_value : (cfg->dtype == QLD_U8 ? 255u : 65535u);
-    auto bins_rows = [&](int *rows_out) {
+    // INT_REFS: references with den = 3 or 6 and no phase offset take the two-row integer-reference form
+    auto compact = [&](int k, bool want) {
+        const RefPlan &rp = pl->ref[k];
+        return want && (rp.den == 3 || rp.den == 6) && rp.phase == 0.0 && (rp.phase_quarter & 3) == 0;
+    };
+    auto bins_rows = [&](int *rows_out, bool want_compact) {
         int rows = 0;
         for (int k = 0; k < cfg->K; ++k) {
             const int64_t den = pl->ref[k].den;
-            rows += (int)((den % 2 == 0) ? den / 2 : den);
+            rows += compact(k, want_compact) ? 2 : (int)((den % 2 == 0) ? den / 2 : den);
         }
         *rows_out = rows;
         return rows <= QLD_MAX_ROWS;
     };
-    auto bins_fit = [&]() {   // |row sum| <= vmax * (number of frames that can land in one row)
+    auto bins_fit = [&](bool want_compact) {   // |row sum| <= vmax * (number of frames that can land in one row)
         for (int k = 0; k < cfg->K; ++k) {
             const int64_t den = pl->ref[k].den;
-            const int64_t per_row = ((int64_t)cfg->N + den - 1) / den * ((den % 2 == 0) ? 1 : 1);
-            // a difference row takes +x from bin r and -x from bin r+den/2: magnitude bounded by one bin's sum
+            // a difference row takes +x from bin r and -x from bin r+den/2: magnitude bounded by one bin's sum; an
+            // integer-reference row takes every frame with a weight of magnitude <= 2
+            const int64_t per_row = compact(k, want_compact) ? 2 * (int64_t)cfg->N : ((int64_t)cfg->N + den - 1) / den;
             if ((unsigned __int128)vmax * (uint64_t)(per_row + 1) >= (1ull << 31)) return false;
         }
         return true;
@@ -224,12 +230,13 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         // store the CUDA-core kernel is instruction-issue bound (16+ FMA per sample) and the
         // exact int8 contraction on the tensor cores is used; otherwise pedestal-subtracted fp32
         const bool tc_ok = !pl->ring && cfg->K >= 4 && (pl->HW * pl->bytes) % 16 == 0 && cfg->N <= 65536 && !(cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64));
-        acc = (all_rational && max_den <= 16 && bins_rows(&rows) && bins_fit()) ? QLD_ACC_INT_BINS : (tc_ok ? QLD_ACC_FIXED : QLD_ACC_FP32);
+        acc = (all_rational && max_den <= 16 && bins_rows(&rows, true) && bins_fit(true)) ? QLD_ACC_INT_REFS : (tc_ok ? QLD_ACC_FIXED : QLD_ACC_FP32);
     }
-    if (acc == QLD_ACC_INT_BINS) {
+    const bool want_compact = acc == QLD_ACC_INT_REFS;
+    if (acc == QLD_ACC_INT_BINS || acc == QLD_ACC_INT_REFS) {
         if (!all_rational) return bad(QLD_E_UNSUPPORTED, "INT_BINS needs every reference rational (den > 0)");
-        if (!bins_rows(&rows)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
-        if (!bins_fit()) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
+        if (!bins_rows(&rows, want_compact)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
+        if (!bins_fit(want_compact)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
     }
     if (acc == QLD_ACC_FIXED && pl->ring) {
         if (cfg->K > 2) return bad(QLD_E_UNSUPPORTED, "FIXED on a ring: at most 2 references");
@@ -244,7 +251,7 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     }
     if ((pl->maps & QLD_MAP_SUMS_I64) && acc != QLD_ACC_FIXED) return bad(QLD_E_INVAL, "QLD_MAP_SUMS_I64 needs QLD_ACC_FIXED");
     pl->accum = acc;
-    pl->is_int = acc == QLD_ACC_INT_BINS;
+    pl->is_int = acc == QLD_ACC_INT_BINS || acc == QLD_ACC_INT_REFS;
     pl->is_fixed = acc == QLD_ACC_FIXED && !pl->ring;
     pl->fix_ring = acc == QLD_ACC_FIXED && pl->ring;
     FinParams &f = pl->fin;
@@ -254,8 +261,8 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         int off = 0;
         for (int k = 0; k < cfg->K; ++k) {
             RefPlan &rp = pl->ref[k];
-            rp.use_diff = rp.den % 2 == 0;
-            rp.n_rows = (int)(rp.use_diff ? rp.den / 2 : rp.den);
+            rp.use_diff = compact(k, want_compact) ? 2 : (rp.den % 2 == 0 ? 1 : 0);
+            rp.n_rows = rp.use_diff == 2 ? 2 : (int)(rp.use_diff ? rp.den / 2 : rp.den);
             rp.row_off = off;
             f.row_off[k] = off; f.n_rows[k] = rp.n_rows;
             off += rp.n_rows;                   // f.sw / f.cw are filled on the device by qld_create (k_bin_weights)
@@ -557,7 +564,7 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
     p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
     p.fin = fin_with_maps(c);
     p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
-    p.onehot = c->is_int && c->K == 1;
+    p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0) {
@@ -614,7 +621,7 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
         q.cum_lo = (int)(a_win % c->cap_w); q.cum_hi = (int)((a_win + c->N) % c->cap_w);
         q.wtab = c->wtab; q.cum = c->cum;
         q.acc_out = c->acc; q.acc_add = 1;
-        q.onehot = c->is_int && c->K == 1;
+        q.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
         q.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
         q.part_sub = 1;
         q.ped_in = c->is_int ? nullptr : c->ped;
@@ -634,7 +641,7 @@ int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool a
     p.cum_lo = (int)(a_win % c->cap_w); p.cum_hi = (int)((a_win + c->N) % c->cap_w);
     p.wtab = c->wtab; p.cum = c->cum;
     p.acc_out = c->acc; p.acc_add = add ? 1 : 0;
-    p.onehot = c->is_int && c->K == 1;
+    p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
     p.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
     p.part_sub = sub ? 1 : 0;
     if (!c->is_int) {
@@ -717,7 +724,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         q.cum_lo = (int)(a_new % c->cap_w); q.cum_hi = (int)((a_new + c->N) % c->cap_w);
         q.wtab = c->wtab; q.cum = c->cum;
         q.acc_out = c->acc; q.acc_add = 1;
-        q.onehot = c->is_int && c->K == 1;
+        q.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
         q.ped_in = c->is_int ? nullptr : c->ped;
         q.fin = fin_with_maps(c);
         int n = add_runs(c, q.run, 0, a_old, hop, -1);
@@ -737,7 +744,7 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
         p.wtab = c->wtab; p.cum = c->cum;
         p.acc_out = c->acc; p.acc_add = 1;
-        p.onehot = c->is_int && c->K == 1;
+        p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
         p.ped_in = c->is_int ? nullptr : c->ped;
         p.fin = fin_with_maps(c);
         int n = add_runs(c, p.run, 0, a_old, hop, -1);            // expired: frames a_old+1 .. a_old+hop

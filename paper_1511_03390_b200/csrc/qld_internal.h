@@ -16,7 +16,8 @@ struct RefPlan {
     int64_t num, den;
     int32_t phase_quarter;
     int32_t row_off, n_rows;
-    int32_t use_diff;  // even den: rows are B_r - B_{r+den/2}
+    int32_t use_diff;  // 1: even den, rows are B_r - B_{r+den/2};  0: rows are the bins B_r;  2: integer-valued scaled references
+                       // (den = 3 or 6, no phase): row 0 = sum x * (2/sqrt3) sin theta_s, row 1 = sum x * 2 cos theta_s, weights in 0, +-1, +-2
 };
 
 // Epilogue (A4) parameters, passed by value to the kernels.

@@ -38,8 +38,16 @@ __global__ void k_table_fill(const TableFillParams p)
             const int64_t r = bin_of(rf, s);
             int *w = static_cast<int *>(p.wtab) + e * p.rows + rf.row_off;
             const int64_t half = rf.den / 2;
-            for (int rr = 0; rr < rf.n_rows; ++rr)
-                w[rr] = rf.use_diff ? ((r == rr) - (r == rr + half)) : (r == rr);
+            if (rf.use_diff == 2) {
+                // theta = 2 pi r / den with den = 3 or 6: (2/sqrt3) sin theta and 2 cos theta are the integers below (sixths of a turn)
+                const int wi6[6] = {0, 1, 1, 0, -1, -1}, wq6[6] = {2, 1, -1, -2, -1, 1};
+                const int j = (int)(rf.den == 6 ? r : 2 * r);
+                w[0] = wi6[j];
+                w[1] = wq6[j];
+            } else {
+                for (int rr = 0; rr < rf.n_rows; ++rr)
+                    w[rr] = rf.use_diff ? ((r == rr) - (r == rr + half)) : (r == rr);
+            }
         }
     }
     __syncthreads();
@@ -73,6 +81,12 @@ __global__ void k_bin_weights(const TableFillParams p, double *out)
         const RefPlan &rf = p.ref[k];
         const int r = t - rf.row_off;
         if (r < 0 || r >= rf.n_rows) continue;
+        if (rf.use_diff == 2) {
+            // scaled integer references: I = (sqrt3 / 2) * row 0, Q = (1/2) * row 1
+            out[t] = r == 0 ? 0.5 * sqrt(3.0) : 0.0;
+            out[QLD_MAX_ROWS + t] = r == 1 ? 0.5 : 0.0;
+            continue;
+        }
         const int64_t D = 4 * rf.den;
         const int64_t a = (4 * (int64_t)r + (int64_t)(rf.phase_quarter & 3) * rf.den) % D;
         double sn, cs;

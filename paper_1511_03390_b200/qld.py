@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(_PKG, "libqld.so")
 
 QLD_U8, QLD_U16, QLD_U16_BE = 0, 1, 2
 QLD_OK, QLD_E_INVAL, QLD_E_NOMEM, QLD_E_CUDA, QLD_E_STATE, QLD_E_OVERRUN, QLD_E_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
-QLD_ACC_AUTO, QLD_ACC_FP32, QLD_ACC_INT_BINS, QLD_ACC_FIXED = 0, 1, 2, 3
+QLD_ACC_AUTO, QLD_ACC_FP32, QLD_ACC_INT_BINS, QLD_ACC_FIXED, QLD_ACC_INT_REFS = 0, 1, 2, 3, 4
 QLD_NORM_PAPER, QLD_NORM_AMPLITUDE = 0, 1
 QLD_WHOLE, QLD_SLIDE = 0, 1
 QLD_MAP_I, QLD_MAP_Q, QLD_MAP_AMP, QLD_MAP_PHASE, QLD_MAP_ALL, QLD_MAP_SUMS_I64 = 1, 2, 4, 8, 15, 16
@@ -293,7 +293,7 @@ class QLD:
         return int(self.lib.qld_accum_mode(self._ctx))
 
     def accum_name(self) -> str:
-        return {QLD_ACC_FP32: "FP32", QLD_ACC_INT_BINS: "INT_BINS", QLD_ACC_FIXED: "FIXED"}[self.accum_mode()]
+        return {QLD_ACC_FP32: "FP32", QLD_ACC_INT_BINS: "INT_BINS", QLD_ACC_FIXED: "FIXED", QLD_ACC_INT_REFS: "INT_REFS"}[self.accum_mode()]
 
     def debug_set_tile(self, which, a: int = 0, b: int = 0, c: int = 0) -> None:
         """qld_debug_set_tile: which = "stream" (SEG, KC), "tc" (T, STAGES, KC) or "slide" (1 = always k_slide_bulk, 2 = never)."""

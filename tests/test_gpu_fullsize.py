@@ -4,7 +4,7 @@ the strongest modulation -- are recomputed one by one by the oracle from the see
 import numpy as np
 import pytest
 
-from _parity import check_float_maps
+from _parity import check_float_maps, expected_int_rows
 
 pytestmark = pytest.mark.gpu
 
@@ -66,12 +66,11 @@ def test_whole_window_full_size_sampled(Q, oracle, name, accum_name, kernel):
         assert np.array_equal(got_bytes.reshape(x.shape), x)
         got = _gpu_on_pixels(ctx, k, pix)
         # the floor of the tolerance is the median amplitude of the sampled pixels (background-dominated, as the map's)
-        check_float_maps(got, ora, rel=1e-6 if mode in ("INT_BINS", "FIXED") else 1e-5, what=f"{name} {mode} k={k}")
-        if mode == "INT_BINS" and k == 0:
-            den = refs[0]["den"]
-            B = oracle.bins(x, refs[0]["num"], den)
-            rows = ctx.get_bins(0).reshape(den // 2, -1)[:, torch.from_numpy(pix).cuda()].cpu().numpy()
-            assert np.array_equal(rows.reshape(den // 2, 1, -1), B[:den // 2] - B[den // 2:])
+        check_float_maps(got, ora, rel=1e-6 if mode in ("INT_BINS", "INT_REFS", "FIXED") else 1e-5, what=f"{name} {mode} k={k}")
+        if mode in ("INT_BINS", "INT_REFS") and k == 0:
+            exp = expected_int_rows(oracle, x, refs[0], 1, mode)
+            rows = ctx.get_bins(0).reshape(exp.shape[0], -1)[:, torch.from_numpy(pix).cuda()].cpu().numpy()
+            assert np.array_equal(rows.reshape(exp.shape), exp)
     ctx.destroy()
     del frames
     torch.cuda.empty_cache()
@@ -109,11 +108,11 @@ def test_sliding_full_size_sampled(Q, oracle, accum_name, slide_hop):
             ctx.sync()
             x, ora = _oracle_on_pixels(oracle, sc, pix, ref, w * hop + 1, N)
             got = _gpu_on_pixels(ctx, 0, pix)
-            check_float_maps(got, ora, rel=1e-6 if ctx.accum_name() == "INT_BINS" else 1e-5, what=f"cfg3 window {w}")
-            if ctx.accum_name() == "INT_BINS":
-                B = oracle.bins(x, 1, 6, s_first=w * hop + 1)
-                rows = ctx.get_bins(0).reshape(3, -1)[:, torch.from_numpy(pix).cuda()].cpu().numpy()
-                assert np.array_equal(rows.reshape(3, 1, -1), B[:3] - B[3:]), f"window {w}"
+            check_float_maps(got, ora, rel=1e-6 if ctx.accum_name() in ("INT_BINS", "INT_REFS") else 1e-5, what=f"cfg3 window {w}")
+            if ctx.accum_name() in ("INT_BINS", "INT_REFS"):
+                exp = expected_int_rows(oracle, x, ref, w * hop + 1, ctx.accum_name())
+                rows = ctx.get_bins(0).reshape(exp.shape[0], -1)[:, torch.from_numpy(pix).cuda()].cpu().numpy()
+                assert np.array_equal(rows.reshape(exp.shape), exp), f"window {w}"
     ctx.destroy()
 
 
@@ -142,10 +141,8 @@ def test_whole_window_full_maps(Q, oracle, name, rows):
         ora = oracle.qld(x, refs[k], nthreads=nt)
         got = tuple(m[:rows].cpu().numpy() for m in ctx.get_maps(k))
         check_float_maps(got, ora, rel=1e-5 if mode == "FP32" else 1e-6, what=f"{name} {mode} full maps k={k}")
-    if mode == "INT_BINS":
-        den = refs[0]["den"]
-        B = oracle.bins(x, refs[0]["num"], den)
-        assert np.array_equal(ctx.get_bins(0).cpu().numpy(), B[:den // 2] - B[den // 2:])
+    if mode in ("INT_BINS", "INT_REFS"):
+        assert np.array_equal(ctx.get_bins(0).cpu().numpy(), expected_int_rows(oracle, x, refs[0], 1, mode))
     ctx.destroy()
     del frames
     torch.cuda.empty_cache()
@@ -188,7 +185,8 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
         if (i + 1) * batch >= N:
             ctx.demod(Q.QLD_SLIDE, hop)
             if is_int is None:
-                is_int = ctx.accum_name() == "INT_BINS"
+                is_int = ctx.accum_name() in ("INT_BINS", "INT_REFS")
+                int_mode = ctx.accum_name()
             if is_fix is None:
                 is_fix = ctx.accum_name() == "FIXED"
             if w in full_windows or w % tile_every == 0:
@@ -225,9 +223,7 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
             oI, oQ = oracle.demod_int(tile[a:a + N], gs.astype(np.int64), gc.astype(np.int64), nthreads=nt)
             assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"exact sums of window {ww}"
         if is_int:
-            B = oracle.bins(x, ref["num"], ref["den"], s_first=a + 1)
-            h = ref["den"] // 2
-            assert np.array_equal(keep[ww][4], B[:h] - B[h:]), f"bins of window {ww}"
+            assert np.array_equal(keep[ww][4], expected_int_rows(oracle, x, ref, a + 1, int_mode)), f"integer rows of window {ww}"
     if curve_path:
         import os
         os.makedirs(os.path.dirname(curve_path), exist_ok=True)

@@ -6,7 +6,7 @@ map median).  Every call goes through paper_1511_03390_b2
 import numpy as np
 import pytest
 
-from _parity import check_float_maps, forced, oracle_maps
+from _parity import check_float_maps, expected_int_rows, forced, oracle_maps
 
 pytestmark = pytest.mark.gpu
 
@@ -717,4 +717,58 @@ def test_window_relative_maps(Q, oracle, path, accum_name, refs):
     ctx.demod(Q.QLD_WHOLE)
     ctx.sync()
     check_float_maps(_maps(ctx, 0), oracle_maps(oracle, stream[T - N:T], refs[0], s_first=1), rel=1e-6 if accum_name == "INT_BINS" else 1e-5, what="whole on ring")
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ INT_REFS: two integer sums per reference
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("path", ["whole_small", "whole_stream", "whole_tc", "slide_small", "slide_bulk", "slide_partial"])
+@pytest.mark.parametrize("dtype", ["u8", "u16"])
+@pytest.mark.parametrize("refs", [[{"num": 1, "den": 6}], [{"num": 1, "den": 3}], [{"num": 1, "den": 6}, {"num": 1, "den": 4}], [{"num": 1, "den": 6, "phase": 0.3}]])
+def test_integer_reference_rows(Q, oracle, path, dtype, refs):
+    """QLD_ACC_INT_REFS (and AUTO): den = 3 or 6 without a phase offset is carried by two exact int32 sums (weights 0, +-1, +-2)
+    instead of three bin rows; other references of the context keep their bins (a reference with a phase offset falls back to
+    bins too).  Rows bit-exact against the integer oracle, maps to 1e-6, through every kernel that takes integer weights."""
+    rng = np.random.default_rng(len(path) + len(refs))
+    H, W, N, hop = 16, 128, 96, 32
+    npdt = np.uint8 if dtype == "u8" else np.uint16
+    hi = 256 if dtype == "u8" else 65536
+    x = rng.integers(0, hi, size=(N + 4 * hop, H, W)).astype(npdt)
+    kw = dict(accum=Q.QLD_ACC_AUTO, max_value=hi - 1)
+    if path == "whole_stream":
+        kw["debug_tile"] = ("stream", 512, 16)
+    if path == "whole_tc":
+        kw["debug_tile"] = ("tc", 4, 5, 64)
+    ring = path.startswith("slide")
+    if ring:
+        kw["ring_frames"] = N + 2 * hop + 3
+    if path == "slide_partial":
+        kw["slide_hop"] = hop
+        kw["debug_tile"] = ("stream", 512, 16)
+    ctx = Q.QLD(H, W, dtype, N, refs, **kw)
+    assert ctx.accum_name() == "INT_REFS"
+    if path in ("slide_bulk", "slide_partial"):
+        ctx.debug_set_tile("slide", 1)
+    ctx.push_frames(x[:N])
+    n_win = 5 if ring else 1
+    for w in range(n_win):
+        if ring:
+            if w > 0:
+                ctx.push_frames(x[N + (w - 1) * hop:N + w * hop])
+            ctx.demod(Q.QLD_SLIDE, hop)
+        else:
+            ctx.demod(Q.QLD_WHOLE)
+        ctx.sync()
+        a = w * hop
+        for k, ref in enumerate(refs):
+            exp = expected_int_rows(oracle, x[a:a + N], ref, a + 1, "INT_REFS")
+            got = ctx.get_bins(k).cpu().numpy()
+            compact = ref["den"] in (3, 6) and not ref.get("phase")
+            assert got.shape[0] == (2 if compact else (ref["den"] // 2 if ref["den"] % 2 == 0 else ref["den"]))
+            assert np.array_equal(got, exp), f"{path} window {w} k={k}"
+            check_float_maps(_maps(ctx, k), oracle_maps(oracle, x[a:a + N], ref, s_first=a + 1), rel=1e-6, what=f"{path} window {w} k={k}")
+    if path == "whole_tc":
+        assert ctx.last_kernel() == "k_demod_tc"
+    if path in ("slide_bulk", "slide_partial"):
+        assert ctx.last_kernel() == "k_slide_bulk"
     ctx.destroy()

@@ -185,6 +185,30 @@ def test_bins_brute_force_and_recombination(oracle):
 
 
 # ---------------------------------------------------------------- structure: axes, linearity, invariances
+def test_sixth_period_integer_references(oracle):
+    """nu = 1/6 (BASELINE.json configs[3]) and nu = 1/3: (2/sqrt3) sin theta_s and 2 cos theta_s are integers, so two exact sums
+    carry the whole result: 2Q = 2B0 + B1 - B2 - 2B3 - B4 + B5 and (2/sqrt3) I = B1 + B2 - B4 - B5 in terms of
+    the phase bins -- brute force in Python integers, and against the float definition."""
+    rng = np.random.default_rng(6)
+    N = 61
+    x = rng.integers(0, 65536, size=(N, 7)).astype(np.uint16)
+    for den, s_first in ((6, 1), (6, 1000), (3, 5)):
+        sn, cs = oracle.ref_tables(_ref(num=1, den=den), s_first, N)
+        wi, wq = np.rint(sn * 2 / math.sqrt(3)).astype(np.int64), np.rint(cs * 2).astype(np.int64)
+        assert np.abs(wi - sn * 2 / math.sqrt(3)).max() < 1e-15 and np.abs(wq - cs * 2).max() < 1e-15
+        assert set(wi.tolist()) <= {-1, 0, 1} and set(np.abs(wq).tolist()) <= {1, 2}
+        I2, Q2 = oracle.demod_int(x, wi, wq)
+        for p in range(x.shape[1]):                                    # brute force, Python integers
+            assert int(I2[p]) == sum(int(x[i, p]) * int(wi[i]) for i in range(N))
+            assert int(Q2[p]) == sum(int(x[i, p]) * int(wq[i]) for i in range(N))
+        B = oracle.bins(x, 1, den, s_first=s_first).astype(np.int64)
+        if den == 6:
+            assert np.array_equal(Q2, 2 * B[0] + B[1] - B[2] - 2 * B[3] - B[4] + B[5])
+            assert np.array_equal(I2, B[1] + B[2] - B[4] - B[5])
+        I, Q, _, _ = oracle.qld(x, _ref(num=1, den=den), s_first=s_first)
+        assert np.allclose(I, I2 * (math.sqrt(3) / 2), rtol=1e-13, atol=1e-6) and np.allclose(Q, Q2 / 2, rtol=1e-13, atol=1e-6)
+
+
 def test_pixel_axis_not_transposed(oracle):
     """Pixel p carries amplitude p+1 at its own phase; R[p] = (p+1) N/2.  A frame/pixel transposition or a
     wrong stride breaks this."""
