@@ -772,3 +772,44 @@ def test_integer_reference_rows(Q, oracle, path, dtype, refs):
     if path in ("slide_bulk", "slide_partial"):
         assert ctx.last_kernel() == "k_slide_bulk"
     ctx.destroy()
+
+
+@pytest.mark.timeout(300, method="thread")
+def test_concurrent_contexts_on_separate_streams(Q, oracle):
+    """Three contexts on three streams at once -- two sliding rings (dependent launches of k_slide_bulk that start while the
+    previous hop drains) and one whole-window tensor-core context -- interleaved for 40 hops: no launch may wait for SMs that a
+    waiting launch holds, and every result equals the oracle's."""
+    import torch
+    rng = np.random.default_rng(77)
+    H, W, N, hop, n_hops = 64, 512, 128, 32, 40
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    data = [rng.integers(0, 4096, size=(N + n_hops * hop, H, W)).astype(np.uint16) for _ in range(2)]
+    refs = [{"num": 1, "den": 6}, {"nu": 0.0937, "phase": 0.3}]
+    rings = []
+    for i in range(2):
+        with torch.cuda.stream(streams[i]):
+            ctx = Q.QLD(H, W, "u16", N, [refs[i]], ring_frames=N + 3 * hop, max_value=4095, slide_hop=hop if i == 0 else 0,
+                        debug_tile=("stream", 2048, 16) if i == 0 else None)
+        ctx.debug_set_tile("slide", 1)
+        ctx.push_frames(data[i][:N])
+        ctx.demod(Q.QLD_SLIDE, hop)
+        rings.append(ctx)
+    xw = rng.integers(0, 65536, size=(256, H, W)).astype(np.uint16)
+    with torch.cuda.stream(streams[2]):
+        whole = Q.QLD(H, W, "u16", 256, [{"nu": 0.05 + 0.05 * k} for k in range(8)], maps=Q.QLD_MAP_AMP)
+    whole.push_frames(xw)
+    for w in range(1, n_hops + 1):
+        for i in range(2):
+            rings[i].push_frames(data[i][N + (w - 1) * hop:N + w * hop])
+            rings[i].demod(Q.QLD_SLIDE, hop)
+        whole.demod(Q.QLD_WHOLE)
+    for c in rings + [whole]:
+        c.sync()
+    a = n_hops * hop
+    for i in range(2):
+        assert rings[i].last_kernel() == "k_slide_bulk"
+        check_float_maps(_maps(rings[i]), oracle_maps(oracle, data[i][a:a + N], refs[i], s_first=a + 1), rel=1e-6 if i == 0 else 1e-5, what=f"ring {i}")
+    amp = whole.get_maps(7)[2].cpu().numpy()
+    check_float_maps((None, None, amp, None), oracle_maps(oracle, xw, {"nu": 0.4}), rel=1e-6, what="whole")
+    for c in rings + [whole]:
+        c.destroy()
