@@ -79,7 +79,7 @@ typedef enum {
  *             with float references and no drift at all, at any nu; the table entry of a frame is a function of its
  *             absolute index and is extended per push.
  *  AUTO     : INT_REFS (= INT_BINS, compact where possible) when every reference is rational with den <= 16 and the bound holds; else FIXED for
- *             K >= 4 references on a whole-window store that meets FIXED's conditions (the CUDA-core kernel is
+ *             K >= 2 references on a whole-window store that meets FIXED's conditions (the CUDA-core kernel is
  *             instruction-bound there, the contraction is HBM-bound and more accurate than fp32); else FP32. */
 typedef enum { QLD_ACC_AUTO = 0, QLD_ACC_FP32 = 1, QLD_ACC_INT_BINS = 2, QLD_ACC_FIXED = 3, QLD_ACC_INT_REFS = 4 } qld_accum;
 

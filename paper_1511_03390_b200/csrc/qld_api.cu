@@ -226,10 +226,11 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     int acc = cfg->accum;
     int rows = 0;
     if (acc == QLD_ACC_AUTO) {
-        // bins when the references allow them (exact, cheapest); for K >= 4 float references on a whole-window
-        // store the CUDA-core kernel is instruction-issue bound (16+ FMA per sample) and the
-        // exact int8 contraction on the tensor cores is used; otherwise pedestal-subtracted fp32
-        const bool tc_ok = !pl->ring && cfg->K >= 4 && (pl->HW * pl->bytes) % 16 == 0 && cfg->N <= 65536 && !(cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64));
+        // bins when the references allow them (exact, cheapest); for K >= 2 float references on a whole-window
+        // store the CUDA-core kernel is instruction-issue bound (measured on the cfg2 stack: K = 2 5.8 TB/s, K = 3 3.6 TB/s
+        // against 6.2-6.4 TB/s for the contraction) and the exact int8 contraction on the tensor
+        // cores is used; otherwise (K = 1: the CUDA cores sit on the HBM roof) pedestal-subtracted fp32
+        const bool tc_ok = !pl->ring && cfg->K >= 2 && (pl->HW * pl->bytes) % 16 == 0 && cfg->N <= 65536 && !(cfg->maps & ~(QLD_MAP_ALL | QLD_MAP_SUMS_I64));
         acc = (all_rational && max_den <= 16 && bins_rows(&rows, true) && bins_fit(true)) ? QLD_ACC_INT_REFS : (tc_ok ? QLD_ACC_FIXED : QLD_ACC_FP32);
     }
     const bool want_compact = acc == QLD_ACC_INT_REFS;
