@@ -182,6 +182,11 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
             const int sb = it % NSB;
             const int64_t pix0 = (int64_t)tile * TP;
             const int npx = (int)min((int64_t)TP, p.HW - pix0);
+            // The first tile's frames do not depend on the launch before this one, its state does: when all of the tile's stages
+            // fit the (still empty) ring, the frames go in flight first and the dependency wait + state copies follow, so that
+            // the ramp-up of this launch overlaps the tail of the previous one (programmatic dependent launch).
+            const bool late_state = it == 0 && n_chunks <= STAGES;
+            auto issue_state = [&]() {
             if (lane == 0) {
                 SL_TRACE(1, it);
                 if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's sums are final from here on
@@ -198,6 +203,8 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                 }
                 if (IS_F32) bulk_load(st + SM.off_ped, p.ped_in + pix0, (uint32_t)(npx * 4), &state_full[sb]);
             }
+            };
+            if (!late_state) issue_state();
             for (int run = 0; run < p.n_runs; ++run) {
                 const int rn = p.run[run].n, rslot = p.run[run].slot0, rw0 = p.run[run].w0;
                 const WT sgn = (WT)p.run[run].sign;
@@ -244,6 +251,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                     if (++stage == STAGES) { stage = 0; phase ^= 1; }
                 }
             }
+            if (late_state) issue_state();
         }
         return;
     }
