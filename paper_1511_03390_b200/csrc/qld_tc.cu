@@ -606,14 +606,20 @@ TcShape tc_shape(int nc, int64_t row_bytes, int N, int n_sms, const int *force)
 {
     TcShape sh;
     const int n_sub = (int)((row_bytes + SUB_BYTES - 1) / SUB_BYTES);
-    // Measured on cfg2 (B200): the tensor pipe takes about 200 cycles to fetch one MN-major 8-bit A tile (128 bytes x
-    // 32 frames) from shared memory whatever N is, i.e. about 21 B/clk/SM = 6.1 TB/s over 148 SMs -- that, not HBM,
-    // bounds this kernel.  64-frame stages (two MMAs per span per barrier round trip) and 1 KB of contiguous
-    // bytes per frame were the best point of the sweep (T,stages,KC = 8,3,64: 6.17 TB/s; 16,3,32: 5.05; 4,6,64: 5.78).
-    int T = 512 / nc;                                               // one accumulator set may fill the TMEM (K = 8: T = 8)
-    if (T > 8) T = 8;
-    while (T & (T - 1)) --T;                                        // power of two
-    while (T > 1 && (n_sub + T - 1) / T < 2 * n_sms) T /= 2;      // small frames: keep every SM busy
+    // T spans (T * 128 contiguous bytes of every frame) per tile and 64-frame stages: on large frames 1 KB per frame (T = 8) is
+    // what DRAM serves best (6.2 TB/s against 5.6 for 512 B; the kernel is HBM-bound once the MMA warp issues warp-uniformly).
+    // On frames with only a few tiles per SM the last round of equal tiles leaves SMs idle, so T is the power of two that
+    // minimises rounds * (T + 1) -- the "+ 1" standing for the per-tile cost of ramp and epilogue -- larger T winning ties.
+    int Tmax = 512 / nc;                                            // one accumulator set may fill the TMEM (K = 8: T = 8)
+    if (Tmax > 8) Tmax = 8;
+    while (Tmax & (Tmax - 1)) --Tmax;                               // power of two
+    int T = Tmax;
+    long best = -1;
+    for (int t = Tmax; t >= 1; t /= 2) {
+        const long tiles = (n_sub + t - 1) / t, rounds = (tiles + n_sms - 1) / n_sms;
+        const long cost = rounds * (t + 1);
+        if (best < 0 || cost < best) { best = cost; T = t; }
+    }
     sh.T = T;
     sh.kc = 64;
     sh.stages = (225 * 1024) / TcSmem(nc, T, 1, sh.kc).off_bar;
@@ -657,6 +663,9 @@ cudaError_t launch_tc(const CUtensorMap *tmaps, const TcParams &p, int n_sms, cu
     const TcShape sh = tc_shape(NC, p.row_bytes, p.N, n_sms, force);
     // the shape of large frames (T = 8 spans = 1 KB of every frame, 64-frame stages) has its own instantiation
     if (sh.T == 8 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 8, 64, MODE>(tmaps, p, sh, n_sms, st);
+    if constexpr (MODE == 1) {                              // integer bins on mid-size frames (BASELINE.json configs[1]): T = 4 unrolled too
+        if (sh.T == 4 && sh.kc == 64) return launch_tc_shape<NC, BYTES, 4, 64, MODE>(tmaps, p, sh, n_sms, st);
+    }
     return launch_tc_shape<NC, BYTES, 0, 0, MODE>(tmaps, p, sh, n_sms, st);
 }
 
