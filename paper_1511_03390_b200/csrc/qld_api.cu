@@ -503,6 +503,35 @@ int stream_tmap_for(qld_ctx *c, const StreamShape &sh)
     return QLD_OK;
 }
 
+// The fields every launch over the ring / store shares: the store, the tables, the stored sums, the epilogue.  a_win = frames
+// before the window the launch finalises (for the pedestal sums of the fp32 mode).
+DemodParams base_params(const qld_ctx *c, int64_t a_win)
+{
+    DemodParams p;
+    memset(&p, 0, sizeof p);
+    p.big_endian = c->big_endian;
+    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
+    p.cap = c->cap; p.cap_w = c->cap_w;
+    p.cum_lo = (int)(a_win % c->cap_w); p.cum_hi = (int)((a_win + c->N) % c->cap_w);
+    p.wtab = c->wtab; p.cum = c->cum;
+    p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
+    p.fin = fin_with_maps(c);
+    return p;
+}
+
+// one k_demod_stream launch with the next pair of tile counters
+int launch_stream(qld_ctx *c, const DemodParams &p, const StreamShape &sh)
+{
+    int rc = stream_tmap_for(c, sh);
+    if (rc) return rc;
+    unsigned int *cur, *nxt;
+    next_counters(c, &cur, &nxt);
+    CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
+    c->launches++;
+    c->last_kernel = "k_demod_stream";
+    return QLD_OK;
+}
+
 // whole-window kernel over absolute frames a+1 .. a+N; seeds the sliding accumulators when asked
 int run_whole_tc(qld_ctx *c)
 {
@@ -553,34 +582,20 @@ int run_whole(qld_ctx *c, int64_t a, bool seed)
         const StreamShape big = qld_stream_shape(c->dtype, 1, c->rows_pad, c->HW, c->frames, c->n_sms, 0, 0);
         if (c->dbg_tc[0] > 0 || (big.seg > 0 && c->dbg_stream[0] == 0)) return run_whole_tc_bins(c);
     }
-    DemodParams p;
-    memset(&p, 0, sizeof p);
-    p.big_endian = c->big_endian;
-    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
-    p.cap = c->cap; p.slot0 = (int)(a % c->cap); p.n = c->N;
-    p.cap_w = c->cap_w; p.w0 = (int)((a + 1) % c->cap_w);
-    p.cum_lo = (int)(a % c->cap_w); p.cum_hi = (int)((a + c->N) % c->cap_w);
-    p.wtab = c->wtab; p.cum = c->cum;
+    DemodParams p = base_params(c, a);
+    p.slot0 = (int)(a % c->cap); p.n = c->N;
+    p.w0 = (int)((a + 1) % c->cap_w);
     p.acc_out = (seed || c->is_int) ? c->acc : nullptr;
     p.ped_out = (seed && !c->is_int) ? c->ped : nullptr;
-    p.fin = fin_with_maps(c);
     p.n_runs = add_runs(c, p.run, 0, a, c->N, +1);
-    p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
     // large, 16-byte-aligned frames: the TMA-fed persistent kernel; otherwise the register-staged one
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0) {
-        int rc = stream_tmap_for(c, sh);
-        if (rc) return rc;
-        {
-            unsigned int *cur, *nxt;
-            next_counters(c, &cur, &nxt);
-            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
-        }
-        c->last_kernel = "k_demod_stream";
-    } else {
-        CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
-        c->last_kernel = "k_demod_whole";
+        const int rc = launch_stream(c, p, sh);
+        return rc ? rc : record_demod(c, a + 1);
     }
+    CU(c, qld_launch_demod_whole(c->dtype, c->is_int, c->rows_pad, p, c->s_comp));
+    c->last_kernel = "k_demod_whole";
     c->launches++;
     return record_demod(c, a + 1);
 }
@@ -613,53 +628,24 @@ int try_slide_bulk(qld_ctx *c, const DemodParams &p)
 // expired batch: taken off the accumulators, then overwritten).
 int run_partial_batch(qld_ctx *c, int64_t a_win, int64_t first, int slot, bool add, bool sub, bool first_of_seed)
 {
+    DemodParams p = base_params(c, a_win);
+    p.acc_out = c->acc; p.acc_add = add ? 1 : 0;
+    p.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
+    p.part_sub = sub ? 1 : 0;
+    p.n_runs = add_runs(c, p.run, 0, first, c->slide_hop, +1);
     if (add && sub) {                                       // steady state: every byte through the copy engines
-        DemodParams q;
-        memset(&q, 0, sizeof q);
-        q.big_endian = c->big_endian;
-        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
-        q.cap = c->cap; q.cap_w = c->cap_w;
-        q.cum_lo = (int)(a_win % c->cap_w); q.cum_hi = (int)((a_win + c->N) % c->cap_w);
-        q.wtab = c->wtab; q.cum = c->cum;
-        q.acc_out = c->acc; q.acc_add = 1;
-        q.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
-        q.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
-        q.part_sub = 1;
+        DemodParams q = p;
         q.ped_in = c->is_int ? nullptr : c->ped;
-        q.fin = fin_with_maps(c);
-        q.n_runs = add_runs(c, q.run, 0, first, c->slide_hop, +1);
         const int rc = try_slide_bulk(c, q);
         if (rc != 0) return rc < 0 ? rc : QLD_OK;
     }
     if (c->fix_ring) return fail(c, QLD_E_UNSUPPORTED, "FIXED on a ring: the state of a tile does not fit the bulk-copy kernel's shared memory");
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg == 0 || c->slide_hop < sh.kc) return fail(c, QLD_E_UNSUPPORTED, "slide_hop: frames too small / hop too short for the TMA kernel");
-    DemodParams p;
-    memset(&p, 0, sizeof p);
-    p.big_endian = c->big_endian;
-    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
-    p.cap = c->cap; p.cap_w = c->cap_w;
-    p.cum_lo = (int)(a_win % c->cap_w); p.cum_hi = (int)((a_win + c->N) % c->cap_w);
-    p.wtab = c->wtab; p.cum = c->cum;
-    p.acc_out = c->acc; p.acc_add = add ? 1 : 0;
-    p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
-    p.part = c->part + (size_t)slot * c->rows_pad * c->HW * (c->is_int ? 4 : 8);
-    p.part_sub = sub ? 1 : 0;
     if (!c->is_int) {
         if (first_of_seed) p.ped_out = c->ped; else p.ped_in = c->ped;
     }
-    p.fin = fin_with_maps(c);
-    p.n_runs = add_runs(c, p.run, 0, first, c->slide_hop, +1);
-    int rc = stream_tmap_for(c, sh);
-    if (rc) return rc;
-    {
-            unsigned int *cur, *nxt;
-            next_counters(c, &cur, &nxt);
-            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
-        }
-    c->launches++;
-    c->last_kernel = "k_demod_stream";
-    return QLD_OK;
+    return launch_stream(c, p, sh);
 }
 
 // window a+1 .. a+N from scratch: the sums, and (block-partial mode) the N/hop per-batch partials
@@ -672,14 +658,8 @@ int seed_fix_ring(qld_ctx *c, int64_t a)
     if (c->slide_hop > 0) CU(c, cudaMemsetAsync(c->part, 0, rowset * c->n_part, c->s_comp));
     const int n_launch = c->slide_hop > 0 ? c->n_part : 1;
     for (int b = 0; b < n_launch; ++b) {
-        DemodParams q;
-        memset(&q, 0, sizeof q);
-        q.big_endian = c->big_endian;
-        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
-        q.cap = c->cap; q.cap_w = c->cap_w;
-        q.wtab = c->wtab; q.cum = c->cum;
+        DemodParams q = base_params(c, a);
         q.acc_out = c->acc; q.acc_add = 1;
-        q.fin = fin_with_maps(c);
         if (c->slide_hop > 0) {
             q.part = c->part + (size_t)b * rowset;
             q.part_sub = 1;
@@ -715,52 +695,24 @@ int run_slide(qld_ctx *c, int64_t a_old, int hop)
         if (rc) return rc;
         return record_demod(c, a_old + 1);                    // conservative: the whole window stays protected from overwriting
     }
+    // {expired, -w} + {new, +w} added to the stored sums
+    DemodParams q = base_params(c, a_new);
+    q.acc_out = c->acc; q.acc_add = 1;
+    q.ped_in = c->is_int ? nullptr : c->ped;
     {
-        // {expired, -w} + {new, +w} added to the stored sums: k_slide_bulk when the frames are large enough
-        DemodParams q;
-        memset(&q, 0, sizeof q);
-        q.big_endian = c->big_endian;
-        q.frames = c->frames; q.frame_stride = c->HW * c->bytes; q.HW = c->HW;
-        q.cap = c->cap; q.cap_w = c->cap_w;
-        q.cum_lo = (int)(a_new % c->cap_w); q.cum_hi = (int)((a_new + c->N) % c->cap_w);
-        q.wtab = c->wtab; q.cum = c->cum;
-        q.acc_out = c->acc; q.acc_add = 1;
-        q.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
-        q.ped_in = c->is_int ? nullptr : c->ped;
-        q.fin = fin_with_maps(c);
-        int n = add_runs(c, q.run, 0, a_old, hop, -1);
-        q.n_runs = add_runs(c, q.run, n, a_old + c->N, hop, +1);
-        const int rc = try_slide_bulk(c, q);
+        const int n = add_runs(c, q.run, 0, a_old, hop, -1);        // expired: frames a_old+1 .. a_old+hop
+        q.n_runs = add_runs(c, q.run, n, a_old + c->N, hop, +1);   // new: frames a_old+N+1 .. a_old+N+hop
+    }
+    {
+        const int rc = try_slide_bulk(c, q);                       // k_slide_bulk when the frames are large enough
         if (rc != 0) return rc < 0 ? rc : record_demod(c, a_old + 1);
         if (c->fix_ring) return fail(c, QLD_E_UNSUPPORTED, "FIXED on a ring: the state of a tile does not fit the bulk-copy kernel's shared memory");
     }
-    // large frames and hops of at least one pipeline stage: the TMA-fed kernel over {expired, -w} + {new, +w}
+    // smaller frames, hops of at least one pipeline stage: the TMA-fed whole-window kernel over the same run list
     const StreamShape sh = qld_stream_shape(c->dtype, c->is_int, c->rows_pad, c->HW, c->frames, c->n_sms, c->dbg_stream[0], c->dbg_stream[1]);
     if (sh.seg > 0 && hop >= sh.kc) {
-        DemodParams p;
-        memset(&p, 0, sizeof p);
-        p.big_endian = c->big_endian;
-    p.frames = c->frames; p.frame_stride = c->HW * c->bytes; p.HW = c->HW;
-        p.cap = c->cap; p.cap_w = c->cap_w;
-        p.cum_lo = (int)(a_new % c->cap_w); p.cum_hi = (int)((a_new + c->N) % c->cap_w);
-        p.wtab = c->wtab; p.cum = c->cum;
-        p.acc_out = c->acc; p.acc_add = 1;
-        p.onehot = c->is_int && c->K == 1 && c->ref[0].use_diff != 2;
-        p.ped_in = c->is_int ? nullptr : c->ped;
-        p.fin = fin_with_maps(c);
-        int n = add_runs(c, p.run, 0, a_old, hop, -1);            // expired: frames a_old+1 .. a_old+hop
-        n = add_runs(c, p.run, n, a_old + c->N, hop, +1);        // new: frames a_old+N+1 .. a_old+N+hop
-        p.n_runs = n;
-        int rc = stream_tmap_for(c, sh);
-        if (rc) return rc;
-        {
-            unsigned int *cur, *nxt;
-            next_counters(c, &cur, &nxt);
-            CU(c, qld_launch_demod_stream(c->dtype, c->is_int, c->rows_pad, c->stream_tmap, p, sh, cur, nxt, c->n_sms, c->s_comp));
-        }
-        c->launches++;
-        c->last_kernel = "k_demod_stream";
-        return record_demod(c, a_old + 1);
+        const int rc = launch_stream(c, q, sh);
+        return rc ? rc : record_demod(c, a_old + 1);
     }
     SlideParams p;
     memset(&p, 0, sizeof p);
