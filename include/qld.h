@@ -194,7 +194,11 @@ int qld_push_done(qld_ctx *ctx, int block);
  *             the window by hop frames (1 <= hop <= N; window w = frames w*hop+1 .. w*hop+N for constant
  *             hop, G10), adding the hop new frames and subtracting the hop expired ones.
  * References are indexed by absolute frame number in both modes.
- * QLD_E_STATE if the frames the window needs are not all pushed yet. */
+ * QLD_E_STATE if the frames the window needs are not all pushed yet.
+ * Consecutive sliding updates may overlap on the device (the next launch ramps up while the previous one drains; it touches the
+ * stored sums only once the previous launch is complete), so the maps of window w are defined for work ordered after THAT
+ * qld_demod on the compute stream (qld_read_map, a kernel of the caller's on the same stream) or after qld_sync -- not for a
+ * reader on an unrelated stream. */
 int qld_demod(qld_ctx *ctx, int mode, int hop);
 
 /* The processed images ("resulting in the 32-bit n x n processed image"; I and Q are the "two different 2-D arrays

@@ -11,11 +11,17 @@
 // R = sum_j d_j 256^j is split into four signed base-256 digits d_j in [-128, 127] (four N columns).  The MMA
 // produces P[byte][j] = sum_s byte_s * d_j(s) (|P| <= 255*128*N, exact in int32) and the epilogue recombines
 //     sum_s x_s R_s = sum_b sum_j 256^(b+j) P[b][j]     exactly in int64.
-// The kernel is HBM-bound for any K <= 8 (N columns = 8K <= 64): per 32-frame MMA step the tensor pipe needs
-// 128*N/256 <= 32 cycles for 4 KB of samples, about five times faster than HBM delivers them to one SM.
+// The kernel is HBM-bound for any K <= 8 (N columns = 8K <= 64): measured, an M = 128, N <= 128, K = 32 kind::i8 MMA retires in
+// about 40 ns (MN-major and K-major operands alike), i.e. 4 KB of samples per 40 ns per SM, twice what HBM delivers to one SM --
+// PROVIDED the MMA warp issues warp-uniformly (see the MMA issuer below).
+//
+// The same kernel runs two more contractions (template MODE): the integer phase bins of A3' (MODE 1: the bin indicators 0, +-1
+// are a one-digit B operand of 16 columns, the epilogue writes the exact int32 rows) and the unknown-frequency search (MODE 2:
+// 32 DFT bins = 256 columns per launch, arg-max in the epilogue; qld_spectrum.cu).
 //
 // Structure (one persistent CTA per SM, 320 threads): warp 0 = TMA producer, warp 1 = MMA issuer, warps 2-9 =
-// epilogue (TMEM -> registers -> maps; two quartets, each warp reads its own TMEM lane quarter).  A CTA tile is T adjacent 128-byte pixel spans over all frames.  When two
+// epilogue (TMEM -> registers -> maps; two quartets, each warp reads its own TMEM lane quarter).  A CTA tile is T adjacent
+// 128-byte pixel spans over all frames.  When two
 // tiles' accumulators fit the 512 TMEM columns (2 * T * NC <= 512) they are double buffered; otherwise (K = 8: NC = 64,
 // T = 8 -- 1 KB of contiguous bytes per frame, which DRAM serves measurably better than 512 B) there is one set and the
 // epilogue hands the columns back span by span: the MMA warp restarts span t of the next tile as soon as span t is
