@@ -229,9 +229,11 @@ int qld_read_ref_table(qld_ctx *ctx, int k, int64_t s_first, int n, float *sin_o
  * INT_BINS contexts).  Blocks until the device tables are rebuilt. */
 int qld_set_ref_tables(qld_ctx *ctx, int k, const double *sin_tab, const double *cos_tab, int64_t len);
 
-/* QLD_ACC_FIXED only.  Replace the Q1.30 reference table of reference k by caller-supplied integers (host
- * arrays of n == N entries, entry i belongs to frame i+1, each in [-2^30, 2^30]); blocks until the device
- * table is rebuilt.  qld_read_ref_table_fixed copies the table in use back to the host (blocks). */
+/* QLD_ACC_FIXED only.  Replace the Q1.30 reference table of reference k by caller-supplied integers (host arrays, each
+ * entry in [-2^30, 2^30]); blocks until the device table is rebuilt.  Whole-window store: n == N entries, entry i belongs to
+ * frame i+1.  Ring: the entries of the n most recently pushed frames (1 <= n <= frames pushed), to be called after the push
+ * that brought them and before the qld_demod that uses them.  qld_read_ref_table_fixed copies the table in use back to the
+ * host (blocks). */
 int qld_set_ref_table_fixed(qld_ctx *ctx, int k, const int32_t *sin_q30, const int32_t *cos_q30, int n);
 /* N entries each.  Whole-window store: frames 1..N.  Ring: the N most recently pushed frames. */
 int qld_read_ref_table_fixed(qld_ctx *ctx, int k, int32_t *sin_q30, int32_t *cos_q30);

@@ -1022,13 +1022,24 @@ int qld_set_ref_table_fixed(qld_ctx *c, int k, const int32_t *sin_q30, const int
 {
     if (!c || k < 0 || k >= c->K || !sin_q30 || !cos_q30) return c ? fail(c, QLD_E_INVAL, "set_ref_table_fixed: bad argument") : QLD_E_INVAL;
     if (c->sticky) return QLD_E_CUDA;
-    if (!c->is_fixed) return fail(c, QLD_E_STATE, "set_ref_table_fixed: context does not use QLD_ACC_FIXED");
-    if (n != c->N) return fail(c, QLD_E_INVAL, "set_ref_table_fixed: n must equal N");
+    if (!c->is_fixed && !c->fix_ring) return fail(c, QLD_E_STATE, "set_ref_table_fixed: context does not use QLD_ACC_FIXED");
+    if (c->fix_ring ? (n < 1 || n > c->pushed || n >= c->cap_w) : n != c->N)
+        return fail(c, QLD_E_INVAL, c->fix_ring ? "set_ref_table_fixed: n must be 1 .. frames pushed (and fit the table ring)" : "set_ref_table_fixed: n must equal N");
     for (int i = 0; i < n; ++i)
         if (sin_q30[i] > (1 << 30) || sin_q30[i] < -(1 << 30) || cos_q30[i] > (1 << 30) || cos_q30[i] < -(1 << 30))
             return fail(c, QLD_E_INVAL, "set_ref_table_fixed: entries must lie in [-2^30, 2^30]");
     int rc = qld_sync(c);
     if (rc) return rc;
+    if (c->fix_ring) {
+        // ring: the entries of the n most recently pushed frames (absolute indices pushed-n+1 .. pushed), in place in the table ring
+        int32_t *w = static_cast<int32_t *>(c->wtab);
+        for (int i = 0; i < n; ++i) {
+            const int64_t e = (c->pushed - n + 1 + i) % c->cap_w;
+            const int32_t pair[2] = {sin_q30[i], cos_q30[i]};
+            CU(c, cudaMemcpy(w + e * c->rows_pad + 2 * k, pair, sizeof pair, cudaMemcpyHostToDevice));
+        }
+        return QLD_OK;
+    }
     CU(c, cudaMemcpy(c->rfix + (size_t)(2 * k) * c->N, sin_q30, (size_t)n * 4, cudaMemcpyHostToDevice));
     CU(c, cudaMemcpy(c->rfix + (size_t)(2 * k + 1) * c->N, cos_q30, (size_t)n * 4, cudaMemcpyHostToDevice));
     CU(c, qld_launch_digit_pack(c->rfix, c->N, c->N, c->K, c->digits, c->s_comp));

@@ -172,6 +172,7 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
     keep = {}                                                     # window -> (I, Q, amp, phase[, bins]) on the host
     is_int = None
     is_fix, fix = None, {}
+    supply_fixed = accum == Q.QLD_ACC_FIXED
     nt = oracle.max_threads()
     w = 0
     for i in range(n_batches):
@@ -182,6 +183,9 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
         buf.copy_(dev)
         tile[i * batch:(i + 1) * batch] = buf[:, y0:y0 + 128, x0:x0 + 128].numpy()
         ctx.push_frames(buf)
+        if supply_fixed:                                              # exact-sum checks run on the ORACLE's Q1.30 integers
+            osn, ocs = oracle.ref_tables(ref, 1 + i * batch, batch)
+            ctx.set_ref_table_fixed(0, np.rint(osn * 2.0 ** 30).astype(np.int64), np.rint(ocs * 2.0 ** 30).astype(np.int64))
         if (i + 1) * batch >= N:
             ctx.demod(Q.QLD_SLIDE, hop)
             if is_int is None:
@@ -219,8 +223,9 @@ def _stream_cfg3(Q, oracle, ref, accum, slide_hop, resync_hops, full_windows, ti
         if is_fix:
             gs, gc, gI, gQ = fix[ww]
             osn, ocs = oracle.ref_tables(ref, a + 1, N)
-            assert np.abs(gs - np.rint(osn * 2.0 ** 30)).max() <= 1 and np.abs(gc - np.rint(ocs * 2.0 ** 30)).max() <= 1
-            oI, oQ = oracle.demod_int(tile[a:a + N], gs.astype(np.int64), gc.astype(np.int64), nthreads=nt)
+            os_, oc = np.rint(osn * 2.0 ** 30).astype(np.int64), np.rint(ocs * 2.0 ** 30).astype(np.int64)
+            assert np.array_equal(gs, os_) and np.array_equal(gc, oc)          # the table in use is the oracle's (supplied per batch)
+            oI, oQ = oracle.demod_int(tile[a:a + N], os_, oc, nthreads=nt)
             assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"exact sums of window {ww}"
         if is_int:
             assert np.array_equal(keep[ww][4], expected_int_rows(oracle, x, ref, a + 1, int_mode)), f"integer rows of window {ww}"

@@ -226,21 +226,34 @@ def test_fixed_point_sliding_is_exact(Q, oracle, dtype, H, W, hop, cap, partial,
     raw = x.byteswap() if dtype == "u16be" else x
     ctx = Q.QLD(H, W, dtype, N, refs, ring_frames=cap, accum=Q.QLD_ACC_FIXED, slide_hop=hop if partial else 0)
     assert ctx.accum_name() == "FIXED"
-    ctx.push_frames(raw[:N])
+    def q30(ref, s_first, n):                                          # the oracle's table, rounded to Q1.30
+        sn, cs = oracle.ref_tables(ref, s_first, n)
+        return np.rint(sn * 2.0 ** 30).astype(np.int64), np.rint(cs * 2.0 ** 30).astype(np.int64)
+
+    def push(first, n):
+        """push frames first+1 .. first+n; the library's own table entries must be the rounded oracle table (+-1 on rounding
+        ties); they are then replaced by the oracle's, so that the exact sums below are compared on the ORACLE's integers"""
+        ctx.push_frames(raw[first:first + n])
+        for k, ref in enumerate(refs):
+            os_, oc = q30(ref, first + 1, n)
+            if first + n >= N:
+                gs, gc = ctx.read_ref_table_fixed(k)                  # the N most recent entries
+                assert np.abs(gs[-n:] - os_).max() <= 1 and np.abs(gc[-n:] - oc).max() <= 1
+            ctx.set_ref_table_fixed(k, os_, oc)
+
+    push(0, N)
     ctx.demod(Q.QLD_SLIDE, hop)
     nt = oracle.max_threads()
     for w in range(0, (T - N) // hop + 1):
         if w > 0:
-            ctx.push_frames(raw[N + (w - 1) * hop:N + w * hop])
+            push(N + (w - 1) * hop, hop)
             ctx.demod(Q.QLD_SLIDE, hop)
         ctx.sync()
         assert ctx.last_kernel() == "k_slide_bulk"
         a = w * hop
         for k, ref in enumerate(refs):
-            gs, gc = ctx.read_ref_table_fixed(k)                       # entries of frames a+1 .. a+N
-            osn, ocs = oracle.ref_tables(ref, a + 1, N)
-            assert np.abs(gs - np.rint(osn * 2.0 ** 30)).max() <= 1 and np.abs(gc - np.rint(ocs * 2.0 ** 30)).max() <= 1
-            oI, oQ = oracle.demod_int(x[a:a + N], gs.astype(np.int64), gc.astype(np.int64), nthreads=nt)
+            os_, oc = q30(ref, a + 1, N)
+            oI, oQ = oracle.demod_int(x[a:a + N], os_, oc, nthreads=nt)
             gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(k)]
             assert np.array_equal(gI, oI) and np.array_equal(gQ, oQ), f"window {w} k={k}"
             check_float_maps(_maps(ctx, k), oracle_maps(oracle, x[a:a + N], ref, s_first=a + 1), rel=1e-6, what=f"window {w} k={k}")
