@@ -297,6 +297,31 @@ int qld_cnr(const float *map_device, int32_t H, int32_t W, int32_t y0, int32_t x
 int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_t H, int32_t W, int32_t N, int32_t q_lo, int32_t q_hi,
                      float *amp_max_device, int32_t *bin_device, void *stream);
 
+/* qld_dominant_bin for callers that cannot allocate device memory -- a camera loop that must not stall on the driver lock
+ * cudaMalloc / cudaFree take (the real-time threads), or a process whose HBM another allocator already holds in
+ * full.  Same search, same arguments, same results as the tensor-core route of qld_dominant_bin, but its scratch
+ * (the Q1.30 digit tiles of the bins, two tile counters) lives in one fixed array inside the library instead of pool memory;
+ * the call issues no cudaMalloc, cudaFree or other allocating routine.  The caller still owns and passes the inputs and outputs.
+ *   Limits: the digit tiles take 256 * (N rounded up to a multiple of 128) * ceil((q_hi - q_lo + 1) / 32) bytes (qld_dominant_bin_static_bytes
+ * computes it) and must fit QLD_SEARCH_STATIC_BYTES = 4 MiB -- e.g. all 511 bins of an N = 1024 window, or 128 bins of N = 4096;
+ * a larger search returns QLD_E_NOMEM (split the bin range over several calls and combine, or use qld_dominant_bin).  Only frames
+ * whose byte size is a multiple of 16 in a 16-byte aligned stack: QLD_E_UNSUPPORTED otherwise (the other route builds contexts).
+ * Every GPU on which this library's kernels are loaded holds the array (4 MiB + 256 B) until the process exits.
+ *   First call on a device: looks up the array's address on that device (the device must be current, as for every call
+ * here) and, if nothing ran from the library on it before, loads the kernels; make that call during set-up, before any
+ * stream capture begins.  Later calls on the device do no set-up.
+ *   Sharing: all calls on one device use the same array, which keeps the last call's contents; the entry point re-zeroes
+ * the counters and rewrites every digit it reads, so calls one after the other are independent.  Two calls whose GPU work
+ * overlaps (two host threads, two streams) race on it and give wrong maps: serialise them.  The call returns after the last
+ * pass has finished (it synchronises `stream` only).
+ *   Errors: QLD_E_INVAL as qld_dominant_bin, QLD_E_NOMEM / QLD_E_UNSUPPORTED as above, QLD_E_CUDA; the text of this thread's
+ * last failure is at qld_dominant_bin_static_error() ("" after a success; never NULL). */
+#define QLD_SEARCH_STATIC_BYTES (4 << 20)
+int qld_dominant_bin_static(const void *frames_device, int32_t dtype, int32_t H, int32_t W, int32_t N, int32_t q_lo, int32_t q_hi,
+                            float *amp_max_device, int32_t *bin_device, void *stream);
+int64_t qld_dominant_bin_static_bytes(int32_t N, int32_t q_lo, int32_t q_hi);   /* scratch bytes of that search; QLD_E_INVAL (< 0) for a bad range */
+const char *qld_dominant_bin_static_error(void);
+
 /* Display mapping (the processed 32-bit image "is displayed on the computer monitor"; there is no graphics stack
  * here, the 8-bit image is delivered to device memory; reading G22): lo / hi = smallest / largest non-NaN value
  * of the n floats at map_device, out_device[i] = rint(255 * (x_i - lo) / (hi - lo)) clamped to 0..255 (0 for NaN and

@@ -27,7 +27,8 @@ _STATUS = {0: "QLD_OK", -1: "QLD_E_INVAL", -2: "QLD_E_NOMEM", -3: "QLD_E_CUDA", 
 EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_frames_device", "qld_attach_frames_device",
            "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table", "qld_set_ref_tables",
            "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel", "qld_debug_set_tile",
-           "qld_cnr", "qld_dominant_bin", "qld_display_map", "qld_synth_fill"]
+           "qld_cnr", "qld_dominant_bin", "qld_dominant_bin_static", "qld_dominant_bin_static_bytes", "qld_dominant_bin_static_error",
+           "qld_display_map", "qld_synth_fill"]
 
 
 class qld_ref(C.Structure):
@@ -103,6 +104,11 @@ def load_library():
     l.qld_debug_set_tile.argtypes = [vp, i, i, i, i]
     l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
     l.qld_dominant_bin.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
+    l.qld_dominant_bin_static.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
+    l.qld_dominant_bin_static_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+    l.qld_dominant_bin_static_bytes.restype = C.c_int64
+    l.qld_dominant_bin_static_error.argtypes = []
+    l.qld_dominant_bin_static_error.restype = C.c_char_p
     l.qld_display_map.argtypes = [vp, C.c_int64, vp, vp, vp, vp]
     l.qld_synth_fill.argtypes = [C.POINTER(qld_synth_scene), i64, i, vp, vp]
     _lib = l
@@ -358,6 +364,33 @@ def dominant_bin(frames, q_lo: int, q_hi: int):
                               torch.cuda.current_stream(frames.device).cuda_stream or 1)
     if rc != QLD_OK:
         raise QLDError(rc, lib.qld_last_error(None).decode())
+    return amp, bins
+
+
+QLD_SEARCH_STATIC_BYTES = 4 << 20
+
+
+def dominant_bin_static(frames, q_lo: int, q_hi: int, amp=None, bins=None):
+    """qld_dominant_bin_static: the search of dominant_bin() without any device allocation inside the library, for callers
+    that cannot afford one (a live acquisition loop, a process whose HBM is already spoken for): the scratch is a fixed
+    4 MiB array in the library, so the search must fit it (QLDError with QLD_E_NOMEM otherwise) and the frames must be a
+    multiple of 16 bytes.  Pass preallocated `amp` [H, W] float32 and `bins` [H, W] int32 to keep this wrapper from
+    allocating too.  One search at a time per device: overlapping calls share the scratch and race."""
+    import torch
+    lib = load_library()
+    assert frames.is_cuda and frames.is_contiguous() and frames.dim() == 3
+    N, H, W = (int(x) for x in frames.shape)
+    dtype = QLD_U8 if frames.element_size() == 1 else QLD_U16
+    if amp is None:
+        amp = torch.empty((H, W), dtype=torch.float32, device=frames.device)
+    if bins is None:
+        bins = torch.empty((H, W), dtype=torch.int32, device=frames.device)
+    assert amp.is_contiguous() and bins.is_contiguous() and amp.dtype == torch.float32 and bins.dtype == torch.int32
+    with torch.cuda.device(frames.device):
+        rc = lib.qld_dominant_bin_static(frames.data_ptr(), dtype, H, W, N, int(q_lo), int(q_hi), amp.data_ptr(), bins.data_ptr(),
+                                         torch.cuda.current_stream(frames.device).cuda_stream or 1)
+    if rc != QLD_OK:
+        raise QLDError(rc, lib.qld_dominant_bin_static_error().decode())
     return amp, bins
 
 
