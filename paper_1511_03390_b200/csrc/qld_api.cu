@@ -474,6 +474,11 @@ int record_demod(qld_ctx *c, int64_t oldest_read)
 {
     DemodEvent &d = c->demod_ev[c->demod_ev_next];
     c->demod_ev_next = (c->demod_ev_next + 1) % N_DEMOD_EVENTS;
+    // Only the last N_DEMOD_EVENTS launches are remembered, and the host is never throttled: on a roomy ring it can be more
+    // launches than that ahead of the GPU.  A launch about to be forgotten may still be queued; what it reads (frames: wait_for_readers,
+    // table entries: the look-ahead in push_common) is protected only while it is remembered.  So the copy stream is held behind it
+    // before its slot is reused: nothing the copy stream is given from here on can overtake a launch older than the remembered ones.
+    if (d.used) CU(c, cudaStreamWaitEvent(c->s_copy, d.ev, 0));
     d.oldest_read = oldest_read; d.used = true;
     CU(c, cudaEventRecord(d.ev, c->s_comp));
     return QLD_OK;

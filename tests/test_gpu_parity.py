@@ -813,3 +813,52 @@ def test_concurrent_contexts_on_separate_streams(Q, oracle):
     check_float_maps((None, None, amp, None), oracle_maps(oracle, xw, {"nu": 0.4}), rel=1e-6, what="whole")
     for c in rings + [whole]:
         c.destroy()
+
+
+# ------------------------------------------------------------------------------------------------ host far ahead of the GPU
+@pytest.mark.timeout(300, method="thread")
+@pytest.mark.parametrize("mode", ["bins", "bins_partial", "bins_small", "fp32", "fp32_partial", "fixed", "fixed_partial"])
+@pytest.mark.parametrize("ring_hops", [50, 130])
+def test_many_hops_queued_behind_a_busy_gpu(Q, oracle, mode, ring_hops):
+    """120 hops are pushed and requested without a single host-side wait while the compute stream is held up, so every update
+    is still queued when the last push is issued -- far more than the 32 launches the context remembers.  Nothing the copy
+    stream does (frames that wrap around a 50-hop ring; table entries written ahead on the roomy 130-hop ring, whose table
+    ring wraps first) may overtake an update that still reads the old contents: the last window equals the oracle's direct
+    recomputation -- integer rows bit for bit; FIXED from the library's own tables (never supplied, never synchronised):
+    the table is the rounded oracle table up to rint ties, and the int64 sums are the oracle's within what those ties allow."""
+    import torch
+    H, W, N, hop, n_hops = 12, 128, 128, 32, 120
+    T = N + n_hops * hop
+    rng = np.random.default_rng(ring_hops + len(mode))
+    stream = _rand_stack(rng, T, H, W, np.uint16)
+    dev = torch.from_numpy(stream.view(np.int16)).cuda()
+    fixed, fp32 = mode.startswith("fixed"), mode.startswith("fp32")
+    ref = {"num": 1, "den": 6} if mode.startswith("bins") else {"nu": 0.0937, "phase": 0.3}
+    accum = Q.QLD_ACC_FIXED if fixed else Q.QLD_ACC_FP32 if fp32 else Q.QLD_ACC_INT_BINS
+    ctx = Q.QLD(H, W, "u16", N, [ref], ring_frames=N + ring_hops * hop, accum=accum, max_value=4095, resync_hops=-1,
+                slide_hop=hop if mode.endswith("partial") else 0, debug_tile=("stream", 512, 16) if mode.endswith("partial") else None)
+    ctx.debug_set_tile("slide", 2 if mode == "bins_small" else 1)
+    ctx.push_frames(dev[:N])
+    ctx.demod(Q.QLD_SLIDE, hop)
+    torch.cuda._sleep(400_000_000)                                  # ~0.2 s on the compute stream: everything below queues up behind it
+    for w in range(1, n_hops + 1):
+        ctx.push_frames(dev[N + (w - 1) * hop:N + w * hop])
+        ctx.demod(Q.QLD_SLIDE, hop)
+    assert ctx.counters() == (T, n_hops + 1)
+    ctx.sync()
+    assert (ctx.last_kernel() == "k_slide_bulk") == (mode != "bins_small")
+    a = n_hops * hop
+    last = stream[a:a + N]
+    check_float_maps(_maps(ctx), oracle_maps(oracle, last, ref, s_first=a + 1), rel=1e-5 if fp32 else 1e-6, what=mode)
+    if mode.startswith("bins"):
+        assert np.array_equal(ctx.get_bins(0).cpu().numpy(), expected_int_rows(oracle, last, ref, s_first=a + 1, mode=ctx.accum_name()))
+    if fixed:
+        sn, cs = oracle.ref_tables(ref, a + 1, N)
+        os_, oc = np.rint(sn * 2.0 ** 30).astype(np.int64), np.rint(cs * 2.0 ** 30).astype(np.int64)
+        gs, gc = ctx.read_ref_table_fixed(0)                        # the N most recent entries: this window's
+        assert np.abs(gs - os_).max() <= 1 and np.abs(gc - oc).max() <= 1
+        oI, oQ = oracle.demod_int(last, os_, oc, nthreads=oracle.max_threads())
+        gI, gQ = [t.cpu().numpy() for t in ctx.get_sums_i64(0)]
+        # each entry that differs (by one unit, on a rint tie) moves a sum by at most one sample value
+        assert np.abs(gI - oI).max() <= 4095 * int((gs != os_).sum()) and np.abs(gQ - oQ).max() <= 4095 * int((gc != oc).sum())
+    ctx.destroy()
