@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of libqld.so (product side only).
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <stdint.h>
 
 #include "qld.h"
@@ -119,4 +120,25 @@ inline int qld_sm_count()
     int &n = cached[dev & 63];
     if (n == 0 && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 1;
     return n > 0 ? n : 1;
+}
+
+// Lift a kernel's dynamic shared-memory limit to the device's opt-in maximum, once per (kernel instantiation, device);
+// `done` is the instantiation's own zero-initialised table.  Whoever writes the attribute writes the same value, so two host
+// threads that launch different tile shapes of one kernel at the same time (distinct contexts are independent across threads,
+// qld.h) cannot leave it below what a later launch needs -- which a cached "largest size set so far" could.
+template <typename Kernel>
+inline cudaError_t qld_allow_max_smem(Kernel kern, std::atomic<int> (&done)[64])
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < 64;
+    if (cached && done[dev].load(std::memory_order_acquire)) return cudaSuccess;
+    int optin = 0;
+    e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    if (e != cudaSuccess) return e;
+    if (cached) done[dev].store(1, std::memory_order_release);
+    return cudaSuccess;
 }

@@ -79,13 +79,6 @@ struct SlideSmem {
     }
 };
 
-#ifdef QLD_SL_TRACE   // development builds only: time stamps of CTA 0
-__device__ unsigned long long g_sl_trace[8 * 64];
-__device__ __forceinline__ unsigned long long sl_gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define SL_TRACE(kind, n) do { if (blockIdx.x == 0 && (n) < 64) g_sl_trace[(kind) * 64 + (n)] = sl_gtime(); } while (0)
-#else
-#define SL_TRACE(kind, n) do { } while (0)
-#endif
 
 template <typename T, typename ACC, int ROWS, bool PART>
 __global__ void __launch_bounds__(SL_THREADS, 1)
@@ -125,7 +118,6 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     for (int run = 0; run < p.n_runs; ++run) n_chunks += (p.run[run].n + KC - 1) / KC;
 
     if (threadIdx.x == 0) {
-        SL_TRACE(0, 0);
         if (blockIdx.x == 0) {
             *counter_next = 0;                    // the next launch's tile counter (three rotate: no memset between launches)
             __threadfence();
@@ -188,10 +180,8 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
             const bool late_state = it == 0 && n_chunks <= STAGES;
             auto issue_state = [&]() {
             if (lane == 0) {
-                SL_TRACE(1, it);
                 if (it == 0) asm volatile("griddepcontrol.wait;" ::: "memory");   // the previous launch's sums are final from here on
                 mbar_wait(&state_empty[sb], (uint32_t)((it / NSB) & 1) ^ 1u);
-                SL_TRACE(2, it);
                 unsigned char *st = sState + (size_t)sb * SM.state_bytes;
                 const uint32_t rb = (uint32_t)(npx * (int)sizeof(RED));
                 uint32_t bytes = (uint32_t)ROWS * rb * (PART ? 2u : 1u) + (IS_F32 ? (uint32_t)(npx * 4) : 0u);
@@ -286,7 +276,6 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                             bulk_store(map_ptr[w] + (int64_t)k * p.HW + pix0, st + SM.off_map + (size_t)(k * n_which + map_slot[w]) * TP * 4, (uint32_t)(npx * 4));
                 bulk_commit();
                 bulk_wait_read0();                         // the copies have read the buffer (their global writes may still be in flight)
-                SL_TRACE(7, it);
                 mbar_arrive(&state_empty[sb]);
             }
             __syncwarp();
@@ -312,7 +301,6 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
     uint32_t phase = 0;
     for (int it = 0;; ++it) {
         mbar_wait(&full[stage], phase);
-        if (ct == 0) SL_TRACE(3, it);
         const int tile = tile_q[it & (SL_TQ - 1)];
         const int sb = it % NSB;
         const uint32_t spar = (uint32_t)((it / NSB) & 1);
@@ -435,9 +423,7 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
         }
 
         // ---- update the stored sums (A5) in place in the state buffer, then A4 ----
-        if (ct == 0) SL_TRACE(4, it);
         if constexpr (!IS_F32) mbar_wait(&state_full[sb], spar);
-        if (ct == 0) SL_TRACE(5, it);
         RED a[ROWS][V];
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
@@ -503,7 +489,6 @@ k_slide_bulk(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ D
                     store_vec<float, V>(reinterpret_cast<float *>(st + SM.off_map) + (size_t)(k * n_which + map_slot[w]) * TP + (size_t)ct * V, o[w]);
         }
         fence_async_smem();                                // generic-proxy writes before the store warp's bulk copies read them
-        if (ct == 0) SL_TRACE(6, it);
         if (ct == 0) out_tile[sb] = tile;
         mbar_arrive(&out_full[sb]);
     }
@@ -520,16 +505,9 @@ cudaError_t launch_slide_n(const void *tmap, const DemodParams &p, const SlideSh
     constexpr bool IS_F32 = std::is_same<ACC, float>::value;
     const SlideSmem SM(sh.seg, sh.kc, sh.stages, sh.nsb, ROWS, IS_INT ? 4 : 8, PART, IS_F32, n_map_rows);
     auto kern = k_slide_bulk<T, ACC, ROWS, PART>;
-    static int smem_set_dev[64] = {0};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int &smem_set = smem_set_dev[dev & 63];
-    cudaError_t e = cudaSuccess;
-    if (SM.total + 128 > smem_set) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
-        if (e != cudaSuccess) return e;
-        smem_set = SM.total + 128;
-    }
+    static std::atomic<int> smem_ok[64];                  // per instantiation (qld_allow_max_smem)
+    cudaError_t e = qld_allow_max_smem(kern, smem_ok);
+    if (e != cudaSuccess) return e;
     const int n_tiles = (int)((p.HW + SL_TP - 1) / SL_TP);
     cudaLaunchConfig_t lc;
     memset(&lc, 0, sizeof lc);
@@ -537,9 +515,20 @@ cudaError_t launch_slide_n(const void *tmap, const DemodParams &p, const SlideSh
     lc.blockDim = dim3(SL_THREADS);
     lc.dynamicSmemBytes = (size_t)SM.total + 128;
     lc.stream = st;
+    // The three rotating tile counters are safe under the dependent launch only while launch w + 2 cannot start before launch w has
+    // claimed its last tile (w + 2 zeroes the counter w counts on).  That holds when a CTA fills more than half of an SM's shared
+    // memory -- then launch w + 1 becomes resident, and lets w + 2 go, only as the CTAs of w exit, and a CTA exits after its last
+    // claim -- and when no tile is claimed through the counter at all (n_tiles <= grid: every CTA owns the tile of its index).
+    // Any other shape (small forced tiles) is launched in plain stream order.
+    static std::atomic<int> smem_per_sm[64];
+    int dev = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64) per_sm = smem_per_sm[dev].load(std::memory_order_relaxed);
+    if (per_sm == 0 && cudaDeviceGetAttribute(&per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev) == cudaSuccess && dev >= 0 && dev < 64)
+        smem_per_sm[dev].store(per_sm, std::memory_order_relaxed);
+    const bool overlap_ok = n_tiles <= (int)lc.gridDim.x || (per_sm > 0 && 2 * (lc.dynamicSmemBytes + 1024) > (size_t)per_sm);
     cudaLaunchAttribute at;
     at.id = cudaLaunchAttributeProgrammaticStreamSerialization;    // may overlap the tail of the launch before it (see the kernel)
-    at.val.programmaticStreamSerializationAllowed = 1;
+    at.val.programmaticStreamSerializationAllowed = overlap_ok ? 1 : 0;
     lc.attrs = &at;
     lc.numAttrs = 1;
     return cudaLaunchKernelEx(&lc, kern, *reinterpret_cast<const CUtensorMap *>(tmap), p, sh, n_map_rows, counter, counter_next);
@@ -627,10 +616,3 @@ cudaError_t qld_launch_slide_bulk(int dtype, int kind, int rows, const void *tma
     default: return cudaErrorInvalidValue;
     }
 }
-
-#ifdef QLD_SL_TRACE
-extern "C" int qld_sl_trace_read(unsigned long long *out, int n)
-{
-    return (int)cudaMemcpyFromSymbol(out, g_sl_trace, sizeof(unsigned long long) * (size_t)n);
-}
-#endif

@@ -587,18 +587,9 @@ cudaError_t launch_stream_n(const void *tmap, const DemodParams &p, const Stream
     constexpr bool IS_INT = std::is_same<ACC, int>::value;
     const StreamSmem SM(sh.seg, sh.kc, sh.stages, ROWS, red_bytes_for(sh.seg, V * (int)sizeof(T), ROWS, V, IS_INT, NWT, NEPI));
     auto kern = k_demod_stream<T, ACC, ROWS, V, NWT, NEPI, PART>;
-    // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
-    // function, and re-setting it on every launch costs a driver call)
-    static int smem_set_dev[64] = {0};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int &smem_set = smem_set_dev[dev & 63];
-    cudaError_t e = cudaSuccess;
-    if (SM.total + 128 > smem_set) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 128);
-        if (e != cudaSuccess) return e;
-        smem_set = SM.total + 128;
-    }
+    static std::atomic<int> smem_ok[64];                  // per instantiation (qld_allow_max_smem)
+    cudaError_t e = qld_allow_max_smem(kern, smem_ok);
+    if (e != cudaSuccess) return e;
     const int64_t row_bytes = p.HW * (int64_t)sizeof(T);
     const int n_tiles = (int)((row_bytes + sh.seg - 1) / sh.seg);
     kern<<<n_tiles < n_sms ? n_tiles : n_sms, 32 * (NWT + 1 + NEPI), SM.total + 128, st>>>(*reinterpret_cast<const CUtensorMap *>(tmap), p, sh, counter, counter_next);

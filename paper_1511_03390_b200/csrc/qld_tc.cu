@@ -199,13 +199,6 @@ __global__ void k_spectrum_digits(int N, int q_lo, int n_bins, int n_steps, int8
 // ---------------------------------------------------------------------------------------------------
 // the contraction kernel
 // ---------------------------------------------------------------------------------------------------
-#ifdef QLD_TC_TRACE   // development builds only: per-chunk time stamps of CTA 0 (producer issue, data landed, MMAs issued)
-__device__ unsigned long long g_tc_trace[3 * 1024];
-__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TC_TRACE(kind, n) do { if (blockIdx.x == 0 && (n) < 1024) g_tc_trace[(kind) * 1024 + (n)] = gtime(); } while (0)
-#else
-#define TC_TRACE(kind, n) do { } while (0)
-#endif
 // sqrt of a non-negative double to a few units in 1e-14: fp32 reciprocal square root of the rounded argument, one Newton
 // step in fp64 (the library routine is correctly rounded but several times longer; the result is stored as fp32)
 __device__ __forceinline__ double sqrt_newton(double x)
@@ -300,9 +293,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
         // Tiles are claimed from a global counter: under HBM contention SMs progress at very different rates
         // (ncu: fastest SM done in 56 % of the time with a static split), so the split must be dynamic.
         if (lane == 0) {
-            int stage = 0, it = 0, n_issued = 0;
+            int stage = 0, it = 0;
             uint32_t phase = 0;
-            (void)n_issued;
             for (;; ++it) {
                 int tile = (int)atomicAdd(p.tile_counter, 1u);
                 if (tile >= n_tiles) tile = -1;
@@ -317,7 +309,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                 const uint64_t hint = 0x12F0000000000000ull;     // evict first: every sample is read once
                 for (int c = 0; c < n_chunks; ++c) {
                     mbar_wait(&empty[stage], phase ^ 1);
-                    TC_TRACE(0, n_issued); ++n_issued;
                     unsigned char *dst = sA + stage * SM.a_stage;
                     if (use4d && (c + 1) * KC <= n_full) {
                         // one 4-D box {128 B, 8 frames, T spans, KC/8 groups}: the TMA walks the T adjacent spans of a
@@ -351,9 +342,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
         const bool leader = elect_one();
         const uint32_t sA0 = smem_u32(sA), sB0 = smem_u32(sB);
         const uint32_t a_sbo = (uint32_t)(T * GRP * SUB_BYTES);
-        int stage = 0, n_done = 0;
+        int stage = 0;
         uint32_t phase = 0;
-        (void)n_done;
         for (int it = 0;; ++it) {
             const int buf = it & 1;                           // hand-off slot (tfull / tbuf_tile), always alternating
             const int abuf = NBUF == 2 ? buf : 0;             // accumulator set
@@ -373,7 +363,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
             for (int c = 0; c < n_chunks; ++c) {
                 if (c > 0) mbar_wait(&full[stage], phase);
                 tc_fence_after();
-                if (leader) TC_TRACE(1, n_done);
                 // descriptors of this stage: A MN-major with 128-byte swizzle (rows of 128 pixel bytes, 8-frame atoms T KB
                 // apart = SBO); B K-major without swizzle (K halves 128 B apart = LBO, 8-column groups 256 B apart = SBO).
                 // The start address sits in the low 14 bits (units of 16 bytes): span t / K step ks are plain additions.
@@ -414,9 +403,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                         tc_commit(&tfull[buf]);               // arrival 1 of 2: the accumulators are complete
                         mbar_arrive(&tfull[buf]);             // arrival 2 of 2: releases tbuf_tile[buf]
                     }
-                    TC_TRACE(2, n_done);
                 }
-                ++n_done;
                 __syncwarp();
                 if (++stage == STAGES) { stage = 0; phase ^= 1; }
             }
@@ -426,6 +413,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
         const int q = warp & 3;                         // TMEM lane quarter this warp may read
         const int eset = (warp - 2) >> 2;               // which quartet of epilogue warps: it drains spans t % EPI_SETS == eset
         const int m = q * 32 + lane;                    // accumulator row = byte index inside the 128-byte span
+        int span_seq = 0;                               // search mode: spans this CTA has reduced so far (both quartets count alike)
         for (int it = 0; MODE == 2 || eset < T; ++it) { // a quartet without spans (T < EPI_SETS) has nothing to do
             const int buf = it & 1;
             const int abuf = NBUF == 2 ? buf : 0;
@@ -456,11 +444,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                     if (writer && !p.spec_first) prev_amp = __ldg(p.spec_amp + pixel);
                     uint32_t rn[16];
                     tc_ld16(taddr + eset * 16, rn);                             // software pipeline: the next group's columns are in flight
-#ifdef QLD_SPEC_PROBE
-                    for (int g = eset; g < QLD_SPEC_PROBE; g += EPI_SETS) {
-#else
                     for (int g = eset; g < NC / 16; g += EPI_SETS) {
-#endif
                         uint32_t r[16];
                         tc_wait_ld();
 #pragma unroll
@@ -494,7 +478,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) k_demod_tc(const __grid_constan
                         const int oq = __shfl_xor_sync(0xffffffffu, best_q, 1);
                         if (ob > best || (ob == best && oq < best_q)) { best = ob; best_q = oq; }
                     }
-                    double *sx = spec_x + (size_t)(it & 1) * 192;              // 128 doubles + 128 ints per buffer
+                    // 128 doubles + 128 ints per buffer; the buffers alternate from span to span (not from tile to tile: with one
+                    // barrier per span, quartet 1 would otherwise write span t + 1 into the buffer quartet 0 still reads for span t)
+                    double *sx = spec_x + (size_t)(span_seq++ & 1) * 192;
                     if (eset == 1) { sx[m] = best; reinterpret_cast<int *>(sx + 128)[m] = best_q; }
                     named_barrier(2, 128 * EPI_SETS);
                     if (eset == 0) {
@@ -643,18 +629,9 @@ cudaError_t launch_tc_shape(const CUtensorMap *tmaps, const TcParams &p, const T
 {
     const TcSmem SM(NC, sh.T, sh.stages, sh.kc);
     auto kern = k_demod_tc<NC, BYTES, TT, KCC, MODE>;
-    // raise the kernel's dynamic shared-memory limit once per size (per instantiation; the attribute is per device
-    // function, and re-setting it on every launch costs a driver call)
-    static int smem_set_dev[64] = {0};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    int &smem_set = smem_set_dev[dev & 63];
-    cudaError_t e = cudaSuccess;
-    if (SM.total + 1024 > smem_set) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SM.total + 1024);
-        if (e != cudaSuccess) return e;
-        smem_set = SM.total + 1024;
-    }
+    static std::atomic<int> smem_ok[64];                  // per instantiation (qld_allow_max_smem)
+    cudaError_t e = qld_allow_max_smem(kern, smem_ok);
+    if (e != cudaSuccess) return e;
     const int n_sub = (int)((p.row_bytes + SUB_BYTES - 1) / SUB_BYTES);
     const int n_tiles = (n_sub + sh.T - 1) / sh.T;
     const int grid = n_tiles < n_sms ? n_tiles : n_sms;
@@ -811,10 +788,3 @@ cudaError_t qld_launch_demod_tc(const void *tmaps, const TcParams &p, int n_sms,
     }
     return cudaErrorInvalidValue;
 }
-
-#ifdef QLD_TC_TRACE
-extern "C" int qld_tc_trace_read(unsigned long long *out, int n)
-{
-    return (int)cudaMemcpyFromSymbol(out, g_tc_trace, sizeof(unsigned long long) * (size_t)n);
-}
-#endif

@@ -862,3 +862,40 @@ def test_many_hops_queued_behind_a_busy_gpu(Q, oracle, mode, ring_hops):
         # each entry that differs (by one unit, on a rint tie) moves a sum by at most one sample value
         assert np.abs(gI - oI).max() <= 4095 * int((gs != os_).sum()) and np.abs(gQ - oQ).max() <= 4095 * int((gc != oc).sum())
     ctx.destroy()
+
+
+def test_two_host_threads_with_different_tile_shapes(Q, oracle):
+    """include/qld.h: distinct contexts are independent across host threads.  Two threads each build their own contexts, one
+    walking the tile shapes of k_demod_stream upwards and one downwards (their shared-memory needs differ by a factor of
+    eight), each on a stream of its own; a per-kernel shared-memory limit left too low by the other thread would make a launch
+    fail, a shared counter or table would spoil the maps."""
+    import threading
+    import torch
+    H, W, N = 33, 256, 100
+    ref = {"nu": 0.0937, "phase": 0.3}
+    xs = [_rand_stack(np.random.default_rng(70 + i), N, H, W, np.uint16) for i in range(2)]
+    want = [oracle_maps(oracle, x, ref) for x in xs]
+    errors, seen = [], set()
+
+    def worker(i):
+        try:
+            with torch.cuda.stream(torch.cuda.Stream()):
+                for rep in range(3):
+                    for tile in (STREAM_TILES if i == 0 else STREAM_TILES[::-1]):
+                        ctx = forced(Q, "stream", tile)(H, W, "u16", N, [ref], accum=Q.QLD_ACC_FP32)
+                        ctx.push_frames(xs[i])
+                        ctx.demod(Q.QLD_WHOLE)
+                        ctx.sync()
+                        seen.add(ctx.last_kernel())                  # (a shape the frame cannot take falls back to k_demod_whole)
+                        check_float_maps(_maps(ctx), want[i], what=f"thread {i} tile {tile}")
+                        ctx.destroy()
+        except BaseException as e:                                   # noqa: BLE001 -- handed to the main thread
+            errors.append((i, e))
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    assert "k_demod_stream" in seen, seen
