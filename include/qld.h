@@ -67,7 +67,9 @@ typedef enum {
  *             references (2/sqrt3) sin theta_s in {0, +-1} and 2 cos theta_s in {+-1, +-2} are integers, so TWO exact int32 sums
  *             per reference suffice (2Q = 2B0+B1-B2-2B3-B4+B5, (2/sqrt3) I = B1+B2-B4-B5) instead of three bin
  *             rows: I = (sqrt3/2) row 0, Q = row 1 / 2.  Other references of the context keep their bin rows.  A third less
- *             accumulator traffic in a sliding update.  qld_get_bins then returns those two integer-reference sums.
+ *             accumulator traffic in a sliding update.  qld_get_bins then returns those two integer-reference sums.  A row of
+ *             the compact form collects up to 4N/3 sample values (a bin row N/den): where max_value * (4N/3 + 2) reaches 2^31 the
+ *             references keep their bin rows, and qld_accum_mode reports INT_BINS when none is compact.
  *  FIXED    : fixed-point references R(s) = rint(2^30 * sin/cos(theta_s)) (Q1.30 integers; the table can also
  *             be supplied, qld_set_ref_table_fixed).  I*2^30 = sum_s x_s R_sin(s), Q likewise, exact in int64:
  *             computed on the tcgen05 tensor cores as a [pixel bytes x frames].[frames x reference digits]

@@ -200,9 +200,13 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
     // accumulation mode
     const uint64_t vmax = cfg->max_value ? cfg->max_value : (cfg->dtype == QLD_U8 ? 255u : 65535u);
     // INT_REFS: references with den = 3 or 6 and no phase offset take the two-row integer-reference form
+    // (their weights 2 cos theta_s run through +-2, +-1, +-1 per half period: at most 4N/3 + 2/3 sample values land in a row; a
+    // reference whose two rows could overflow int32 keeps its plain bin rows, whose bound is N/den)
+    const int64_t compact_per_row = (4 * (int64_t)cfg->N + 2) / 3 + 1;
+    const bool compact_fits = (unsigned __int128)vmax * (uint64_t)(compact_per_row + 1) < (1ull << 31);
     auto compact = [&](int k, bool want) {
         const RefPlan &rp = pl->ref[k];
-        return want && (rp.den == 3 || rp.den == 6) && rp.phase == 0.0 && (rp.phase_quarter & 3) == 0;
+        return want && compact_fits && (rp.den == 3 || rp.den == 6) && rp.phase == 0.0 && (rp.phase_quarter & 3) == 0;
     };
     auto bins_rows = [&](int *rows_out, bool want_compact) {
         int rows = 0;
@@ -217,8 +221,8 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         for (int k = 0; k < cfg->K; ++k) {
             const int64_t den = pl->ref[k].den;
             // a difference row takes +x from bin r and -x from bin r+den/2: magnitude bounded by one bin's sum; an
-            // integer-reference row takes every frame with a weight of magnitude <= 2
-            const int64_t per_row = compact(k, want_compact) ? 2 * (int64_t)cfg->N : ((int64_t)cfg->N + den - 1) / den;
+            // integer-reference row: see compact_per_row
+            const int64_t per_row = compact(k, want_compact) ? compact_per_row : ((int64_t)cfg->N + den - 1) / den;
             if ((unsigned __int128)vmax * (uint64_t)(per_row + 1) >= (1ull << 31)) return false;
         }
         return true;
@@ -238,6 +242,11 @@ int make_plan(const qld_config *cfg, Plan *pl, std::string *err)
         if (!all_rational) return bad(QLD_E_UNSUPPORTED, "INT_BINS needs every reference rational (den > 0)");
         if (!bins_rows(&rows, want_compact)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: more than 16 bin rows in total");
         if (!bins_fit(want_compact)) return bad(QLD_E_UNSUPPORTED, "INT_BINS: a bin sum could overflow int32 for this N and max_value");
+        if (want_compact) {                                  // no reference took the compact form: these are plain bins, say so
+            bool any = false;
+            for (int k = 0; k < cfg->K; ++k) any = any || compact(k, true);
+            if (!any) acc = QLD_ACC_INT_BINS;
+        }
     }
     if (acc == QLD_ACC_FIXED && pl->ring) {
         if (cfg->K > 2) return bad(QLD_E_UNSUPPORTED, "FIXED on a ring: at most 2 references");

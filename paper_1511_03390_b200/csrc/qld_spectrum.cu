@@ -34,6 +34,33 @@ __global__ void k_peak_update(const float *amp, int K, int64_t HW, int q0, int f
     bin[p] = q;
 }
 
+constexpr size_t SEARCH_GROUP_BYTES = 64ull << 20;    // digit tiles built at a time by qld_dominant_bin
+
+// the library's own memory pool on the current device (created on first use, kept until exit; nullptr if that fails)
+cudaMemPool_t search_pool()
+{
+    static std::mutex mu;
+    static cudaMemPool_t pools[64] = {nullptr};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!pools[dev]) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+        uint64_t keep = SEARCH_GROUP_BYTES + (1ull << 20);          // what one search takes stays with the pool between calls
+        (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        (void)cudaGetLastError();
+        pools[dev] = pool;
+    }
+    return pools[dev];
+}
+
 }  // namespace
 
 extern "C" int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_t H, int32_t W, int32_t N, int32_t q_lo, int32_t q_hi,
@@ -47,49 +74,52 @@ extern "C" int qld_dominant_bin(const void *frames_device, int32_t dtype, int32_
     if (dtype != QLD_U8 && dtype != QLD_U16 && dtype != QLD_U16_BE) return QLD_E_INVAL;
     if ((HW * bytes) % 16 == 0 && (reinterpret_cast<uintptr_t>(frames_device) & 15) == 0 && N <= 65536) {
         // ---- 32 bins per pass on the tensor cores, arg-max in the epilogue
-        const int n_bins = q_hi - q_lo + 1;
+        const int n_bins = q_hi - q_lo + 1, n_pass = (n_bins + 31) / 32;
         size_t pass_bytes = 0;
-        const size_t dig_bytes = qld_tc_spectrum_digit_bytes(N, n_bins, &pass_bytes);
+        (void)qld_tc_spectrum_digit_bytes(N, n_bins, &pass_bytes);
+        // the digit tiles are built for a group of passes at a time (at most SEARCH_GROUP_BYTES: a long window would otherwise
+        // ask for 4 N^2 bytes at once) and the groups follow each other in stream order through one buffer
+        int group = (int)(SEARCH_GROUP_BYTES / pass_bytes);
+        group = group < 1 ? 1 : (group > n_pass ? n_pass : group);
+        const size_t dig_bytes = (size_t)group * pass_bytes;
         unsigned char *scratch = nullptr;                    // digit tiles + two tile counters
-        // stream-ordered allocation: no device-wide synchronisation on either side of the search; the default pool is told to
-        // keep what it has at synchronisation points (it otherwise returns the block to the driver after every call, which
-        // costs milliseconds now and then)
-        {
-            int dev = 0;
-            cudaMemPool_t pool;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                uint64_t keep = 64ull << 20, cur = 0;
-                if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &cur) == cudaSuccess && cur < keep)
-                    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
+        // stream-ordered allocation from a pool of the library's own (no device-wide synchronisation on either side of the search;
+        // the pool keeps its block between calls; the process's default pool is left as it is)
+        cudaMemPool_t pool = search_pool();
+        if (!pool || cudaMallocFromPoolAsync(reinterpret_cast<void **>(&scratch), dig_bytes + 256, pool, st) != cudaSuccess) {
             (void)cudaGetLastError();
+            scratch = nullptr;                               // no memory for the tiles: the eight-bins-per-pass route below needs far less
         }
-        if (cudaMallocAsync(reinterpret_cast<void **>(&scratch), dig_bytes + 256, st) != cudaSuccess) { (void)cudaGetLastError(); return QLD_E_NOMEM; }
-        int8_t *digits = reinterpret_cast<int8_t *>(scratch);
-        unsigned int *counters = reinterpret_cast<unsigned int *>(scratch + dig_bytes);
-        int rc = QLD_OK;
-        alignas(64) unsigned char tmaps[256];
-        int force[3];
-        qld_tc_spectrum_shape(force);
-        int n_sms = qld_sm_count();
-        if (cudaMemsetAsync(counters, 0, 8, st) != cudaSuccess) rc = QLD_E_CUDA;
-        if (rc == QLD_OK && qld_launch_spectrum_digits(N, q_lo, n_bins, digits, st) != cudaSuccess) rc = QLD_E_CUDA;
-        if (rc == QLD_OK && qld_tc_encode_tmap(tmaps, frames_device, HW * bytes, N, 32 /* 256 columns */, n_sms, force) != cudaSuccess) rc = QLD_E_CUDA;
-        for (int P = 0; rc == QLD_OK && P * 32 < n_bins; ++P) {
-            TcParams p;
-            memset(&p, 0, sizeof p);
-            p.HW = HW; p.row_bytes = HW * bytes; p.N = N; p.bytes = bytes; p.big_endian = dtype == QLD_U16_BE;
-            p.digits = digits + (size_t)P * pass_bytes;
-            p.tile_counter = counters + (P & 1); p.tile_counter_next = counters + ((P + 1) & 1);
-            p.fin.K = 1; p.fin.scale = 1.0;
-            p.spec_amp = amp_max_device; p.spec_bin = bin_device;
-            p.spec_q0 = q_lo + 32 * P; p.spec_nbins = n_bins - 32 * P < 32 ? n_bins - 32 * P : 32; p.spec_first = P == 0;
-            if (qld_launch_demod_tc_spectrum(tmaps, p, n_sms, st) != cudaSuccess) rc = QLD_E_CUDA;
+        if (scratch) {
+            int8_t *digits = reinterpret_cast<int8_t *>(scratch);
+            unsigned int *counters = reinterpret_cast<unsigned int *>(scratch + dig_bytes);
+            int rc = QLD_OK;
+            alignas(64) unsigned char tmaps[256];
+            int force[3];
+            qld_tc_spectrum_shape(force);
+            int n_sms = qld_sm_count();
+            if (cudaMemsetAsync(counters, 0, 8, st) != cudaSuccess) rc = QLD_E_CUDA;
+            if (rc == QLD_OK && qld_tc_encode_tmap(tmaps, frames_device, HW * bytes, N, 32 /* 256 columns */, n_sms, force) != cudaSuccess) rc = QLD_E_CUDA;
+            for (int P = 0; rc == QLD_OK && P < n_pass; ++P) {
+                if (P % group == 0) {
+                    const int bins_here = n_bins - 32 * P < 32 * group ? n_bins - 32 * P : 32 * group;
+                    if (qld_launch_spectrum_digits(N, q_lo + 32 * P, bins_here, digits, st) != cudaSuccess) { rc = QLD_E_CUDA; break; }
+                }
+                TcParams p;
+                memset(&p, 0, sizeof p);
+                p.HW = HW; p.row_bytes = HW * bytes; p.N = N; p.bytes = bytes; p.big_endian = dtype == QLD_U16_BE;
+                p.digits = digits + (size_t)(P % group) * pass_bytes;
+                p.tile_counter = counters + (P & 1); p.tile_counter_next = counters + ((P + 1) & 1);
+                p.fin.K = 1; p.fin.scale = 1.0;
+                p.spec_amp = amp_max_device; p.spec_bin = bin_device;
+                p.spec_q0 = q_lo + 32 * P; p.spec_nbins = n_bins - 32 * P < 32 ? n_bins - 32 * P : 32; p.spec_first = P == 0;
+                if (qld_launch_demod_tc_spectrum(tmaps, p, n_sms, st) != cudaSuccess) rc = QLD_E_CUDA;
+            }
+            cudaFreeAsync(scratch, st);
+            if (cudaStreamSynchronize(st) != cudaSuccess) rc = QLD_E_CUDA;
+            (void)cudaGetLastError();
+            return rc;
         }
-        cudaFreeAsync(scratch, st);
-        if (cudaStreamSynchronize(st) != cudaSuccess) rc = QLD_E_CUDA;
-        (void)cudaGetLastError();
-        return rc;
     }
     int first = 1;
     for (int q0 = q_lo; q0 <= q_hi; q0 += 8) {

@@ -746,7 +746,8 @@ def test_integer_reference_rows(Q, oracle, path, dtype, refs):
         kw["slide_hop"] = hop
         kw["debug_tile"] = ("stream", 512, 16)
     ctx = Q.QLD(H, W, dtype, N, refs, **kw)
-    assert ctx.accum_name() == "INT_REFS"
+    any_compact = any(r["den"] in (3, 6) and not r.get("phase") and not r.get("phase_quarter") for r in refs)
+    assert ctx.accum_name() == ("INT_REFS" if any_compact else "INT_BINS")     # the mode reported is the one in use
     if path in ("slide_bulk", "slide_partial"):
         ctx.debug_set_tile("slide", 1)
     ctx.push_frames(x[:N])
@@ -899,3 +900,27 @@ def test_two_host_threads_with_different_tile_shapes(Q, oracle):
         t.join()
     assert not errors, errors
     assert "k_demod_stream" in seen, seen
+
+
+@pytest.mark.parametrize("N,want", [(16384, "INT_REFS"), (24574, "INT_REFS"), (24575, "INT_BINS"), (32768, "INT_BINS")])
+def test_auto_stays_exact_when_the_compact_rows_could_overflow(Q, oracle, N, want):
+    """AUTO with full-range 16-bit samples and nu = 1/6 on long windows: a compact integer-reference row collects up to 4N/3 + 2/3
+    sample values, so it is taken up to N = 24574 (65535 * (floor((4N + 2) / 3) + 2) < 2^31) and no further; from there the references keep
+    their three difference bins (bound N/6), still exact -- AUTO must not fall to fp32.  Samples at the top of the range, so
+    that a row that did overflow would show."""
+    rng = np.random.default_rng(N)
+    H, W = 2, 16
+    x = rng.integers(65000, 65536, size=(N, H, W)).astype(np.uint16)
+    ref = {"num": 1, "den": 6}
+    ctx = Q.QLD(H, W, "u16", N, [ref])                                   # accum AUTO, max_value unset: 65535
+    assert ctx.accum_name() == want
+    ctx.push_frames(x)
+    ctx.demod(Q.QLD_WHOLE)
+    ctx.sync()
+    assert np.array_equal(ctx.get_bins(0).cpu().numpy(), expected_int_rows(oracle, x, ref, mode=want))
+    check_float_maps(_maps(ctx), oracle_maps(oracle, x, ref), rel=1e-6, what=f"N={N}")
+    ctx.destroy()
+    if want == "INT_BINS":                                               # asked for by name, the compact form degrades the same way
+        ctx = Q.QLD(H, W, "u16", N, [ref], accum=Q.QLD_ACC_INT_REFS)
+        assert ctx.accum_name() == "INT_BINS"
+        ctx.destroy()

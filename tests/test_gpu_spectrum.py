@@ -79,3 +79,18 @@ def test_dominant_bin_many_passes(Q, oracle, H, W, N, dtype, q_lo, q_hi):
     for q in (q_lo, (q_lo + q_hi) // 2, q_hi):
         x[:, : H // 4, : W // 2] = np.clip(x[:, : H // 4, : W // 2].astype(np.int64) // 2 + (hi // 5) * (1 + np.sin(2 * np.pi * q * s / N)), 0, hi - 1).astype(dtype)
     _check(Q, oracle, x, q_lo, q_hi)
+
+
+@pytest.mark.timeout(600, method="thread")
+def test_dominant_bin_long_window_in_groups_of_passes(Q, oracle):
+    """A long window: the digit tiles of a pass take 256 bytes per frame (2 MB at N = 8192), and they are built for at most
+    64 MB worth of passes at a time -- 32 here -- so the 47 passes of bins 1..1500 run as two groups through one buffer; the
+    running arg-max carries across the groups, and bins of the second group must win where they are the strongest."""
+    rng = np.random.default_rng(8192)
+    N, H, W = 8192, 4, 8
+    x = rng.integers(0, 256, size=(N, H, W)).astype(np.uint8)
+    s = np.arange(1, N + 1)[:, None]
+    for col, q in enumerate((3, 700, 1023, 1024, 1025, 1400, 1500, 64)):       # one strong tone per column of the first row
+        x[:, 0, col:col + 1] = np.clip(100 + 80 * np.sin(2 * np.pi * q * s / N + col), 0, 255).astype(np.uint8)
+    bins = _check(Q, oracle, x, 1, 1500)
+    assert list(bins[0]) == [3, 700, 1023, 1024, 1025, 1400, 1500, 64]
