@@ -230,12 +230,47 @@ def load_traffic(workload: str, kernel: str):
     return None
 
 
+READ_CEILING = {}        # filled once per process by measure_read_ceiling()
+
+
+def measure_read_ceiling(env, gib: int = 16, iters: int = 5):
+    """what this GPU sustains on READS alone -- qld_probe_read (a plain read-only sum kernel of the library) over a
+    16 GiB buffer, CUDA events around `iters` launches after 3 untimed ones.  The paths here read every sample once and write
+    almost nothing, so this, not the read+write copy figure of MEASURED_PEAKS.json, is the ceiling they can approach."""
+    torch = env.torch
+    from paper_1511_03390_b200 import qld
+    try:
+        buf = torch.empty(gib << 30, dtype=torch.uint8, device=env.dev)
+    except Exception as e:                                       # noqa: BLE001 -- e.g. many ranks sharing one device
+        READ_CEILING.update({"read_ceiling_GBps": None, "read_ceiling_note": f"not measured: {type(e).__name__}"})
+        return
+    out = torch.zeros(qld.QLD_PROBE_OUT_WORDS, dtype=torch.int32, device=env.dev)
+    for _ in range(3):
+        qld.probe_read(buf, out)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(iters):
+        qld.probe_read(buf, out)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / iters
+    READ_CEILING.update({"read_ceiling_GBps": (gib << 30) / (ms * 1e-3) / 1e9,
+                         "read_ceiling_note": f"qld_probe_read (k_probe_read, read-only sum) over {gib} GiB, mean of {iters} launches, this run"})
+    del buf
+    torch.cuda.empty_cache()
+
+
 def roofline_hbm(algo_bytes: float, ms_per_launch: float, workload: str, kernel: str, notes=None):
     peak, peak_src = load_peaks()
     achieved = algo_bytes / (ms_per_launch * 1e-3) / 1e9
     r = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
          "traffic": load_traffic(workload, kernel), "peak_source": peak_src, "algorithmic_bytes_per_launch": algo_bytes,
          "frac_of_nominal_8TBps": achieved / 8000.0, "kernel": kernel}
+    if READ_CEILING.get("read_ceiling_GBps"):
+        r["read_ceiling_GBps"] = READ_CEILING["read_ceiling_GBps"]
+        r["frac_of_read_ceiling"] = achieved / READ_CEILING["read_ceiling_GBps"]
+        r["read_ceiling_note"] = READ_CEILING["read_ceiling_note"]
     if notes:
         r["note"] = notes
     return r
@@ -620,7 +655,7 @@ def compact(r: dict) -> dict:
     rf = r["roofline"]
     out = {"value": r["value"], "ms_per_step": r["ms_per_step"], "kernel": r["kernel"], "frac": rf["frac"], "achieved_GBps": rf["achieved"],
            "peak_GBps": rf["peak"], "bytes_per_launch": rf["algorithmic_bytes_per_launch"]}
-    for k in ("frac_survey_A5", "survey_A5_bytes_per_launch"):
+    for k in ("frac_survey_A5", "survey_A5_bytes_per_launch", "frac_of_read_ceiling", "read_ceiling_GBps"):
         if k in rf:
             out[k] = rf[k]
     if r.get("parity"):
@@ -649,7 +684,7 @@ def main():
                     "(SURVEY.md 8(a) A5 as literally stated) instead of keeping per-batch partial sums (8(f3), cfg.slide_hop: "
                     "identical results, fewer bytes, and the faster of the two on B200: the default)")
     ap.add_argument("--also", default="default", help="comma list of other workloads to run briefly first, one compact JSON line each "
-                    "(default: cfg2,cfg3,cfg1,f2 when --workload is cfg4 on one GPU; 'none' to skip)")
+                    "(default: cfg2,cfg3,cfg1,cfg0,f2 when --workload is cfg4 on one GPU; 'none' to skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -660,9 +695,11 @@ def main():
         spawn_ranks(args.gpus)                                  # does not return
 
     env = Env(args)
+    if not env.oversubscribed:
+        measure_read_ceiling(env)
     names = args.also
     if names == "default":
-        names = "cfg2,cfg3,cfg1,f2" if (args.workload == "cfg4" and env.world == 1 and args.accum == "auto") else "none"
+        names = "cfg2,cfg3,cfg1,cfg0,f2" if (args.workload == "cfg4" and env.world == 1 and args.accum == "auto") else "none"
     also = {}
     if names != "none":
         for w in [x for x in names.split(",") if x and x != args.workload]:

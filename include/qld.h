@@ -324,6 +324,15 @@ int qld_dominant_bin_static(const void *frames_device, int32_t dtype, int32_t H,
 int64_t qld_dominant_bin_static_bytes(int32_t N, int32_t q_lo, int32_t q_hi);   /* scratch bytes of that search; QLD_E_INVAL (< 0) for a bad range */
 const char *qld_dominant_bin_static_error(void);
 
+/* Measuring stick for the benchmark, not a step of the path (the read-only ceiling; P:181 is why reads are
+ * what matters -- QLD keeps two n^2 arrays beside the frames): loads every 16-byte word of buf_device[0 .. bytes) once (bytes
+ * rounded down to a multiple of 16; the buffer 16-byte aligned, in device memory) and writes one checksum word per CTA to
+ * out_device (QLD_PROBE_OUT_WORDS uint32 of device memory; word b = the sum over CTA b's words of x ^ y ^ z ^ w of each 16-byte
+ * load, mod 2^32).  One launch enqueued on `stream` (cudaStream_t or NULL); time it with events around the call: bytes / time is
+ * the read bandwidth this GPU sustains, the ceiling bench.py quotes beside the copy peak. */
+#define QLD_PROBE_OUT_WORDS 4096
+int qld_probe_read(const void *buf_device, int64_t bytes, uint32_t *out_device, void *stream);
+
 /* Display mapping (the processed 32-bit image "is displayed on the computer monitor"; there is no graphics stack
  * here, the 8-bit image is delivered to device memory; reading G22): lo / hi = smallest / largest non-NaN value
  * of the n floats at map_device, out_device[i] = rint(255 * (x_i - lo) / (hi - lo)) clamped to 0..255 (0 for NaN and

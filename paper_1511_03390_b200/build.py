@@ -9,7 +9,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libqld.so")
-SOURCES = ["qld_api.cu", "qld_kernels.cu", "qld_stream.cu", "qld_slide.cu", "qld_tables.cu", "qld_tc.cu", "qld_cnr.cu", "qld_spectrum.cu", "qld_display.cu", "synth_fill.cu"]
+SOURCES = ["qld_api.cu", "qld_kernels.cu", "qld_stream.cu", "qld_slide.cu", "qld_tables.cu", "qld_tc.cu", "qld_cnr.cu", "qld_spectrum.cu", "qld_display.cu", "qld_probe.cu", "synth_fill.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

@@ -28,7 +28,7 @@ EXPORTS = ["qld_workspace_bytes", "qld_create", "qld_push_frames", "qld_push_fra
            "qld_commit_frames", "qld_push_done", "qld_demod", "qld_get_maps", "qld_get_bins", "qld_read_map", "qld_read_ref_table", "qld_set_ref_tables",
            "qld_set_ref_table_fixed", "qld_read_ref_table_fixed", "qld_get_sums_i64", "qld_counters", "qld_sync", "qld_reset", "qld_destroy", "qld_last_error", "qld_kernel_launches", "qld_accum_mode", "qld_last_kernel", "qld_debug_set_tile",
            "qld_cnr", "qld_dominant_bin", "qld_dominant_bin_static", "qld_dominant_bin_static_bytes", "qld_dominant_bin_static_error",
-           "qld_display_map", "qld_synth_fill"]
+           "qld_display_map", "qld_synth_fill", "qld_probe_read"]
 
 
 class qld_ref(C.Structure):
@@ -104,6 +104,7 @@ def load_library():
     l.qld_debug_set_tile.argtypes = [vp, i, i, i, i]
     l.qld_cnr.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp]
     l.qld_dominant_bin.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
+    l.qld_probe_read.argtypes = [vp, C.c_int64, vp, vp]
     l.qld_dominant_bin_static.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp, vp, vp]
     l.qld_dominant_bin_static_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32]
     l.qld_dominant_bin_static_bytes.restype = C.c_int64
@@ -368,6 +369,21 @@ def dominant_bin(frames, q_lo: int, q_hi: int):
 
 
 QLD_SEARCH_STATIC_BYTES = 4 << 20
+QLD_PROBE_OUT_WORDS = 4096
+
+
+def probe_read(buf, out=None):
+    """qld_probe_read: one read-only pass over the CUDA tensor `buf` on torch's current stream (the read
+    ceiling); returns the per-CTA checksum words (uint32 viewed as int32, [QLD_PROBE_OUT_WORDS]; unused words keep their contents)."""
+    import torch
+    lib = load_library()
+    assert buf.is_cuda and buf.is_contiguous()
+    if out is None:
+        out = torch.zeros(QLD_PROBE_OUT_WORDS, dtype=torch.int32, device=buf.device)
+    rc = lib.qld_probe_read(buf.data_ptr(), buf.numel() * buf.element_size(), out.data_ptr(), torch.cuda.current_stream(buf.device).cuda_stream or 1)
+    if rc != QLD_OK:
+        raise QLDError(rc, "qld_probe_read")
+    return out
 
 
 def dominant_bin_static(frames, q_lo: int, q_hi: int, amp=None, bins=None):
