@@ -218,8 +218,8 @@ class Env:
 
 def load_traffic(workload: str, kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` summaries (profiles/r02_traffic.csv, the DRAM bytes of profiles/r02_ncu_full.md); None if absent."""
-    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    `ncu --set full` summaries (profiles/r03_traffic.csv, the DRAM bytes of profiles/r03_ncu_full.md); None if absent."""
+    tpath = os.path.join(ROOT, "profiles", "r03_traffic.csv")
     try:
         for line in open(tpath).read().splitlines()[1:]:
             w, k, v = line.split(",")
